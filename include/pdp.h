@@ -1,0 +1,183 @@
+/*
+ * pdp.h — C ABI of the B200-native pixel-detector reduction chain.
+ *
+ * The chain is the per-frame processing that arxiv 1903.06838 (Blaj, Chang,
+ * Kenney) recasts as tensor operations:
+ *
+ *   dark subtraction + gain correction      PAPER.md:L41 (Fig. 2), L51
+ *   common-mode correction                  PAPER.md:L55, L63 (Fig. 3)
+ *   photon finding + charge summing         PAPER.md:L59-L83 (Fig. 4, Fig. 5)
+ *   photon counting by division + rounding
+ *   subpixel centroid                       PAPER.md:L89-L95 (Fig. 6)
+ *   summarization (photon lists, photon-
+ *   counting maps, sums)
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels behind this boundary.
+ * There is no CPU fallback: on a machine without an sm_100 device
+ * pdp_create() returns PDP_E_NO_SM100 (or PDP_E_CUDA when no driver/device
+ * exists at all).
+ *
+ * Geometry and notation: a frame is `panels` x `rows` x `cols`
+ * pixels, row-major, panel-major; the linear pixel index inside a frame is
+ *     idx = (p * rows + r) * cols + c.
+ * A row segment is `seg_cols` contiguous columns of one row of one panel;
+ * seg_cols divides cols.  v1 = (raw - pedestal) / gain, c = common-mode
+ * estimate of the segment, v2 = v1 - c.
+ *
+ * All functions return 0 on success and a negative pdp_status on failure.
+ * No function throws; no function allocates on the pdp_process() path.
+ */
+#ifndef PDP_H
+#define PDP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PDP_VERSION 100 /* 0.1.0 */
+
+typedef struct pdp_ctx pdp_ctx; /* opaque; owns device copies of the maps + workspace */
+
+typedef enum pdp_status {
+  PDP_OK = 0,
+  PDP_E_NULL = -1,     /* a required pointer argument is NULL */
+  PDP_E_GEOMETRY = -2, /* non-positive dims, seg_cols does not divide cols, or a
+                          shape the kernels do not support (see pdp_create) */
+  PDP_E_VALUE = -3,    /* non-finite pedestal/gain/threshold, gain == 0,
+                          photon_adu <= 0, unknown cm_mode */
+  PDP_E_BATCH = -4,    /* n_frames < 0 or > max_frames_per_batch */
+  PDP_E_ALIGN = -5,    /* raw batch pointer not 16-byte aligned */
+  PDP_E_CUDA = -6,     /* a CUDA runtime call failed; see pdp_last_error() */
+  PDP_E_NO_SM100 = -7, /* current device is not compute capability 10.x */
+  PDP_E_NOMEM = -8     /* host or device allocation failed in pdp_create */
+} pdp_status;
+
+/* Detector geometry (host struct, copied by pdp_create). */
+typedef struct pdp_geometry {
+  int32_t panels;               /* P >= 1; panels never neighbour each other */
+  int32_t rows;                 /* H >= 1 */
+  int32_t cols;                 /* W >= 2, even */
+  int32_t seg_cols;             /* S: common-mode group = one row x S columns; S | W, S even,
+                                   2 <= S <= 1024 */
+  int32_t max_frames_per_batch; /* sizes the look-back workspace; >= 1 */
+} pdp_geometry;
+
+/* Common-mode estimator (BASELINE.json north_star (a)). */
+typedef enum pdp_cm_mode {
+  PDP_CM_MEDIAN = 0,       /* exact median of the sub-threshold pixels of the segment;
+                              even count -> mean of the two middle values; c = 0 when
+                              fewer than cm_min_count pixels are sub-threshold */
+  PDP_CM_MEAN_GUARDED = 1, /* the paper's estimator: sum(sub-threshold v1) /
+                              max(count, sqrt(seg_cols))  ("sqrt(HW) term") */
+  PDP_CM_NONE = 2          /* c = 0 */
+} pdp_cm_mode;
+
+/* The two noise thresholds of the paper plus the expected
+ * single-photon gain.  All in gain-corrected ADU. */
+typedef struct pdp_params {
+  float seed_adu;       /* T_seed: a pixel can seed only if v2 >  T_seed (strict) */
+  float cm_adu;         /* T_cm:   a pixel samples the background iff |v1| < T_cm (strict) */
+  float photon_adu;     /* E_ph > 0: n = max(0, rint(E / E_ph)), round-half-even */
+  int32_t cm_mode;      /* pdp_cm_mode */
+  int32_t cm_min_count; /* MEDIAN only; 0 -> ceil(sqrt(seg_cols)) */
+} pdp_params;
+
+/* One batch of raw frames: DEVICE pointer, contiguous [n_frames][P][H][W]
+ * uint16, 16-byte aligned.  Caller-owned; only read. */
+typedef struct pdp_batch {
+  const uint16_t *data;
+  int32_t n_frames;
+} pdp_batch;
+
+/* Output buffers: all DEVICE pointers, caller-owned, sized as noted for the
+ * n = n_frames of the batch.  Hits of frame f occupy slots
+ * [f*hit_capacity, f*hit_capacity + min(hit_count[f], hit_capacity)) of the
+ * five hit_* arrays (struct-of-arrays, 20 bytes per hit), ordered by
+ * ascending pixel index.  Slots past the count are left untouched. */
+typedef struct pdp_output {
+  uint32_t hit_capacity;   /* slots per frame; ceil(H/2)*ceil(W/2)*P can never overflow */
+  uint32_t *hit_count;     /* [n]  TRUE number of seeds of the frame (may exceed capacity) */
+  uint32_t *hit_pixel;     /* [n*cap] idx of the seed pixel */
+  float *hit_charge;       /* [n*cap] E = sum of v2 over the in-panel 3x3 window */
+  int32_t *hit_nphot;      /* [n*cap] n = max(0, rint(E/E_ph)) */
+  float *hit_dx;           /* [n*cap] centroid offset along columns, pixel pitches */
+  float *hit_dy;           /* [n*cap] centroid offset along rows */
+  uint32_t *frame_photons; /* [n]  sum of n over ALL seeds of the frame */
+  uint32_t *accum;         /* [P*H*W] accum[idx] += n for every seed; persists across
+                              calls; caller zeroes it when a new run starts */
+  uint32_t *status;        /* 1 word, sticky OR of PDP_STATUS_* bits; caller zeroes */
+} pdp_output;
+
+#define PDP_STATUS_HIT_OVERFLOW 1u /* some frame had more seeds than hit_capacity */
+
+/*
+ * pdp_create — build a context on the CURRENT CUDA device.
+ *   geometry, params : host structs (copied).
+ *   pedestal_host, gain_host : HOST float32 arrays of P*H*W elements (copied to
+ *     the device; the context keeps derived maps, not the host pointers).
+ *   out_ctx : receives the context.
+ * Errors: PDP_E_NULL, PDP_E_GEOMETRY (also: cols or seg_cols odd, seg_cols > 1024,
+ * more than 8 segments per row), PDP_E_VALUE (checked over every map element),
+ * PDP_E_NO_SM100, PDP_E_CUDA, PDP_E_NOMEM.  On error *out_ctx is set to NULL.
+ */
+int pdp_create(const pdp_geometry *geometry, const float *pedestal_host, const float *gain_host,
+               const pdp_params *params, pdp_ctx **out_ctx);
+
+/*
+ * pdp_process — enqueue the whole chain for one batch on `cuda_stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream) and
+ * return without synchronising.  Outputs are valid once the stream has been
+ * synchronised.  n_frames == 0 is a no-op returning 0.  The same context must
+ * not be used from two streams at once (the workspace is shared).
+ * Data-dependent conditions are never errors: hit overflow sets
+ * PDP_STATUS_HIT_OVERFLOW in *status, hit_count[f] still holds the true count,
+ * only the first hit_capacity hits (index order) are stored, frame_photons and
+ * accum still include every hit.
+ * Errors: PDP_E_NULL, PDP_E_BATCH, PDP_E_ALIGN, PDP_E_CUDA.
+ */
+int pdp_process(pdp_ctx *ctx, const pdp_batch *raw_u16_batch, void *cuda_stream,
+                const pdp_output *out);
+
+/*
+ * pdp_process_host — the same chain fed from HOST memory (pinned for real
+ * overlap): the n_frames frames at `raw_host` are copied to the device in
+ * chunks of `chunk_frames` on an internal copy stream into two device buffers
+ * owned by the context (allocated on first use, sized chunk_frames), and each
+ * chunk is processed on `cuda_stream` while the next one is in flight
+ * (BASELINE.json config 4 "streamed from pinned host memory with
+ * double-buffered copies on a side stream").  `out` buffers are DEVICE
+ * pointers sized for all n_frames; chunk_frames <= max_frames_per_batch.
+ * Returns after everything has been enqueued; synchronise `cuda_stream`.
+ */
+int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
+                     int32_t chunk_frames, void *cuda_stream, const pdp_output *out);
+
+/* pdp_set_params — replace thresholds / estimator of an existing context
+ * (host struct, validated as in pdp_create).  Must not race with pdp_process. */
+int pdp_set_params(pdp_ctx *ctx, const pdp_params *params);
+
+/* pdp_destroy — free the context and everything it owns.  NULL is a no-op. */
+int pdp_destroy(pdp_ctx *ctx);
+
+/* Number of kernel launches (ours, not memsets/copies) the last pdp_process /
+ * pdp_process_host call on this context enqueued. */
+int pdp_last_launch_count(const pdp_ctx *ctx);
+
+/* Debug/diagnostic: copy the per-segment common-mode estimates of the last
+ * pdp_process call into `cm_device` (DEVICE float32,
+ * [n_frames][P][H][W/seg_cols]).  Only valid when the context was told to keep
+ * them with pdp_keep_common_mode(ctx, 1) before the call (off by default: it
+ * adds 4*W/S bytes per row of HBM writes). */
+int pdp_keep_common_mode(pdp_ctx *ctx, int32_t enable);
+int pdp_get_common_mode(pdp_ctx *ctx, float *cm_device, int64_t n_floats, void *cuda_stream);
+
+const char *pdp_strerror(int code);
+const char *pdp_last_error(const pdp_ctx *ctx); /* "" when none; ctx may be NULL */
+int pdp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDP_H */

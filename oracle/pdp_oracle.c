@@ -1,0 +1,247 @@
+/*
+ * pdp_oracle.c — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of the pixel-detector reduction chain of
+ * arxiv 1903.06838, step by step in the paper's order.  It shares
+ * no code with the CUDA path (paper_1903_06838_b200/csrc) and may only be
+ * called from tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs.
+ *
+ * Steps (DESIGN.md §3 lists every reading "R<n>" of a silent/ambiguous spot):
+ *   O1  d  = raw - dark                     PAPER.md:L41 (Fig. 2), L51
+ *   O2  v1 = d / gain                       PAPER.md:L51 "Subtraction and division"
+ *   O3  common mode c of a group: pixels without signal (|v1| < T_cm) are
+ *       segmented, counted, their signal summed
+ *         MEAN_GUARDED: c = sum / max(count, sqrt(G))     PAPER.md:L55 (R4: form of the
+ *                                                          sqrt(HW) guard, G = group size)
+ *         MEDIAN:       c = median of the segmented pixels (BASELINE.json north_star (a));
+ *                       even count -> mean of the two middle values, c = 0 below
+ *                       cm_min_count (R6)
+ *       group = one row x seg_cols columns ("row ... by reshaping")
+ *   O4  v2 = v1 - c ("subtracted from the input signal")
+ *   O5  seed: v2 > T_seed and strict 3x3 local maximum, ties to the lower linear
+ *       index (north_star (b); "the pixel with the highest signal");
+ *       pixels outside the panel do not exist (zero padding)
+ *   O6  E = sum of v2 over the in-panel 3x3 window
+ *   O7  n = max(0, rint(E / E_ph)), half-to-even
+ *   O8  dx = sum(dc * v2) / E, dy = sum(dr * v2) / E, in pixel pitches, 0 if E <= 0
+ *                                                         PAPER.md:L89, L95
+ *   O9  hit list ordered by pixel index
+ *   O10 frame_photons = sum n ; accum[idx] += n
+ *   OF  fragile flags: which decisions sit within `band` ADU of a threshold
+ *       (BASELINE.json: "pixels whose fp64 value lies within 1e-4 ADU of a
+ *       threshold; these are counted and reported")
+ *
+ * Pins (tests/test_oracle_pins.py, tests/golden/): hand-worked fixtures,
+ * numpy.median / numpy.mean on the masked subset, brute-force seed enumeration
+ * on 8x8 frames with an independently written rule, charge conservation, the
+ * erf closed form of the 3x3 centroid, noise-only frames, list invariants.
+ * PARITY UNPINNED against the paper itself: PAPER.md prints no input/output
+ * values for any step, and the form of the sqrt guard (R4) comes from a missing
+ * figure; see DESIGN.md §3.
+ *
+ * Build: gcc -O2 -std=c11 -fopenmp -shared -fPIC pdp_oracle.c -o libpdp_oracle.so -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_CM_MEDIAN 0
+#define ORACLE_CM_MEAN_GUARDED 1
+#define ORACLE_CM_NONE 2
+
+#define FRAGILE_F1 1u /* pixel lies in a segment whose CM mask is within band of flipping */
+#define FRAGILE_F2 2u /* |v2 - T_seed| < band */
+#define FRAGILE_F3 4u /* near-tie with a 3x3 neighbour while near/above T_seed */
+#define FRAGILE_F4 8u /* seed whose E/E_ph is within band of a rounding boundary */
+
+typedef struct {
+  int32_t panels, rows, cols, seg_cols;
+} oracle_geometry;
+
+typedef struct {
+  double seed_adu, cm_adu, photon_adu;
+  int32_t cm_mode, cm_min_count; /* cm_min_count 0 -> ceil(sqrt(seg_cols)) */
+  double band;                   /* fragile band in ADU (1e-4) */
+} oracle_params;
+
+static int cmp_double(const void *a, const void *b) {
+  double x = *(const double *)a, y = *(const double *)b;
+  return (x > y) - (x < y);
+}
+
+/* O3: common-mode estimate of one group of S values. */
+static double common_mode(const double *v1, int S, const oracle_params *prm, double *scratch,
+                          int *fragile_mask) {
+  int k = 0;
+  double sum = 0.0;
+  *fragile_mask = 0;
+  for (int j = 0; j < S; ++j) {
+    double a = fabs(v1[j]);
+    if (fabs(a - prm->cm_adu) < prm->band) *fragile_mask = 1;
+    if (a < prm->cm_adu) { /* "pixel signal smaller than 3 sigma", two-sided (L63) */
+      scratch[k++] = v1[j];
+      sum += v1[j];
+    }
+  }
+  if (prm->cm_mode == ORACLE_CM_NONE) {
+    *fragile_mask = 0;
+    return 0.0;
+  }
+  if (prm->cm_mode == ORACLE_CM_MEAN_GUARDED) {
+    double guard = sqrt((double)S);
+    double denom = (double)k > guard ? (double)k : guard;
+    return sum / denom;
+  }
+  /* MEDIAN */
+  int min_count = prm->cm_min_count > 0 ? prm->cm_min_count : (int)ceil(sqrt((double)S));
+  if (k < min_count || k == 0) return 0.0;
+  qsort(scratch, (size_t)k, sizeof(double), cmp_double);
+  if (k & 1) return scratch[(k - 1) / 2];
+  return 0.5 * (scratch[k / 2 - 1] + scratch[k / 2]);
+}
+
+/*
+ * One frame.  Outputs (any may be NULL): v2_out[Npix], cm_out[Npix/seg_cols],
+ * fragile_out[Npix] (OR of FRAGILE_* bits); hit arrays of `hit_capacity` slots.
+ * Returns the TRUE number of seeds (may exceed hit_capacity; only the first
+ * hit_capacity are stored).  photons_out receives sum of n over all seeds.
+ * accum (may be NULL) gets += n at every seed.
+ */
+int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const float *gain,
+                         const oracle_params *prm, const uint16_t *raw, double *v2_out,
+                         double *cm_out, uint8_t *fragile_out, int64_t hit_capacity,
+                         uint32_t *hit_pixel, double *hit_charge, int32_t *hit_nphot,
+                         double *hit_dx, double *hit_dy, uint64_t *photons_out, uint32_t *accum) {
+  const int P = g->panels, H = g->rows, W = g->cols, S = g->seg_cols;
+  const int64_t npix = (int64_t)P * H * W;
+  double *v2 = (double *)malloc((size_t)npix * sizeof(double));
+  double *scratch = (double *)malloc((size_t)S * sizeof(double));
+  uint8_t *frag = (uint8_t *)calloc((size_t)npix, 1);
+  if (!v2 || !scratch || !frag) {
+    free(v2);
+    free(scratch);
+    free(frag);
+    return -1;
+  }
+  /* O1, O2 */
+  for (int64_t i = 0; i < npix; ++i) {
+    double d = (double)raw[i] - (double)pedestal[i];
+    v2[i] = d / (double)gain[i];
+  }
+  /* O3, O4 */
+  const int nseg = W / S;
+  for (int p = 0; p < P; ++p)
+    for (int r = 0; r < H; ++r)
+      for (int s = 0; s < nseg; ++s) {
+        int64_t base = ((int64_t)p * H + r) * W + (int64_t)s * S;
+        int fmask;
+        double c = common_mode(v2 + base, S, prm, scratch, &fmask);
+        if (cm_out) cm_out[((int64_t)p * H + r) * nseg + s] = c;
+        for (int j = 0; j < S; ++j) {
+          v2[base + j] -= c;
+          if (fmask) frag[base + j] |= FRAGILE_F1;
+        }
+      }
+  /* O5..O10 */
+  int64_t count = 0;
+  uint64_t photons = 0;
+  for (int p = 0; p < P; ++p)
+    for (int r = 0; r < H; ++r)
+      for (int c = 0; c < W; ++c) {
+        int64_t i = ((int64_t)p * H + r) * W + c;
+        double x = v2[i];
+        if (fabs(x - prm->seed_adu) < prm->band) frag[i] |= FRAGILE_F2;
+        int near_seed = x > prm->seed_adu - prm->band;
+        int is_seed = x > prm->seed_adu;
+        double E = 0.0, sx = 0.0, sy = 0.0;
+        for (int dr = -1; dr <= 1; ++dr)
+          for (int dc = -1; dc <= 1; ++dc) {
+            int rr = r + dr, cc = c + dc;
+            if (rr < 0 || rr >= H || cc < 0 || cc >= W) continue; /* no such pixel */
+            int64_t q = ((int64_t)p * H + rr) * W + cc;
+            double y = v2[q];
+            E += y;
+            sx += (double)dc * y;
+            sy += (double)dr * y;
+            if (q == i) continue;
+            if (near_seed && fabs(x - y) < prm->band) {
+              frag[i] |= FRAGILE_F3;
+              frag[q] |= FRAGILE_F3;
+            }
+            /* strict maximum; a tie goes to the lower linear index */
+            if (!(x > y || (x == y && i < q))) is_seed = 0;
+          }
+        if (!is_seed) continue;
+        double ratio = E / prm->photon_adu;
+        double rn = nearbyint(ratio); /* default rounding mode: half to even */
+        if (fabs(ratio - (floor(ratio) + 0.5)) * prm->photon_adu < prm->band)
+          frag[i] |= FRAGILE_F4;
+        int32_t n = rn > 0.0 ? (rn > 2147483647.0 ? 2147483647 : (int32_t)rn) : 0;
+        double dx = 0.0, dy = 0.0;
+        if (E > 0.0) {
+          dx = sx / E;
+          dy = sy / E;
+        }
+        if (count < hit_capacity) {
+          if (hit_pixel) hit_pixel[count] = (uint32_t)i;
+          if (hit_charge) hit_charge[count] = E;
+          if (hit_nphot) hit_nphot[count] = n;
+          if (hit_dx) hit_dx[count] = dx;
+          if (hit_dy) hit_dy[count] = dy;
+        }
+        ++count;
+        photons += (uint64_t)n;
+        if (accum) {
+#pragma omp atomic
+          accum[i] += (uint32_t)n; /* integer add: order-independent */
+        }
+      }
+  if (photons_out) *photons_out = photons;
+  if (v2_out) memcpy(v2_out, v2, (size_t)npix * sizeof(double));
+  if (fragile_out) memcpy(fragile_out, frag, (size_t)npix);
+  free(v2);
+  free(scratch);
+  free(frag);
+  return count;
+}
+
+/*
+ * A batch of frames, frames distributed over `threads` OpenMP threads
+ * (frames are independent units, PAPER.md:L51 minibatch dimension).  Hit arrays
+ * are [n_frames][hit_capacity]; hit_count[n_frames] holds true counts;
+ * frame_photons[n_frames]; accum[Npix] += n of EVERY seed (also those past
+ * hit_capacity; integer atomic adds, so the thread schedule cannot change the
+ * result); fragile_out [n_frames][Npix]
+ * and cm_out [n_frames][Npix/seg_cols] optional.  Returns 0, or -1 on
+ * allocation failure.
+ */
+int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const float *gain,
+                     const oracle_params *prm, const uint16_t *raw, int32_t n_frames,
+                     int32_t threads, int64_t hit_capacity, int64_t *hit_count,
+                     uint32_t *hit_pixel, double *hit_charge, int32_t *hit_nphot, double *hit_dx,
+                     double *hit_dy, uint64_t *frame_photons, uint32_t *accum, double *cm_out,
+                     uint8_t *fragile_out) {
+  const int64_t npix = (int64_t)g->panels * g->rows * g->cols;
+  const int64_t nsegs = npix / g->seg_cols;
+  int failed = 0;
+  if (threads < 1) threads = 1;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads)
+  for (int32_t f = 0; f < n_frames; ++f) {
+    uint64_t ph = 0;
+    int64_t off = (int64_t)f * hit_capacity;
+    int64_t cnt = pdp_oracle_frame(
+        g, pedestal, gain, prm, raw + (int64_t)f * npix, NULL, cm_out ? cm_out + f * nsegs : NULL,
+        fragile_out ? fragile_out + f * npix : NULL, hit_capacity, hit_pixel + off,
+        hit_charge + off, hit_nphot + off, hit_dx + off, hit_dy + off, &ph, accum);
+    if (cnt < 0) {
+#pragma omp atomic write
+      failed = 1;
+      cnt = 0;
+    }
+    hit_count[f] = cnt;
+    frame_photons[f] = ph;
+  }
+  return failed ? -1 : 0;
+}
