@@ -1,0 +1,189 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Integers bit-exact except oracle-flagged fragile pixels (counted), floats within
+1e-4 + 1e-4*|ref| (tests/compare.py)."""
+import dataclasses
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from tests.compare import compare
+
+pytestmark = pytest.mark.gpu
+
+if not torch.cuda.is_available():  # collected everywhere, run only where a GPU exists
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+from paper_1903_06838_b200 import binding, build, synth  # noqa: E402
+
+build.build()
+DEV = "cuda"
+
+
+def small(cfg_id, **kw):
+    return dataclasses.replace(synth.CONFIGS[cfg_id], **kw)
+
+
+def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=False, host_chunk=None,
+            n_calls=1):
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
+                          max_frames_per_batch=max(1, raw.shape[0]), pedestal=ped.cpu(), gain=gain.cpu(),
+                          seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu,
+                          cm_mode=cm_mode, cm_min_count=cm_min_count)
+    if keep_cm:
+        ctx.keep_common_mode(True)
+    out = binding.alloc_output(raw.shape[0], cfg.npix, cap or cfg.max_hits, DEV)
+    for _ in range(n_calls):
+        if host_chunk:
+            ctx.process_host(raw.cpu().pin_memory(), out, host_chunk)
+        else:
+            ctx.process(raw, out)
+    torch.cuda.synchronize()
+    res = {k: getattr(out, k).cpu().numpy() for k in
+           ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum", "status")}
+    res["hit_count"] = res["hit_count"].astype(np.int64) & 0xFFFFFFFF
+    res["frame_photons"] = res["frame_photons"].astype(np.int64) & 0xFFFFFFFF
+    if keep_cm:
+        res["cm"] = ctx.common_mode(raw.shape[0]).cpu().numpy()
+    res["launches"] = ctx.last_launch_count
+    ctx.close()
+    return res
+
+
+def oracle_run(oracle, cfg, raw, ped, gain, cm_mode, **kw):
+    return oracle.process(raw.cpu().numpy(), ped.cpu().numpy(), gain.cpu().numpy(), panels=cfg.panels,
+                          rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, seed_adu=cfg.seed_adu,
+                          cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm_mode, threads=os.cpu_count() or 1,
+                          want_fragile=True, **kw)
+
+
+def make(cfg, n):
+    ped, gain = synth.make_maps(cfg, DEV)
+    raw = synth.make_frames(cfg, 0, n, ped, gain)
+    return raw, ped, gain
+
+
+CASES = {
+    "tiny_185x388": (small(0), 6),
+    "epix_704x768": (small(1), 3),
+    "epix_T30": (small(1, seed_adu=30.0), 2),
+    "cspad_3x185x388": (small(2, panels=3), 3),
+    "dense_96x1024": (small(3, rows=96), 3),
+    "lcls2_2x70x512": (small(4, panels=2, rows=70), 3),
+    "ragged_2x11x72_s24": (small(0, panels=2, rows=11, cols=72, seg_cols=24, occupancy=0.02), 5),
+    "narrow_5x60_s30": (small(0, rows=5, cols=60, seg_cols=30, occupancy=0.03), 7),
+    "one_row": (small(0, rows=1, cols=128, seg_cols=64, occupancy=0.03), 4),
+    "single_segment_40x256": (small(4, panels=1, rows=40, cols=256, seg_cols=256), 3),
+}
+
+
+@pytest.mark.parametrize("cm_mode", [0, 1, 2], ids=["median", "mean", "none"])
+@pytest.mark.parametrize("case", list(CASES), ids=list(CASES))
+def test_parity(oracle, case, cm_mode):
+    cfg, n = CASES[case]
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode)
+    o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    print(case, cm_mode, rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 0
+    assert rep.exempt_hits <= max(3, rep.hits_oracle // 200)       # exemptions stay rare
+    assert g["status"][0] == 0 and g["launches"] == 1
+
+
+@pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
+def test_common_mode_values(oracle, cm_mode):
+    """c of every segment against the oracle: the kernel's fp32 order statistic / mean."""
+    cfg, n = small(1, rows=64), 2
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode, keep_cm=True)
+    o = oracle.process(raw.cpu().numpy(), ped.cpu().numpy(), gain.cpu().numpy(), panels=1, rows=cfg.rows,
+                       cols=cfg.cols, seg_cols=cfg.seg_cols, seed_adu=50, cm_adu=20, photon_adu=80,
+                       cm_mode=cm_mode, want_cm=True, want_fragile=True)
+    cm_o = o.cm.reshape(g["cm"].shape)
+    frag_seg = (o.fragile.reshape(n, 1, cfg.rows, cfg.cols // cfg.seg_cols, cfg.seg_cols) & 1).any(-1)
+    err = np.abs(g["cm"] - cm_o)[~frag_seg]
+    assert err.max() < 1e-5, err.max()                # |c_gpu - c_oracle| <= ~7e-6
+
+
+def test_integer_exact_suite(oracle):
+    """Integer pedestals, power-of-two gains, thresholds at x.5: fp32 == fp64, frequent ties,
+    nothing can sit within 1e-4 of a threshold => ZERO exemptions allowed."""
+    rng = np.random.default_rng(3)
+    P, H, W, S, n = 2, 37, 96, 48, 12
+    ped = torch.tensor(rng.integers(900, 1100, (P, H, W)).astype(np.float32))
+    gain = torch.tensor(rng.choice([0.5, 1.0, 2.0], (P, H, W)).astype(np.float32))
+    sig = rng.integers(-6, 7, (n, P, H, W)) * 2 + rng.integers(-3, 4, (n, P, H, W // S)).repeat(S, -1) * 2
+    ph = rng.random((n, P, H, W)) < 0.02
+    sig = sig + ph * rng.choice([40, 60, 60, 80, 150, 250], (n, P, H, W))
+    ph2 = np.roll(ph, 1, -1) | np.roll(ph, 1, -2)
+    sig = sig + ph2 * rng.choice([0, 20, 60], (n, P, H, W))                  # neighbours, ties
+    raw = torch.tensor((ped.numpy() + gain.numpy() * sig).astype(np.uint16))
+    cfg = small(0, panels=P, rows=H, cols=W, seg_cols=S, seed_adu=50.5, cm_adu=20.5, photon_adu=100.0)
+    for cm_mode in (0, 1, 2):
+        g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode)
+        o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+        rep = compare(o, g, panels=P, rows=H, cols=W)
+        print(cm_mode, rep.summary())
+        assert rep.ok, rep.failures[:10]
+        if cm_mode != 1:
+            # exact ties (F3) and exact half-integers (F4) do occur here, and must still match exactly
+            assert rep.exempt_hits == 0 and (o.fragile & 3).max() == 0
+            assert rep.max_err["E"] == 0.0
+        assert rep.hits_oracle > 200
+
+
+def test_overflow_and_empty(oracle):
+    cfg, n = small(0, rows=40, cols=128, seg_cols=64, occupancy=0.03), 3
+    raw, ped, gain = make(cfg, n)
+    full = gpu_run(cfg, raw, ped, gain, 0)
+    cap = int(full["hit_count"].min()) // 2
+    g = gpu_run(cfg, raw, ped, gain, 0, cap=cap)
+    assert g["status"][0] & 1
+    assert np.array_equal(g["hit_count"], full["hit_count"])                 # true counts
+    assert np.array_equal(g["frame_photons"], full["frame_photons"])         # totals over ALL hits
+    assert np.array_equal(g["accum"], full["accum"])
+    assert np.array_equal(g["hit_pixel"][:, :cap], full["hit_pixel"][:, :cap])
+    assert np.array_equal(g["hit_charge"][:, :cap], full["hit_charge"][:, :cap])
+    # zero frames: a no-op
+    ctx = binding.Context(panels=1, rows=40, cols=128, seg_cols=64, max_frames_per_batch=4, pedestal=ped.cpu(),
+                          gain=gain.cpu(), seed_adu=50, cm_adu=20, photon_adu=100)
+    out = binding.alloc_output(1, cfg.npix, 8, DEV)
+    ctx.process(raw[:0], out, n_frames=0)
+    torch.cuda.synchronize()
+    assert ctx.last_launch_count == 0 and int(out.accum.sum()) == 0
+    with pytest.raises(binding.PdpError):
+        ctx.process(raw, out, n_frames=5)                                    # > max_frames_per_batch
+    ctx.close()
+
+
+def test_chunking_determinism_accumulation_and_host_feed(oracle, monkeypatch):
+    cfg, n = small(0, rows=50, cols=128, seg_cols=64, occupancy=0.02), 21
+    raw, ped, gain = make(cfg, n)
+    ref = gpu_run(cfg, raw, ped, gain, 0)
+    again = gpu_run(cfg, raw, ped, gain, 0)
+    for k in ref:
+        assert np.array_equal(ref[k], again[k]), k                           # bit-identical run to run
+    monkeypatch.setenv("PDP_CHUNK_FRAMES", "4")                              # 6 chunks, ragged last one
+    chunked = gpu_run(cfg, raw, ped, gain, 0)
+    for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
+        assert np.array_equal(ref[k], chunked[k]), k
+    monkeypatch.delenv("PDP_CHUNK_FRAMES")
+    twice = gpu_run(cfg, raw, ped, gain, 0, n_calls=2)                       # accum persists across calls
+    assert np.array_equal(twice["accum"], 2 * ref["accum"])
+    host = gpu_run(cfg, raw, ped, gain, 0, host_chunk=8)                     # 3 chunks through the side stream
+    for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
+        assert np.array_equal(ref[k], host[k]), k
+    assert host["launches"] == 3
+    o = oracle_run(oracle, cfg, raw, ped, gain, 0)
+    assert compare(o, ref, panels=1, rows=cfg.rows, cols=cfg.cols).ok
+
+
+def test_occupancy_independence_of_lists(oracle):
+    """Noise-only frames: zero hits, zero accum (sigma far below threshold)."""
+    cfg = small(0, occupancy=0.0)
+    raw, ped, gain = make(cfg, 4)
+    g = gpu_run(cfg, raw, ped, gain, 0)
+    assert g["hit_count"].sum() == 0 and g["accum"].sum() == 0 and g["frame_photons"].sum() == 0
