@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fused reduction chain on BASELINE.json's headline workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--cm-mode median|mean]
+    python bench.py --impl reference ...      # the fp64 oracle on the host cores (reference arm)
+
+A step is one pass of the whole hot path (dark, gain, common mode, seed finding, 3x3 charge sum,
+photon count, centroid, ordered hit lists, per-frame totals, accumulated image) over one batch of
+synthetic frames = ALL frames of the config (configs[1]: 2000 frames of 704x768 uint16, 2.16 GB,
+larger than L2).  Prints ONE JSON line (see DESIGN.md §8 for every field).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1903_06838_b200 import synth  # noqa: E402
+
+METRIC = "frames/s through the fused pixel-detector reduction chain (also Mpixel/s, raw GB/s vs HBM roofline)"
+UNIT = "frames/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "~8 TB/s"
+FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum of pdp_fused_kernel per launch, from the committed
+# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
+NCU_TRAFFIC_BYTES = {}
+CM_MODES = {"median": 0, "mean": 1, "none": 2}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                for line in out.strip().splitlines():
+                    self.rows.append([x.strip() for x in line.split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=10)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 7 for n, v in zip(names, r[3:7]) if v.lower().startswith("active")})
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(cfg, raw_cpu, ped, gain, cm_mode, threads):
+    """The oracle as it stands on `raw_cpu` (numpy uint16 [m, ...]); returns (seconds, result)."""
+    from oracle import pdp_oracle
+    pdp_oracle.build()
+    t0 = time.perf_counter()
+    res = pdp_oracle.process(raw_cpu, ped, gain, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols,
+                             seg_cols=cfg.seg_cols, seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu,
+                             photon_adu=cfg.photon_adu, cm_mode=cm_mode, threads=threads, hit_capacity=4096)
+    return time.perf_counter() - t0, res
+
+
+def workload_name(cfg):
+    return (f"configs[{cfg.cfg_id}] {cfg.name}: {cfg.n_frames} frames of {cfg.panels}x{cfg.rows}x{cfg.cols} uint16, "
+            f"S={cfg.seg_cols}, E_ph={cfg.photon_adu:g}, T_seed={cfg.seed_adu:g}, T_cm={cfg.cm_adu:g}")
+
+
+def run_reference(args, cfg, rank, world):
+    if rank != 0:
+        return
+    threads = os.cpu_count() or 1
+    ped, gain = synth.make_maps(cfg)
+    m = args.ref_frames
+    raw = synth.make_frames(cfg, 0, m, ped, gain).numpy()
+    cm = CM_MODES[args.cm_mode]
+    for _ in range(args.warmup):
+        oracle_sample(cfg, raw[: max(1, m // 4)], ped.numpy(), gain.numpy(), cm, threads)
+    t = 0.0
+    for _ in range(args.steps):
+        dt, _ = oracle_sample(cfg, raw, ped.numpy(), gain.numpy(), cm, threads)
+        t += dt
+    fps = m * args.steps / t
+    line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode,
+                       "sample": f"each step = the first {m} frames of the workload"},
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": f"{m} frames x {args.steps} steps, frames over {threads} OpenMP threads"},
+            "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "mpixel_per_s": fps * cfg.npix / 1e6}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs")
+    ap.add_argument("--frames", type=int, default=0, help="override the frame count (debug; 0 = the config's)")
+    ap.add_argument("--cm-mode", default="median", choices=list(CM_MODES))
+    ap.add_argument("--hit-capacity", type=int, default=0, help="slots per frame (0 = 4x the expected hits)")
+    ap.add_argument("--ref-frames", type=int, default=48, help="frames per step of the reference arm / cpu_baseline")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = synth.CONFIGS[args.config]
+    if args.frames:
+        cfg = cfg.scaled(args.frames)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the product has no CPU path")
+    from paper_1903_06838_b200 import binding, build
+    build.build()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- synthetic workload, generated on the device, each rank its own frames (weak scaling) ----
+    t0 = time.perf_counter()
+    ped, gain = synth.make_maps(cfg, dev)
+    n = cfg.n_frames
+    raw = torch.empty((n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
+    synth.make_frames(cfg, rank * n, n, ped, gain, out=raw)
+    torch.cuda.synchronize()
+    gen_s = time.perf_counter() - t0
+
+    cm = CM_MODES[args.cm_mode]
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
+                          max_frames_per_batch=n, pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu,
+                          cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm)
+    # capacity: a first pass at the no-overflow bound on a few frames sizes the lists (4x the max seen)
+    probe = binding.alloc_output(min(n, 8), cfg.npix, cfg.max_hits, dev)
+    ctx.process(raw[: min(n, 8)], probe)
+    torch.cuda.synchronize()
+    seen = int(probe.hit_count.max())
+    cap = args.hit_capacity or min(cfg.max_hits, max(256, 4 * seen))
+    del probe
+    out = binding.alloc_output(n, cfg.npix, cap, dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        ctx.process(raw, out, stream)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches = 0
+    with ClockSampler(local) as clocks:
+        torch.cuda.synchronize()
+        t_begin = torch.cuda.Event(enable_timing=True)
+        t_end = torch.cuda.Event(enable_timing=True)
+        t_begin.record(stream)
+        for a, b in ev:
+            a.record(stream)
+            step()
+            b.record(stream)
+            launches += ctx.last_launch_count
+        t_end.record(stream)
+        torch.cuda.synchronize()
+    total_ms = t_begin.elapsed_time(t_end)
+    kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    if dist:
+        t = torch.tensor([total_ms], device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        dist.barrier()
+    assert int(out.status.item()) == 0, "hit overflow during the bench"
+    hits_per_frame = float(out.hit_count.to(torch.float64).mean().item())
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region ----
+    e2e = None
+    try:
+        raw_host = torch.empty(raw.shape, dtype=torch.uint16).pin_memory()
+        raw_host.copy_(raw)
+        hc = torch.empty((n,), dtype=torch.int32).pin_memory()
+        fp = torch.empty((n,), dtype=torch.int32).pin_memory()
+        acc = torch.empty((cfg.npix,), dtype=torch.int32).pin_memory()
+        lists = [torch.empty((n, cap), dtype=dt).pin_memory() for dt in
+                 (torch.int32, torch.float32, torch.int32, torch.float32, torch.float32)]
+        chunk = max(1, min(n, (256 << 20) // (cfg.npix * 2)))      # ~256 MB per copy
+        def e2e_step():
+            ctx.process_host(raw_host, out, chunk, stream)
+            hc.copy_(out.hit_count, non_blocking=True)
+            fp.copy_(out.frame_photons, non_blocking=True)
+            acc.copy_(out.accum, non_blocking=True)
+            for h, d in zip(lists, (out.hit_pixel, out.hit_charge, out.hit_nphot, out.hit_dx, out.hit_dy)):
+                h.copy_(d, non_blocking=True)
+        e2e_step()
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        if dist:
+            t = torch.tensor([e2e_s], device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        d2h = 8 * n + 4 * cfg.npix + 20 * n * cap
+        e2e = {"value": world * n * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * cfg.npix * 2,
+               "d2h_bytes_per_step": d2h, "h2d_gbs": n * cfg.npix * 2 * args.e2e_steps / e2e_s / 1e9,
+               "chunk_frames": chunk, "api": "pdp_process_host (pinned host frames, double-buffered side-stream copies)"}
+    except Exception as exc:  # e.g. the box cannot pin the whole batch
+        e2e = {"value": None, "unit": UNIT, "error": str(exc)[:200]}
+
+    # ---- roofline of the (single) kernel of a step ----
+    alg_bytes = n * (cfg.npix * 2 + hits_per_frame * 20 + 8) + cfg.npix * 8 + cfg.npix * 8
+    k_ms = statistics.mean(kernel_ms)
+    peak, peak_src = measured_peak()
+    achieved = alg_bytes / (k_ms * 1e-3) / 1e9
+    key = f"cfg{cfg.cfg_id}_{args.cm_mode}"
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get(key), "peak_source": peak_src, "kernel": "pdp_fused_kernel",
+                "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes,
+                "raw_gbs": n * cfg.npix * 2 / (k_ms * 1e-3) / 1e9,
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+
+    fps = world * n * args.steps / (total_ms * 1e-3)
+    line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32 dense pass, f64 on seed candidates",
+            "data": "synthetic", "mpixel_per_s": fps * cfg.npix / 1e6,
+            "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode, "hit_capacity": cap,
+                       "hits_per_frame": hits_per_frame, "l2": "inputs larger than L2 (%.2f GB per step)" % (n * cfg.npix * 2 / 1e9),
+                       "sharding": "each rank processes its own full set of frames; no collective on the data path",
+                       "generation_s": gen_s},
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+
+    if rank == 0 and not args.no_cpu_baseline:
+        threads = os.cpu_count() or 1
+        m = min(n, args.ref_frames)
+        sample = raw[:m].cpu().numpy()
+        dt, res = oracle_sample(cfg, sample, ped.cpu().numpy(), gain.cpu().numpy(), cm, threads)
+        line["cpu_baseline"] = {"value": m / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"first {m} frames of the workload, {dt:.1f} s, {threads} OpenMP threads over frames"}
+        # cheap cross-check of the timed run against the oracle on the sample (counts must agree)
+        line["cpu_baseline"]["hit_count_equal"] = bool(
+            (torch.as_tensor(res.hit_count) == out.hit_count[:m].cpu().to(torch.int64)).all())
+    if rank == 0:
+        print(json.dumps(line))
+    ctx.close()
+    if dist:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
