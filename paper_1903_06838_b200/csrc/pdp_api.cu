@@ -9,8 +9,9 @@
 #include <vector>
 
 #include "../../include/pdp.h"
-#include "pdp_fused.cuh"
+#include "pdp_frames.cuh"
 
+using pdp::FParams;
 using pdp::KParams;
 
 namespace {
@@ -24,6 +25,15 @@ struct LaunchPlan {
   uint32_t stage_bytes = 0, off_v1 = 0, off_ctab = 0, off_cand = 0, off_accum = 0, off_misc = 0, smem = 0;
 };
 
+struct FramesPlan {
+  bool ok = false;
+  int R = 0, TR = 0, bands_per_panel = 0, n_bands = 0, threads = 0;
+  uint32_t stage_bytes = 0, smem = 0;
+  uint32_t off_v2h = 0, off_ctab = 0, off_cand = 0, off_wcnt = 0, off_rowcnt = 0, off_rowphot = 0, off_rowbase = 0,
+           off_swh = 0, off_stg = 0, off_pref = 0, off_phot = 0, off_desc = 0, off_bar = 0;
+};
+constexpr int kFramesPerCtaMax = 1024;
+
 }  // namespace
 
 struct pdp_ctx {
@@ -32,12 +42,15 @@ struct pdp_ctx {
   int device = 0, num_sms = 0;
   size_t npix = 0;
   float *d_ped = nullptr, *d_gain = nullptr, *d_K = nullptr, *d_rg = nullptr, *d_npf = nullptr;
+  double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
   float *d_cm = nullptr;  // optional kept common-mode estimates
   int keep_cm = 0;
   int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
+  FramesPlan fplan;
+  int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel (PDP_KERNEL)
   int chunk_frames_override = 0;
   // host-feed state
   uint16_t *d_feed[2] = {nullptr, nullptr};
@@ -126,7 +139,64 @@ bool make_plan(const pdp_geometry &g, size_t smem_limit, LaunchPlan &pl) {
   return false;
 }
 
+// Same choice for the frame-owner kernel (pdp_frames.cuh), whose shared-memory needs differ.
+bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesPlan &pl) {
+  const int S = g.seg_cols, W = g.cols, nseg = W / S;
+  auto al = [](uint32_t x) { return (x + 127u) & ~127u; };
+  for (int R = pdp::kMaxWarps / nseg - 2; R >= 1; --R) {
+    if (R > g.rows) continue;
+    const int TR = R + 2, n_words = R * WPR;
+    if (n_words > pdp::kThreads) continue;
+    uint32_t off = 0;
+    const uint32_t stage = al((uint32_t)TR * W * 2u + 32u);
+    off += stage * pdp::kRing;
+    pl.off_v2h = off;      off = al(off + pdp::kDepth * (uint32_t)TR * W * 2u);
+    pl.off_ctab = off;     off = al(off + pdp::kHist * (uint32_t)TR * nseg * 4u);
+    pl.off_cand = off;     off = al(off + pdp::kDepth * (uint32_t)n_words * 4u);
+    pl.off_wcnt = off;     off = al(off + pdp::kHist * (uint32_t)n_words * 4u);
+    pl.off_rowcnt = off;   off = al(off + pdp::kDepth * (uint32_t)R * 4u);
+    pl.off_rowphot = off;  off = al(off + pdp::kDepth * (uint32_t)R * 4u);
+    pl.off_rowbase = off;  off = al(off + pdp::kHist * (uint32_t)R * 4u);
+    pl.off_swh = off;      off = al(off + pdp::kDepth * (uint32_t)n_words * 4u);
+    pl.off_stg = off;      off = al(off + pdp::kDepth * 8u * (uint32_t)n_words * 4u);
+    pl.off_pref = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
+    pl.off_phot = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
+    pl.off_desc = off;     off = al(off + pdp::kHist * 16u);
+    pl.off_bar = off;      off = al(off + (pdp::kRing + 2 * pdp::kDepth) * 8u + (pdp::kRing + pdp::kDepth) * 4u);
+    if (off > smem_limit) continue;
+    pl.R = R;
+    pl.TR = TR;
+    pl.bands_per_panel = (g.rows + R - 1) / R;
+    pl.n_bands = pl.bands_per_panel * g.panels;
+    pl.threads = std::max(TR * nseg, (n_words + 31) / 32) * 32;
+    pl.stage_bytes = stage;
+    pl.smem = off;
+    pl.ok = true;
+    return true;
+  }
+  return false;
+}
+
 using KernelFn = void (*)(const KParams);
+using FramesFn = void (*)(const FParams);
+
+FramesFn frames_kernel_for(int V, int G) {
+  switch (V * 10 + G) {
+    case 21: return pdp::pdp_frames_kernel<2, 1>;
+    case 22: return pdp::pdp_frames_kernel<2, 2>;
+    case 23: return pdp::pdp_frames_kernel<2, 3>;
+    case 24: return pdp::pdp_frames_kernel<2, 4>;
+    case 41: return pdp::pdp_frames_kernel<4, 1>;
+    case 42: return pdp::pdp_frames_kernel<4, 2>;
+    case 43: return pdp::pdp_frames_kernel<4, 3>;
+    case 44: return pdp::pdp_frames_kernel<4, 4>;
+    case 81: return pdp::pdp_frames_kernel<8, 1>;
+    case 82: return pdp::pdp_frames_kernel<8, 2>;
+    case 83: return pdp::pdp_frames_kernel<8, 3>;
+    case 84: return pdp::pdp_frames_kernel<8, 4>;
+  }
+  return nullptr;
+}
 
 KernelFn kernel_for(int V, int G) {
   switch (V * 10 + G) {
@@ -153,6 +223,7 @@ void free_ctx(pdp_ctx *c) {
   cudaFree(c->d_K);
   cudaFree(c->d_rg);
   cudaFree(c->d_npf);
+  cudaFree(c->d_rg64);
   cudaFree(c->d_lookback);
   cudaFree(c->d_ticket);
   cudaFree(c->d_cm);
@@ -211,7 +282,9 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   // derived dense-pass maps, evaluated in double: K = 2^23 + rint(ped), rg = 1/gain,
   // npf = -(ped - rint(ped))/gain, so that v1 = fma((2^23 + raw) - K, rg, npf)
   std::vector<float> K, rg, npf;
+  std::vector<double> rg64;
   try {
+    rg64.resize(npix);
     K.resize(npix);
     rg.resize(npix);
     npf.resize(npix);
@@ -225,6 +298,7 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     const double pi = std::nearbyint(p), r = 1.0 / g;
     K[i] = (float)(8388608.0 + pi);
     rg[i] = (float)r;
+    rg64[i] = r;
     npf[i] = (float)(-(p - pi) * r);
   }
 
@@ -245,6 +319,16 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     free_ctx(c);
     return cuda_fail(nullptr, e, "cudaFuncSetAttribute");
   }
+  if (make_plan_frames(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan)) {
+    e = cudaFuncSetAttribute(frames_kernel_for(c->plan.V, c->plan.G), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)c->fplan.smem);
+    if (e != cudaSuccess) {
+      free_ctx(c);
+      return cuda_fail(nullptr, e, "cudaFuncSetAttribute(frames)");
+    }
+  }
+  if (const char *s = std::getenv("PDP_KERNEL"))
+    c->kernel_override = !std::strcmp(s, "lookback") ? 1 : (!std::strcmp(s, "frames") ? 2 : 0);
   const size_t mb = npix * sizeof(float);
   const size_t lb = (size_t)geo->max_frames_per_batch * c->plan.n_bands * sizeof(unsigned long long);
   cudaError_t errs[] = {cudaMalloc(&c->d_ped, mb),     cudaMalloc(&c->d_gain, mb),      cudaMalloc(&c->d_K, mb),
@@ -255,6 +339,12 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
       free_ctx(c);
       return cuda_fail(nullptr, x, "cudaMalloc");
     }
+  e = cudaMalloc(&c->d_rg64, npix * sizeof(double));
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_rg64, rg64.data(), npix * sizeof(double), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    free_ctx(c);
+    return cuda_fail(nullptr, e, "cudaMalloc/cudaMemcpy(rg64)");
+  }
   const void *srcs[] = {ped, gain, K.data(), rg.data(), npf.data()};
   float *dsts[] = {c->d_ped, c->d_gain, c->d_K, c->d_rg, c->d_npf};
   for (int i = 0; i < 5; ++i) {
@@ -368,6 +458,39 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   k.off_accum = pl.off_accum;
   k.off_misc = pl.off_misc;
 
+  // Large batches: frame-owner kernel (every CTA owns a frame range, no inter-CTA exchange).
+  // Small batches do not give every SM a frame range: band x chunk items with decoupled look-back.
+  const bool use_frames = c->fplan.ok && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
+  if (use_frames) {
+    const FramesPlan &fpl = c->fplan;
+    FParams f{};
+    f.k = k;
+    f.k.R = fpl.R;
+    f.k.TR = fpl.TR;
+    f.k.bands_per_panel = fpl.bands_per_panel;
+    f.k.n_bands = fpl.n_bands;
+    f.k.stage_bytes = fpl.stage_bytes;
+    f.frames_per_cta_max = kFramesPerCtaMax;
+    f.off_v2h = fpl.off_v2h;
+    f.off_ctab = fpl.off_ctab;
+    f.off_cand = fpl.off_cand;
+    f.off_wcnt = fpl.off_wcnt;
+    f.off_rowcnt = fpl.off_rowcnt;
+    f.off_rowphot = fpl.off_rowphot;
+    f.off_rowbase = fpl.off_rowbase;
+    f.off_swh = fpl.off_swh;
+    f.off_stg = fpl.off_stg;
+    f.off_pref = fpl.off_pref;
+    f.off_phot = fpl.off_phot;
+    f.off_desc = fpl.off_desc;
+    f.off_bar = fpl.off_bar;
+    f.rg64 = c->d_rg64;
+    const int grid_f = std::max(std::min(c->num_sms, n), (n + kFramesPerCtaMax - 1) / kFramesPerCtaMax);
+    frames_kernel_for(pl.V, pl.G)<<<grid_f, fpl.threads, fpl.smem, st>>>(f);
+    PDP_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return PDP_OK;
+  }
   PDP_CUDA(c, cudaMemsetAsync(c->d_lookback, 0, (size_t)n * pl.n_bands * sizeof(unsigned long long), st));
   PDP_CUDA(c, cudaMemsetAsync(c->d_ticket, 0, sizeof(unsigned), st));
   const int grid = std::min(k.n_items, c->num_sms);

@@ -83,52 +83,71 @@ __device__ __forceinline__ float key2f(unsigned k) {
 
 // ----------------------------------------------------------------------------------------------
 // Exact median of the finite entries of b[0..N) across the warp (entries that do not take part
-// are +INF).  n = number of finite entries (warp total, > 0), mean = their mean (pivot guess),
+// are +INF).  n = number of finite entries (warp total, > 0), mean = their mean (first pivot),
 // lim = bound with |b| < lim for every finite entry, adu_per_rank = running estimate of the
 // spacing between order statistics near the median (updated here, carried by the caller from
 // segment to segment; it only steers the pivots, never the result).
 //
-// Method: value-space search with exact warp-wide counts.  Invariant: cl = #(b < lo) <= kl and
-// kh < ch = #(b < hi), where kl = (n-1)/2 and kh = n/2 are the two middle ranks (equal for odd n).
-// Pivots come from local interpolation; every third one bisects the bracket in float-key space so
-// the loop is bounded.  When the bracket holds at most two elements (or has collapsed onto one
-// value) the two order statistics are read off with one min/max pass.
+// Method: value-space search with exact warp-wide counts (FSET + IADD3 per pixel, REDUX across the
+// warp).  Invariant: cl = #(b < lo) <= kl and kh < ch = #(b < hi), where kl = (n-1)/2 and kh = n/2
+// are the two middle ranks (equal for odd n).  Pivots: the mean, then a density step aimed just
+// past the far side of the target, then secants inside the bracket; a key-space bisection every
+// few passes bounds the loop.  When the bracket holds at most two elements (or has collapsed onto
+// one value) the two order statistics are read off with one min/max pass.
 // The result is the fp32 value of the middle element (or the fp32 mean of the two middle
 // elements): it inherits the rounding of the fp32 v1 values, nothing else.
 // ----------------------------------------------------------------------------------------------
+__device__ __forceinline__ float set_lt(float a, float b) {  // 1.0f if a < b else 0.0f (one FSET.BF)
+  float d;
+  asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+
+template <int N>
+__device__ __forceinline__ int warp_count_below(const float (&b)[N], float p) {
+  float c0 = 0.f, c1 = 0.f, c2 = 0.f;  // exact small integers in fp32; three chains for ILP
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const float d = set_lt(b[j], p);
+    if (j % 3 == 0) c0 += d;
+    else if (j % 3 == 1) c1 += d;
+    else c2 += d;
+  }
+  return warp_sum_i(__float2int_rn(c0 + c1 + c2));
+}
+
 template <int N>
 __device__ __forceinline__ float warp_median(const float (&b)[N], int n, float mean, float lim,
                                              float &adu_per_rank) {
   const int kl = (n - 1) >> 1, kh = n >> 1;
-  const float ktarget = 0.5f * (float)(kl + kh) + 0.5f;
   float lo = -lim, hi = lim;
   int cl = 0, ch = n;
+  bool lo_real = false, hi_real = false;
   float p = mean;
-  float q_prev = 0.f;
-  int c_prev = -1;
   for (int it = 0;; ++it) {
-    // keep the pivot strictly inside (lo, hi); fall back to the key-space midpoint
-    if (!(p > lo && p < hi) || (it % 3) == 2) {
-      unsigned a = f2key(lo), z = f2key(hi);
-      p = key2f(a + ((z - a) >> 1));
-      if (!(p > lo)) break;  // hi is the successor of lo: every element of [lo, hi) equals lo
+    // keep the pivot strictly inside (lo, hi); otherwise (and on late odd passes) bisect in key space
+    const bool force = it >= 8 && (it & 1);
+    if (!(p > lo && p < hi) || force) {
+      const float mid = 0.5f * (lo + hi);
+      if (lo_real && hi_real && mid > lo && mid < hi && !force) {
+        p = mid;
+      } else {
+        const unsigned a = f2key(lo), z = f2key(hi);
+        p = key2f(a + ((z - a) >> 1));
+        if (!(p > lo)) break;  // hi is the successor of lo: every element of [lo, hi) equals lo
+      }
     }
-    int cnt = 0;
-#pragma unroll
-    for (int j = 0; j < N; ++j) cnt += (b[j] < p) ? 1 : 0;
-    const int cp = warp_sum_i(cnt);
-    if (c_prev >= 0 && abs(cp - c_prev) >= 4) {
-      float est = fabsf(p - q_prev) / (float)abs(cp - c_prev);
-      adu_per_rank = 0.75f * adu_per_rank + 0.25f * est;
-    }
-    q_prev = p;
-    c_prev = cp;
+    const int cp = warp_count_below<N>(b, p);
     if (cp <= kl) {
+      if (lo_real && cp - cl >= 3) adu_per_rank = 0.75f * adu_per_rank + 0.25f * (p - lo) / (float)(cp - cl);
       lo = p;
       cl = cp;
+      lo_real = true;
     } else if (cp > kh) {
+      if (hi_real && ch - cp >= 3) adu_per_rank = 0.75f * adu_per_rank + 0.25f * (hi - p) / (float)(ch - cp);
       hi = p;
       ch = cp;
+      hi_real = true;
     } else {
       // kl < cp <= kh: the pivot separates the two middle elements (even n only)
       lo = hi = p;
@@ -136,7 +155,14 @@ __device__ __forceinline__ float warp_median(const float (&b)[N], int n, float m
       break;
     }
     if (ch - cl <= 2) break;
-    p = p + (ktarget - (float)cp) * adu_per_rank;
+    if (lo_real && hi_real) {
+      // secant inside the bracket, aimed at the middle of the two target ranks
+      p = lo + (hi - lo) * (((float)(kl + kh) * 0.5f + 0.5f - (float)cl) / (float)(ch - cl));
+    } else if (lo_real) {
+      p = lo + ((float)(kh + 2 - cl)) * adu_per_rank;   // step just past the upper target rank
+    } else {
+      p = hi - ((float)(ch - kl + 1)) * adu_per_rank;   // step just below the lower target rank
+    }
   }
   // A = smallest element >= lo (rank cl), B = largest element < hi (rank ch-1)
   float A = __int_as_float(0x7f800000), B = __int_as_float(0xff800000);

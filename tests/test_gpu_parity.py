@@ -26,7 +26,13 @@ def small(cfg_id, **kw):
 
 
 def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=False, host_chunk=None,
-            n_calls=1):
+            n_calls=1, kernel=None):
+    # the library picks its kernel by batch size (frame-owner for large batches, band x chunk with
+    # look-back for small ones); PDP_KERNEL pins one so that both are tested on every case
+    if kernel:
+        os.environ["PDP_KERNEL"] = kernel
+    else:
+        os.environ.pop("PDP_KERNEL", None)
     ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
                           max_frames_per_batch=max(1, raw.shape[0]), pedestal=ped.cpu(), gain=gain.cpu(),
                           seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu,
@@ -48,6 +54,7 @@ def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=F
         res["cm"] = ctx.common_mode(raw.shape[0]).cpu().numpy()
     res["launches"] = ctx.last_launch_count
     ctx.close()
+    os.environ.pop("PDP_KERNEL", None)
     return res
 
 
@@ -78,12 +85,13 @@ CASES = {
 }
 
 
+@pytest.mark.parametrize("kernel", ["frames", "lookback"])
 @pytest.mark.parametrize("cm_mode", [0, 1, 2], ids=["median", "mean", "none"])
 @pytest.mark.parametrize("case", list(CASES), ids=list(CASES))
-def test_parity(oracle, case, cm_mode):
+def test_parity(oracle, case, cm_mode, kernel):
     cfg, n = CASES[case]
     raw, ped, gain = make(cfg, n)
-    g = gpu_run(cfg, raw, ped, gain, cm_mode)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel=kernel)
     o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
     rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
     print(case, cm_mode, rep.summary())
@@ -122,11 +130,11 @@ def test_integer_exact_suite(oracle):
     sig = sig + ph2 * rng.choice([0, 20, 60], (n, P, H, W))                  # neighbours, ties
     raw = torch.tensor((ped.numpy() + gain.numpy() * sig).astype(np.uint16))
     cfg = small(0, panels=P, rows=H, cols=W, seg_cols=S, seed_adu=50.5, cm_adu=20.5, photon_adu=100.0)
-    for cm_mode in (0, 1, 2):
-        g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode)
+    for cm_mode, kernel in ((0, "frames"), (0, "lookback"), (1, "frames"), (2, "frames"), (2, "lookback")):
+        g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
         rep = compare(o, g, panels=P, rows=H, cols=W)
-        print(cm_mode, rep.summary())
+        print(cm_mode, kernel, rep.summary())
         assert rep.ok, rep.failures[:10]
         if cm_mode != 1:
             # exact ties (F3) and exact half-integers (F4) do occur here, and must still match exactly
@@ -135,12 +143,13 @@ def test_integer_exact_suite(oracle):
         assert rep.hits_oracle > 200
 
 
-def test_overflow_and_empty(oracle):
+@pytest.mark.parametrize("kernel", ["frames", "lookback"])
+def test_overflow_and_empty(oracle, kernel):
     cfg, n = small(0, rows=40, cols=128, seg_cols=64, occupancy=0.03), 3
     raw, ped, gain = make(cfg, n)
-    full = gpu_run(cfg, raw, ped, gain, 0)
+    full = gpu_run(cfg, raw, ped, gain, 0, kernel=kernel)
     cap = int(full["hit_count"].min()) // 2
-    g = gpu_run(cfg, raw, ped, gain, 0, cap=cap)
+    g = gpu_run(cfg, raw, ped, gain, 0, cap=cap, kernel=kernel)
     assert g["status"][0] & 1
     assert np.array_equal(g["hit_count"], full["hit_count"])                 # true counts
     assert np.array_equal(g["frame_photons"], full["frame_photons"])         # totals over ALL hits
@@ -162,12 +171,12 @@ def test_overflow_and_empty(oracle):
 def test_chunking_determinism_accumulation_and_host_feed(oracle, monkeypatch):
     cfg, n = small(0, rows=50, cols=128, seg_cols=64, occupancy=0.02), 21
     raw, ped, gain = make(cfg, n)
-    ref = gpu_run(cfg, raw, ped, gain, 0)
-    again = gpu_run(cfg, raw, ped, gain, 0)
+    ref = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
+    again = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
     for k in ref:
         assert np.array_equal(ref[k], again[k]), k                           # bit-identical run to run
     monkeypatch.setenv("PDP_CHUNK_FRAMES", "4")                              # 6 chunks, ragged last one
-    chunked = gpu_run(cfg, raw, ped, gain, 0)
+    chunked = gpu_run(cfg, raw, ped, gain, 0, kernel="lookback")
     for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
         assert np.array_equal(ref[k], chunked[k]), k
     monkeypatch.delenv("PDP_CHUNK_FRAMES")
@@ -187,3 +196,17 @@ def test_occupancy_independence_of_lists(oracle):
     raw, ped, gain = make(cfg, 4)
     g = gpu_run(cfg, raw, ped, gain, 0)
     assert g["hit_count"].sum() == 0 and g["accum"].sum() == 0 and g["frame_photons"].sum() == 0
+
+
+@pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
+def test_many_frames_auto_kernel(oracle, cm_mode):
+    """More frames than SMs: the library picks the frame-owner kernel, every CTA owns ~3 frames
+    and walks all bands for them (ragged last band, two panels)."""
+    cfg, n = small(0, panels=2, rows=43, cols=128, seg_cols=64, occupancy=0.02), 437
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode)
+    o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    print(rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
