@@ -49,7 +49,8 @@ struct pdp_ctx {
   int keep_cm = 0;
   int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
-  FramesPlan fplan;
+  FramesPlan fplan[2];      // [0] without, [1] with the fp16 pre-filter tile
+  int prefilter = 0;        // PDP_PREFILTER=1 selects fplan[1]
   int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel (PDP_KERNEL)
   int chunk_frames_override = 0;
   // host-feed state
@@ -140,7 +141,9 @@ bool make_plan(const pdp_geometry &g, size_t smem_limit, LaunchPlan &pl) {
 }
 
 // Same choice for the frame-owner kernel (pdp_frames.cuh), whose shared-memory needs differ.
+template <bool PF>
 bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesPlan &pl) {
+  using P = pdp::Pipe<PF>;
   const int S = g.seg_cols, W = g.cols, nseg = W / S;
   auto al = [](uint32_t x) { return (x + 127u) & ~127u; };
   for (int R = pdp::kMaxWarps / nseg - 2; R >= 1; --R) {
@@ -149,20 +152,20 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
     if (n_words > pdp::kThreads) continue;
     uint32_t off = 0;
     const uint32_t stage = al((uint32_t)TR * W * 2u + 32u);
-    off += stage * pdp::kRing;
-    pl.off_v2h = off;      off = al(off + pdp::kDepth * (uint32_t)TR * W * 2u);
-    pl.off_ctab = off;     off = al(off + pdp::kHist * (uint32_t)TR * nseg * 4u);
-    pl.off_cand = off;     off = al(off + pdp::kDepth * (uint32_t)n_words * 4u);
-    pl.off_wcnt = off;     off = al(off + pdp::kHist * (uint32_t)n_words * 4u);
-    pl.off_rowcnt = off;   off = al(off + pdp::kDepth * (uint32_t)R * 4u);
-    pl.off_rowphot = off;  off = al(off + pdp::kDepth * (uint32_t)R * 4u);
-    pl.off_rowbase = off;  off = al(off + pdp::kHist * (uint32_t)R * 4u);
-    pl.off_swh = off;      off = al(off + pdp::kDepth * (uint32_t)n_words * 4u);
-    pl.off_stg = off;      off = al(off + pdp::kDepth * 8u * (uint32_t)n_words * 4u);
+    off += stage * P::kRing;
+    pl.off_v2h = off;      off = al(off + (PF ? P::D * (uint32_t)TR * W * 2u : 0u));
+    pl.off_ctab = off;     off = al(off + P::NB * (uint32_t)TR * nseg * 4u);
+    pl.off_cand = off;     off = al(off + P::NB * (uint32_t)n_words * 4u);
+    pl.off_wcnt = off;     off = al(off + P::NB * (uint32_t)n_words * 4u);
+    pl.off_rowcnt = off;   off = al(off + P::NB * (uint32_t)R * 4u);
+    pl.off_rowphot = off;  off = al(off + P::NB * (uint32_t)R * 4u);
+    pl.off_rowbase = off;  off = al(off + P::NB * (uint32_t)R * 4u);
+    pl.off_swh = off;      off = al(off + P::D * (uint32_t)n_words * 4u);
+    pl.off_stg = off;      off = al(off + P::D * 4u * (uint32_t)n_words * 4u);
     pl.off_pref = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
     pl.off_phot = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
-    pl.off_desc = off;     off = al(off + pdp::kHist * 16u);
-    pl.off_bar = off;      off = al(off + (pdp::kRing + 2 * pdp::kDepth) * 8u + (pdp::kRing + pdp::kDepth) * 4u);
+    pl.off_desc = off;     off = al(off + P::NB * 16u);
+    pl.off_bar = off;      off = al(off + (P::kRing + 2 * P::NB) * 8u + (P::kRing + P::NB) * 4u);
     if (off > smem_limit) continue;
     pl.R = R;
     pl.TR = TR;
@@ -180,24 +183,6 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
 using KernelFn = void (*)(const KParams);
 using FramesFn = void (*)(const FParams);
 
-FramesFn frames_kernel_for(int V, int G) {
-  switch (V * 10 + G) {
-    case 21: return pdp::pdp_frames_kernel<2, 1>;
-    case 22: return pdp::pdp_frames_kernel<2, 2>;
-    case 23: return pdp::pdp_frames_kernel<2, 3>;
-    case 24: return pdp::pdp_frames_kernel<2, 4>;
-    case 41: return pdp::pdp_frames_kernel<4, 1>;
-    case 42: return pdp::pdp_frames_kernel<4, 2>;
-    case 43: return pdp::pdp_frames_kernel<4, 3>;
-    case 44: return pdp::pdp_frames_kernel<4, 4>;
-    case 81: return pdp::pdp_frames_kernel<8, 1>;
-    case 82: return pdp::pdp_frames_kernel<8, 2>;
-    case 83: return pdp::pdp_frames_kernel<8, 3>;
-    case 84: return pdp::pdp_frames_kernel<8, 4>;
-  }
-  return nullptr;
-}
-
 KernelFn kernel_for(int V, int G) {
   switch (V * 10 + G) {
     case 21: return pdp::pdp_fused_kernel<2, 1>;
@@ -212,6 +197,25 @@ KernelFn kernel_for(int V, int G) {
     case 82: return pdp::pdp_fused_kernel<8, 2>;
     case 83: return pdp::pdp_fused_kernel<8, 3>;
     case 84: return pdp::pdp_fused_kernel<8, 4>;
+  }
+  return nullptr;
+}
+
+template <bool PF>
+FramesFn frames_kernel_for(int V, int G) {
+  switch (V * 10 + G) {
+    case 21: return pdp::pdp_frames_kernel<2, 1, PF>;
+    case 22: return pdp::pdp_frames_kernel<2, 2, PF>;
+    case 23: return pdp::pdp_frames_kernel<2, 3, PF>;
+    case 24: return pdp::pdp_frames_kernel<2, 4, PF>;
+    case 41: return pdp::pdp_frames_kernel<4, 1, PF>;
+    case 42: return pdp::pdp_frames_kernel<4, 2, PF>;
+    case 43: return pdp::pdp_frames_kernel<4, 3, PF>;
+    case 44: return pdp::pdp_frames_kernel<4, 4, PF>;
+    case 81: return pdp::pdp_frames_kernel<8, 1, PF>;
+    case 82: return pdp::pdp_frames_kernel<8, 2, PF>;
+    case 83: return pdp::pdp_frames_kernel<8, 3, PF>;
+    case 84: return pdp::pdp_frames_kernel<8, 4, PF>;
   }
   return nullptr;
 }
@@ -319,14 +323,18 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     free_ctx(c);
     return cuda_fail(nullptr, e, "cudaFuncSetAttribute");
   }
-  if (make_plan_frames(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan)) {
-    e = cudaFuncSetAttribute(frames_kernel_for(c->plan.V, c->plan.G), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)c->fplan.smem);
+  make_plan_frames<false>(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan[0]);
+  make_plan_frames<true>(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan[1]);
+  for (int pf = 0; pf < 2; ++pf) {
+    if (!c->fplan[pf].ok) continue;
+    FramesFn ff = pf ? frames_kernel_for<true>(c->plan.V, c->plan.G) : frames_kernel_for<false>(c->plan.V, c->plan.G);
+    e = cudaFuncSetAttribute(ff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->fplan[pf].smem);
     if (e != cudaSuccess) {
       free_ctx(c);
       return cuda_fail(nullptr, e, "cudaFuncSetAttribute(frames)");
     }
   }
+  if (const char *s = std::getenv("PDP_PREFILTER")) c->prefilter = std::atoi(s) != 0;
   if (const char *s = std::getenv("PDP_KERNEL"))
     c->kernel_override = !std::strcmp(s, "lookback") ? 1 : (!std::strcmp(s, "frames") ? 2 : 0);
   const size_t mb = npix * sizeof(float);
@@ -460,9 +468,11 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
 
   // Large batches: frame-owner kernel (every CTA owns a frame range, no inter-CTA exchange).
   // Small batches do not give every SM a frame range: band x chunk items with decoupled look-back.
-  const bool use_frames = c->fplan.ok && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
+  const int pf = (c->prefilter && c->fplan[1].ok) ? 1 : 0;
+  const bool use_frames =
+      c->fplan[pf].ok && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
   if (use_frames) {
-    const FramesPlan &fpl = c->fplan;
+    const FramesPlan &fpl = c->fplan[pf];
     FParams f{};
     f.k = k;
     f.k.R = fpl.R;
@@ -486,7 +496,8 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
     f.off_bar = fpl.off_bar;
     f.rg64 = c->d_rg64;
     const int grid_f = std::max(std::min(c->num_sms, n), (n + kFramesPerCtaMax - 1) / kFramesPerCtaMax);
-    frames_kernel_for(pl.V, pl.G)<<<grid_f, fpl.threads, fpl.smem, st>>>(f);
+    FramesFn ff = pf ? frames_kernel_for<true>(pl.V, pl.G) : frames_kernel_for<false>(pl.V, pl.G);
+    ff<<<grid_f, fpl.threads, fpl.smem, st>>>(f);
     PDP_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return PDP_OK;

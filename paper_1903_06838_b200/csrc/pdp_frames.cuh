@@ -6,17 +6,17 @@
 // live in registers for all frames of the CTA; they are re-read from L2 once per band.
 //
 // Inside the CTA three stages run on different tiles (tile = one band of one frame); every thread
-// runs all three, one after the other (kDepth = 4):
+// runs all three, one after the other (lags LS < D, see struct Pipe):
 //
-//   iteration i:   dense(i)          calibrate + common mode + fp16 v2 tile + candidate bitmap
-//                  emit(i-kDepth)    hit records -> their slots in the frame's ordered list
-//                  sparse(i-1)       candidates -> fp16 pre-filter -> exact fp64 seed rule, 3x3 sum,
+//   iteration i:   dense(i)          calibrate + common mode + candidate bitmap (+ fp16 v2 tile)
+//                  emit(i-D)         hit records -> their slots in the frame's ordered list
+//                  sparse(i-LS)      candidates -> (fp16 pre-filter ->) fp64 seed rule, 3x3 sum,
 //                                    photon count; per-word counts; band accum image.  The LAST
 //                                    warp to finish sparse(t) finalises the tile: row prefixes,
 //                                    the tile's base in the frame's list, the frame's running totals
 //
 // Stages hand over through mbarriers that every warp ARRIVES on when it finishes a stage and
-// WAITS on later (dense -> sparse: one iteration later; sparse -> emit / buffer reuse: kDepth - 1
+// WAITS on later (dense -> sparse: LS iterations later; sparse -> emit / buffer reuse: D - LS
 // iterations later), so in steady state nobody blocks: a warp that is late (more selection
 // passes, an fp64 candidate with its L2 round trips) is absorbed by the slack of several tiles.
 // Raw tiles arrive through a ring of bulk async copies; the last warp to finish reading a ring
@@ -28,9 +28,27 @@
 
 namespace pdp {
 
-constexpr int kRing = 6;    // raw tile ring depth (bulk copies in flight per SM)
-constexpr int kDepth = 4;   // tile buffers: sparse(t) may finish up to kDepth-1 iterations late
-constexpr int kHist = 8;    // depth of the small per-tile tables read by emit (>= 2*kDepth - 2)
+// Pipeline shape.  PF = true keeps an fp16 copy of v2 per tile for a pre-filter that rejects
+// candidates with a clearly larger neighbour before the fp64 evaluation (pays off when many
+// above-threshold pixels are not local maxima: dense, wide clouds); the tile copies cost shared
+// memory, so the pipeline is shallow.  PF = false sends every candidate to the fp64 evaluation and
+// spends the shared memory on a deeper raw ring and more slack between the stages instead.
+template <bool PF>
+struct Pipe;
+template <>
+struct Pipe<true> {
+  static constexpr int kRing = 6;   // raw tile ring depth (bulk copies in flight per SM)
+  static constexpr int LS = 1;      // sparse(t) runs at iteration t + LS
+  static constexpr int D = 4;       // emit(t) runs at iteration t + D; depth of the per-tile buffers
+  static constexpr int NB = 8;      // depth of the small per-tile tables and of the barrier arrays
+};
+template <>
+struct Pipe<false> {
+  static constexpr int kRing = 10;
+  static constexpr int LS = 3;
+  static constexpr int D = 8;
+  static constexpr int NB = 16;
+};
 
 struct FParams {
   KParams k;
@@ -132,9 +150,11 @@ __device__ __forceinline__ float half_at(const uint16_t *t, int i) {
   return __half2float(__ushort_as_half(t[i]));
 }
 
-template <int V, int G>
+template <int V, int G, bool PF>
 __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams fp) {
   constexpr int N = V * G;
+  using P = Pipe<PF>;
+  constexpr int kRing = P::kRing, LS = P::LS, D = P::D, NB = P::NB;
   const KParams &k = fp.k;
   extern __shared__ __align__(128) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -144,23 +164,23 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
   const int tile_px = k.TR * k.W;
   const int ctab_n = k.TR * k.nseg;
   unsigned char *stage_base = smem;
-  uint16_t *v2h_all = reinterpret_cast<uint16_t *>(smem + fp.off_v2h);     // [kDepth][tile_px]
-  float *ctab_all = reinterpret_cast<float *>(smem + fp.off_ctab);          // [kHist][ctab_n]
-  uint32_t *cand_all = reinterpret_cast<uint32_t *>(smem + fp.off_cand);    // [kDepth][n_words]
-  uint32_t *wcnt_all = reinterpret_cast<uint32_t *>(smem + fp.off_wcnt);    // [kHist][n_words]
-  int *rowcnt_all = reinterpret_cast<int *>(smem + fp.off_rowcnt);          // [kDepth][R]
-  int *rowphot_all = reinterpret_cast<int *>(smem + fp.off_rowphot);        // [kDepth][R]
-  uint32_t *rowbase_all = reinterpret_cast<uint32_t *>(smem + fp.off_rowbase);  // [kHist][R]
-  uint32_t *swh = reinterpret_cast<uint32_t *>(smem + fp.off_swh);          // [kDepth][n_words]
-  uint32_t *stg = reinterpret_cast<uint32_t *>(smem + fp.off_stg);          // [kDepth][2][4][n_words]
-  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + fp.off_pref);        // [frames]
-  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + fp.off_phot);        // [frames]
-  TileDesc *desc = reinterpret_cast<TileDesc *>(smem + fp.off_desc);        // [kHist]
-  uint64_t *raw_full = reinterpret_cast<uint64_t *>(smem + fp.off_bar);     // [kRing]
-  uint64_t *bar_dense = raw_full + kRing;                                   // [kDepth]
-  uint64_t *bar_count = bar_dense + kDepth;                                 // [kDepth]
-  int *stage_cnt = reinterpret_cast<int *>(bar_count + kDepth);             // [kRing]
-  int *fin_cnt = stage_cnt + kRing;                                         // [kDepth]
+  uint16_t *v2h_all = reinterpret_cast<uint16_t *>(smem + fp.off_v2h);          // [D][tile_px] (PF only)
+  float *ctab_all = reinterpret_cast<float *>(smem + fp.off_ctab);               // [NB][ctab_n]
+  uint32_t *cand_all = reinterpret_cast<uint32_t *>(smem + fp.off_cand);         // [NB][n_words]
+  uint32_t *wcnt_all = reinterpret_cast<uint32_t *>(smem + fp.off_wcnt);         // [NB][n_words]
+  int *rowcnt_all = reinterpret_cast<int *>(smem + fp.off_rowcnt);               // [NB][R]
+  int *rowphot_all = reinterpret_cast<int *>(smem + fp.off_rowphot);             // [NB][R]
+  uint32_t *rowbase_all = reinterpret_cast<uint32_t *>(smem + fp.off_rowbase);   // [NB][R]
+  uint32_t *swh = reinterpret_cast<uint32_t *>(smem + fp.off_swh);               // [D][n_words]
+  uint32_t *stg = reinterpret_cast<uint32_t *>(smem + fp.off_stg);               // [D][4][n_words]
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + fp.off_pref);             // [frames]
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + fp.off_phot);             // [frames]
+  TileDesc *desc = reinterpret_cast<TileDesc *>(smem + fp.off_desc);             // [NB]
+  uint64_t *raw_full = reinterpret_cast<uint64_t *>(smem + fp.off_bar);          // [kRing]
+  uint64_t *bar_dense = raw_full + kRing;                                        // [NB]
+  uint64_t *bar_count = bar_dense + NB;                                          // [NB]
+  int *stage_cnt = reinterpret_cast<int *>(bar_count + NB);                      // [kRing]
+  int *fin_cnt = stage_cnt + kRing;                                              // [NB]
 
   // ---- the frames this CTA owns ----
   const int fs = (int)(((long long)blockIdx.x * k.n_frames) / gridDim.x);
@@ -174,15 +194,15 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
       mbar_init(&raw_full[s], 1);
       stage_cnt[s] = 0;
     }
-    for (int s = 0; s < kDepth; ++s) {
+    for (int s = 0; s < NB; ++s) {
       mbar_init(&bar_dense[s], nwarps);
       mbar_init(&bar_count[s], nwarps);
       fin_cnt[s] = 0;
     }
     fence_mbar_init();
   }
-  for (int i = tid; i < kDepth * n_words; i += nthreads) cand_all[i] = 0u;
-  for (int i = tid; i < kDepth * k.R; i += nthreads) rowcnt_all[i] = 0, rowphot_all[i] = 0;
+  for (int i = tid; i < NB * n_words; i += nthreads) cand_all[i] = 0u;
+  for (int i = tid; i < NB * k.R; i += nthreads) rowcnt_all[i] = 0, rowphot_all[i] = 0;
   for (int i = tid; i < FCn; i += nthreads) pref[i] = 0u, phot[i] = 0u;
   __syncthreads();
 
@@ -213,15 +233,18 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
     for (int t = 0; t < kRing && t < T; ++t) issue(t);
 
   const int dense_warps = k.TR * k.nseg;
-  const int tr = warp / k.nseg, sg = warp - tr * k.nseg;        // dense role of this warp
-  const int my_rr = tid / k.WPR, my_wi = tid - my_rr * k.WPR;   // sparse role of this thread
+  const int tr = warp / k.nseg, sg = warp - tr * k.nseg;  // dense role of this warp
+  // sparse role: the bitmap words are spread over all warps (every word_stride-th thread owns one)
+  const int word_stride = max(1, nthreads / n_words);
+  const int my_word = (tid % word_stride == 0 && tid / word_stride < n_words) ? tid / word_stride : -1;
+  const int my_rr = my_word >= 0 ? my_word / k.WPR : 0, my_wi = my_word >= 0 ? my_word - my_rr * k.WPR : 0;
   float adu_per_rank = 0.375f * k.T_cm / (float)k.S;
   float mK[N], mRg[N], mNpf[N];
   TileDesc cur{0, 0, 0, 0};  // tile of dense(i), advanced incrementally
 
-  for (int i = 0; i < T + kDepth; ++i) {
-    // (A) tile i-kDepth is complete (sparse done by every warp, finalised): its buffers are free
-    if (i >= kDepth) mbar_wait(&bar_count[i & (kDepth - 1)], (uint32_t)((i - kDepth) / kDepth) & 1u);
+  for (int i = 0; i < T + D; ++i) {
+    // (A) tile i-D is complete (sparse done by every warp, finalised): emit it, reuse its buffers
+    if (i >= D) mbar_wait(&bar_count[(i - D) % NB], (uint32_t)((i - D) / NB) & 1u);
 
     // ======================================= dense(i) =======================================
     if (i < T) {
@@ -229,8 +252,8 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
       const int tr_first = (r0 == 0) ? 1 : 0, tr_last = min(k.TR - 1, k.H - r0);
       const bool dense = (warp < dense_warps) && tr >= tr_first && tr <= tr_last;
       const int my_row = r0 - 1 + tr;
-      const int buf = i & (kDepth - 1), slot = i % kRing;
-      if (tid == 0) desc[i & (kHist - 1)] = cur;
+      const int nb = i % NB, slot = i % kRing;
+      if (tid == 0) desc[nb] = cur;
       if (dense && fl == 0) {  // new band: this warp's segment row of the maps -> registers
         const size_t base = ((size_t)p * k.H + my_row) * k.W + (size_t)sg * k.S;
 #pragma unroll
@@ -290,22 +313,25 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             c = warp_median<N>(b, n, __fdiv_rn(tot, (float)n), k.T_cm, adu_per_rank);
           }
         }
-        // v2 = v1 - c: fp16 copy for the sparse pre-filter, candidate bits for the band's own rows
-        const float thr = k.T_seed - k.cand_margin;
+        // candidates of the band's own rows: v2 = v1 - c above T_seed (minus a safety margin; the
+        // exact rule is applied in the sparse stage)
+        const float thr = (k.T_seed - k.cand_margin) + c;
         bool any = false;
 #pragma unroll
-        for (int j = 0; j < N; ++j) {
-          a[j] -= c;
-          any |= a[j] > thr;
-        }
-        uint16_t *v2row = v2h_all + (size_t)buf * tile_px + (size_t)tr * k.W + sg * k.S;
+        for (int j = 0; j < N; ++j) any |= a[j] > thr;
+        if constexpr (PF) {
+          float v2[N];
 #pragma unroll
-        for (int g = 0; g < G; ++g) {
-          const int vi = g * 32 + lane;
-          if (vi * V < k.S) store_half<V>(v2row + vi * V, &a[g * V]);
+          for (int j = 0; j < N; ++j) v2[j] = a[j] - c;
+          uint16_t *v2row = v2h_all + (size_t)(i % D) * tile_px + (size_t)tr * k.W + sg * k.S;
+#pragma unroll
+          for (int g = 0; g < G; ++g) {
+            const int vi = g * 32 + lane;
+            if (vi * V < k.S) store_half<V>(v2row + vi * V, &v2[g * V]);
+          }
         }
         if (lane == 0) {
-          ctab_all[(i & (kHist - 1)) * ctab_n + tr * k.nseg + sg] = c;
+          ctab_all[nb * ctab_n + tr * k.nseg + sg] = c;
           if (k.cm_keep && tr >= 1 && tr <= k.R)
             k.cm_keep[(((size_t)(fs + fl) * k.P + p) * k.H + my_row) * k.nseg + sg] = c;
         }
@@ -317,7 +343,7 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             for (int e = 0; e < V; ++e) bits |= (a[g * V + e] > thr ? 1u : 0u) << e;
             if (bits) {
               const int col = sg * k.S + (g * 32 + lane) * V;
-              atomicOr(&cand_all[buf * n_words + (tr - 1) * k.WPR + (col >> 5)], bits << (col & 31));
+              atomicOr(&cand_all[nb * n_words + (tr - 1) * k.WPR + (col >> 5)], bits << (col & 31));
             }
           }
         }
@@ -329,7 +355,7 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
           stage_cnt[slot] = 0;
           if (i + kRing < T) issue(i + kRing);
         }
-        mbar_arrive(&bar_dense[buf]);
+        mbar_arrive(&bar_dense[nb]);
       }
       // advance to the next tile (frames inner, bands outer, panels outermost)
       if (++cur.fl == FCn) {
@@ -340,21 +366,21 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
       }
     }
 
-    // ======================================= emit(i-kDepth) =======================================
-    if (i >= kDepth && tid < n_words) {
-      const int te = i - kDepth;
-      const uint32_t sw = swh[(te & (kDepth - 1)) * n_words + tid];
+    // ======================================= emit(i-D) =======================================
+    if (i >= D && my_word >= 0) {
+      const int te = i - D;
+      const uint32_t sw = swh[(te % D) * n_words + my_word];
       if (sw) {
-        const int e = te & (kHist - 1);
+        const int e = te % NB;
         const TileDesc d = desc[e];
         uint32_t pos = rowbase_all[e * k.R + my_rr];
         const uint32_t *wc = wcnt_all + e * n_words + my_rr * k.WPR;
         for (int w = 0; w < my_wi; ++w) pos += wc[w];
         const size_t fbase = (size_t)(fs + d.fl) * k.cap;
         const uint16_t *frame_raw = k.raw + (size_t)(fs + d.fl) * k.P * k.H * k.W;
-        const uint32_t *sbase = stg + (size_t)(te & (kDepth - 1)) * 8 * n_words + tid;
+        const uint32_t *s = stg + (size_t)(te % D) * 4 * n_words + my_word;
         uint32_t bits = sw;
-        int kk = 0;
+        bool first = true;
         while (bits) {
           const int b = __ffs(bits) - 1;
           bits &= bits - 1;
@@ -362,13 +388,12 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             const int col = my_wi * 32 + b;
             float E, dx, dy;
             int nph;
-            if (kk < 2) {
-              const uint32_t *s = sbase + (size_t)kk * 4 * n_words;
+            if (first) {
               E = __uint_as_float(s[0]);
               nph = (int)s[n_words];
               dx = __uint_as_float(s[2 * n_words]);
               dy = __uint_as_float(s[3 * n_words]);
-            } else {  // more than two seeds in one 32-pixel word: evaluate again
+            } else {  // more than one seed in one 32-pixel word: evaluate again
               const Exact9 e9 = exact9_g(k, fp.rg64, frame_raw, ctab_all + e * ctab_n, d.p, d.r0, my_rr, col);
               E = (float)e9.E;
               nph = photon_count(e9.E, k.dE_ph);
@@ -382,45 +407,47 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             k.hit_dy[fbase + pos] = dy;
           }
           ++pos;
-          ++kk;
+          first = false;
         }
       }
     }
 
-    // ======================================= sparse(i-1) =======================================
-    if (i >= 1 && i - 1 < T) {
-      const int ts = i - 1, buf = ts & (kDepth - 1), e = ts & (kHist - 1);
-      mbar_wait(&bar_dense[buf], (uint32_t)(ts / kDepth) & 1u);
-      if (tid < n_words) {
-        uint32_t bits = cand_all[buf * n_words + tid];
+    // ======================================= sparse(i-LS) =======================================
+    if (i >= LS && i - LS < T) {
+      const int ts = i - LS, e = ts % NB;
+      mbar_wait(&bar_dense[e], (uint32_t)(ts / NB) & 1u);
+      if (my_word >= 0) {
+        uint32_t bits = cand_all[e * n_words + my_word];
         uint32_t seedword = 0;
         int my_phot = 0, kk = 0;
         if (bits) {
-          cand_all[buf * n_words + tid] = 0u;
+          cand_all[e * n_words + my_word] = 0u;
           const TileDesc d = desc[e];
-          const uint16_t *v2h = v2h_all + (size_t)buf * tile_px;
           const float *ctab = ctab_all + e * ctab_n;
           const uint16_t *frame_raw = k.raw + (size_t)(fs + d.fl) * k.P * k.H * k.W;
-          uint32_t *sbase = stg + (size_t)buf * 8 * n_words + tid;
+          uint32_t *s = stg + (size_t)(ts % D) * 4 * n_words + my_word;
           const int row = d.r0 + my_rr;
           while (bits) {
             const int b = __ffs(bits) - 1;
             bits &= bits - 1;
             const int col = my_wi * 32 + b;
-            // fp16 pre-filter: a neighbour that is clearly larger rules the pixel out
-            const float xc = half_at(v2h, (my_rr + 1) * k.W + col);
-            bool loser = false;
-            for (int dr = -1; dr <= 1; ++dr) {
-              const int r = row + dr;
-              if (r < 0 || r >= k.H) continue;
-              for (int dc = -1; dc <= 1; ++dc) {
-                const int cc = col + dc;
-                if (cc < 0 || cc >= k.W || (dr == 0 && dc == 0)) continue;
-                const float y = half_at(v2h, (my_rr + 1 + dr) * k.W + cc);
-                loser |= (y - xc) > 0.0625f + 0.001953125f * (fabsf(y) + fabsf(xc));
+            if constexpr (PF) {
+              // fp16 pre-filter: a neighbour that is clearly larger rules the pixel out
+              const uint16_t *v2h = v2h_all + (size_t)(ts % D) * tile_px;
+              const float xc = half_at(v2h, (my_rr + 1) * k.W + col);
+              bool loser = false;
+              for (int dr = -1; dr <= 1; ++dr) {
+                const int r = row + dr;
+                if (r < 0 || r >= k.H) continue;
+                for (int dc = -1; dc <= 1; ++dc) {
+                  const int cc = col + dc;
+                  if (cc < 0 || cc >= k.W || (dr == 0 && dc == 0)) continue;
+                  const float y = half_at(v2h, (my_rr + 1 + dr) * k.W + cc);
+                  loser |= (y - xc) > 0.0625f + 0.001953125f * (fabsf(y) + fabsf(xc));
+                }
               }
+              if (loser) continue;
             }
-            if (loser) continue;
             const Exact9 e9 = exact9_g(k, fp.rg64, frame_raw, ctab, d.p, d.r0, my_rr, col);
             if (!e9.seed) continue;
             seedword |= 1u << b;
@@ -428,8 +455,7 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             my_phot += nph;
             // accumulated image: one fire-and-forget RED per hit
             if (nph) red_add_u32(k.accum + ((size_t)d.p * k.H + row) * k.W + col, (uint32_t)nph);
-            if (kk < 2) {
-              uint32_t *s = sbase + (size_t)kk * 4 * n_words;
+            if (kk == 0) {
               s[0] = __float_as_uint((float)e9.E);
               s[n_words] = (uint32_t)nph;
               s[2 * n_words] = __float_as_uint(e9.E > 0.0 ? (float)(e9.sx / e9.E) : 0.f);
@@ -438,25 +464,25 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
             ++kk;
           }
         }
-        wcnt_all[e * n_words + tid] = (uint32_t)kk;
-        swh[buf * n_words + tid] = seedword;
+        wcnt_all[e * n_words + my_word] = (uint32_t)kk;
+        swh[(ts % D) * n_words + my_word] = seedword;
         if (kk) {
-          atomicAdd(&rowcnt_all[buf * k.R + my_rr], kk);
-          atomicAdd(&rowphot_all[buf * k.R + my_rr], my_phot);
+          atomicAdd(&rowcnt_all[e * k.R + my_rr], kk);
+          atomicAdd(&rowphot_all[e * k.R + my_rr], my_phot);
         }
       }
       __syncwarp();
       int last = 0;
       if (lane == 0) {
         __threadfence_block();
-        last = (atomicAdd(&fin_cnt[buf], 1) == nwarps - 1);
+        last = (atomicAdd(&fin_cnt[e], 1) == nwarps - 1);
       }
       last = __shfl_sync(FULL, last, 0);
       if (last) {  // every warp has finished sparse(ts): finalise the tile
         __threadfence_block();
         const TileDesc d = desc[e];
-        const int cnt = lane < k.R ? rowcnt_all[buf * k.R + lane] : 0;
-        const int ph = lane < k.R ? rowphot_all[buf * k.R + lane] : 0;
+        const int cnt = lane < k.R ? rowcnt_all[e * k.R + lane] : 0;
+        const int ph = lane < k.R ? rowphot_all[e * k.R + lane] : 0;
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -468,17 +494,17 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_frames_kernel(const FParams f
         const uint32_t base = pref[d.fl];
         if (lane < k.R) {
           rowbase_all[e * k.R + lane] = base + (uint32_t)(incl - cnt);
-          rowcnt_all[buf * k.R + lane] = 0;
-          rowphot_all[buf * k.R + lane] = 0;
+          rowcnt_all[e * k.R + lane] = 0;
+          rowphot_all[e * k.R + lane] = 0;
         }
         if (lane == 0) {
           pref[d.fl] = base + total;
           phot[d.fl] += phs;
-          fin_cnt[buf] = 0;
+          fin_cnt[e] = 0;
         }
         __syncwarp();
       }
-      if (lane == 0) mbar_arrive(&bar_count[buf]);
+      if (lane == 0) mbar_arrive(&bar_count[e]);
     }
   }
 

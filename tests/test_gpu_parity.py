@@ -29,10 +29,13 @@ def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=F
             n_calls=1, kernel=None):
     # the library picks its kernel by batch size (frame-owner for large batches, band x chunk with
     # look-back for small ones); PDP_KERNEL pins one so that both are tested on every case
-    if kernel:
+    os.environ.pop("PDP_KERNEL", None)
+    os.environ.pop("PDP_PREFILTER", None)
+    if kernel == "frames_pf":                      # frame-owner kernel with the fp16 pre-filter tile
+        os.environ["PDP_KERNEL"] = "frames"
+        os.environ["PDP_PREFILTER"] = "1"
+    elif kernel:
         os.environ["PDP_KERNEL"] = kernel
-    else:
-        os.environ.pop("PDP_KERNEL", None)
     ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
                           max_frames_per_batch=max(1, raw.shape[0]), pedestal=ped.cpu(), gain=gain.cpu(),
                           seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu,
@@ -55,6 +58,7 @@ def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=F
     res["launches"] = ctx.last_launch_count
     ctx.close()
     os.environ.pop("PDP_KERNEL", None)
+    os.environ.pop("PDP_PREFILTER", None)
     return res
 
 
@@ -85,7 +89,7 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("kernel", ["frames", "lookback"])
+@pytest.mark.parametrize("kernel", ["frames", "frames_pf", "lookback"])
 @pytest.mark.parametrize("cm_mode", [0, 1, 2], ids=["median", "mean", "none"])
 @pytest.mark.parametrize("case", list(CASES), ids=list(CASES))
 def test_parity(oracle, case, cm_mode, kernel):
@@ -130,7 +134,8 @@ def test_integer_exact_suite(oracle):
     sig = sig + ph2 * rng.choice([0, 20, 60], (n, P, H, W))                  # neighbours, ties
     raw = torch.tensor((ped.numpy() + gain.numpy() * sig).astype(np.uint16))
     cfg = small(0, panels=P, rows=H, cols=W, seg_cols=S, seed_adu=50.5, cm_adu=20.5, photon_adu=100.0)
-    for cm_mode, kernel in ((0, "frames"), (0, "lookback"), (1, "frames"), (2, "frames"), (2, "lookback")):
+    for cm_mode, kernel in ((0, "frames"), (0, "frames_pf"), (0, "lookback"), (1, "frames"), (2, "frames_pf"),
+                            (2, "lookback")):
         g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
         rep = compare(o, g, panels=P, rows=H, cols=W)
@@ -196,6 +201,18 @@ def test_occupancy_independence_of_lists(oracle):
     raw, ped, gain = make(cfg, 4)
     g = gpu_run(cfg, raw, ped, gain, 0)
     assert g["hit_count"].sum() == 0 and g["accum"].sum() == 0 and g["frame_photons"].sum() == 0
+
+
+@pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
+def test_many_frames_prefilter(oracle, cm_mode):
+    cfg, n = small(3, rows=50, cols=256, seg_cols=128), 300     # dense, wide clouds: many non-maximum candidates
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel="frames_pf")
+    o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    print(rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
 
 
 @pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
