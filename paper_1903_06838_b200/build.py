@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpdp.so")
 SOURCES = ["pdp_api.cu"]
-HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_frames.cuh", os.path.join("..", "..", "include", "pdp.h")]
+HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_frames.cuh", "pdp_stream.cuh", os.path.join("..", "..", "include", "pdp.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]

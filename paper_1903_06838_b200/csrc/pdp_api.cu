@@ -10,9 +10,11 @@
 
 #include "../../include/pdp.h"
 #include "pdp_frames.cuh"
+#include "pdp_stream.cuh"
 
 using pdp::FParams;
 using pdp::KParams;
+using pdp::SParams;
 
 namespace {
 
@@ -34,6 +36,12 @@ struct FramesPlan {
 };
 constexpr int kFramesPerCtaMax = 1024;
 
+struct StreamPlan {
+  bool ok = false;
+  int R = 0, NW = 0, FL = 1, bands_per_panel = 0, n_bands = 0;
+  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, smem = 0;
+};
+
 }  // namespace
 
 struct pdp_ctx {
@@ -50,8 +58,10 @@ struct pdp_ctx {
   int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
   FramesPlan fplan[2];      // [0] without, [1] with the fp16 pre-filter tile
+  StreamPlan splan;         // the streaming kernel (pdp_stream.cuh)
+  double amax = 0.0;        // max over pixels of |v1| any uint16 raw value can produce
   int prefilter = 0;        // PDP_PREFILTER=1 selects fplan[1]
-  int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel (PDP_KERNEL)
+  int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel, 3 streaming kernel (PDP_KERNEL)
   int chunk_frames_override = 0;
   // host-feed state
   uint16_t *d_feed[2] = {nullptr, nullptr};
@@ -180,7 +190,55 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
   return false;
 }
 
+// The streaming kernel: one warp per (band row, segment), R = warps / segments rows per band.
+bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, StreamPlan &pl) {
+  const int nseg = g.cols / g.seg_cols;
+  int R = std::min(pdp::kStreamMaxWarps / nseg, (int)g.rows);
+  if (R < 1 || (R < 2 && g.rows > 1)) return false;
+  auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
+  const uint32_t ring = 3u * (uint32_t)R;
+  uint32_t off = 0;
+  pl.off_cm = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
+  pl.off_bits = off;  off = al(off + pdp::kFCH * ring * (uint32_t)WPR * 4u);
+  pl.off_cnt = off;   off = al(off + 3u * pdp::kFCH * 4u);
+  pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
+  pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
+  pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
+  if (off > smem_limit) return false;
+  pl.R = R;
+  pl.NW = R * nseg;
+  pl.FL = (V * G <= 16) ? 2 : 1;
+  if (const char *e = std::getenv("PDP_STREAM_FL")) pl.FL = std::atoi(e) == 1 ? 1 : pl.FL;
+  pl.bands_per_panel = (g.rows + R - 1) / R;
+  pl.n_bands = pl.bands_per_panel * g.panels;
+  pl.smem = off;
+  pl.ok = true;
+  return true;
+}
+
 using KernelFn = void (*)(const KParams);
+using StreamFn = void (*)(const SParams);
+
+template <int FL>
+StreamFn stream_kernel_for(int V, int G) {
+  switch (V * 10 + G) {
+    case 21: return pdp::pdp_stream_kernel<2, 1, FL>;
+    case 22: return pdp::pdp_stream_kernel<2, 2, FL>;
+    case 23: return pdp::pdp_stream_kernel<2, 3, FL>;
+    case 24: return pdp::pdp_stream_kernel<2, 4, FL>;
+    case 41: return pdp::pdp_stream_kernel<4, 1, FL>;
+    case 42: return pdp::pdp_stream_kernel<4, 2, FL>;
+    case 43: return pdp::pdp_stream_kernel<4, 3, FL>;
+    case 44: return pdp::pdp_stream_kernel<4, 4, FL>;
+    case 81: return pdp::pdp_stream_kernel<8, 1, FL>;
+    case 82: return pdp::pdp_stream_kernel<8, 2, FL>;
+  }
+  return nullptr;
+}
+StreamFn stream_kernel(int V, int G, int FL) {
+  if (V == 8 && G > 2) return FL == 1 ? (G == 3 ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 4, 1>) : nullptr;
+  return FL == 2 ? stream_kernel_for<2>(V, G) : stream_kernel_for<1>(V, G);
+}
 using FramesFn = void (*)(const FParams);
 
 KernelFn kernel_for(int V, int G) {
@@ -287,6 +345,7 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   // npf = -(ped - rint(ped))/gain, so that v1 = fma((2^23 + raw) - K, rg, npf)
   std::vector<float> K, rg, npf;
   std::vector<double> rg64;
+  double amax = 0.0;
   try {
     rg64.resize(npix);
     K.resize(npix);
@@ -300,6 +359,7 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     if (!std::isfinite(p) || !std::isfinite(g) || g == 0.0 || std::fabs(p) > 4.0e6)
       return fail(nullptr, PDP_E_VALUE, "pdp_create: non-finite or out-of-range pedestal/gain");
     const double pi = std::nearbyint(p), r = 1.0 / g;
+    amax = std::max(amax, (65535.0 + std::fabs(p)) * std::fabs(r));
     K[i] = (float)(8388608.0 + pi);
     rg[i] = (float)r;
     rg64[i] = r;
@@ -334,9 +394,22 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
       return cuda_fail(nullptr, e, "cudaFuncSetAttribute(frames)");
     }
   }
+  c->amax = amax;
+  if (make_plan_stream(*geo, c->plan.V, c->plan.G, c->plan.WPR, prop.sharedMemPerBlockOptin, c->splan)) {
+    StreamFn sf = stream_kernel(c->plan.V, c->plan.G, c->splan.FL);
+    if (!sf) {
+      c->splan.ok = false;
+    } else {
+      e = cudaFuncSetAttribute(sf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->splan.smem);
+      if (e != cudaSuccess) {
+        free_ctx(c);
+        return cuda_fail(nullptr, e, "cudaFuncSetAttribute(stream)");
+      }
+    }
+  }
   if (const char *s = std::getenv("PDP_PREFILTER")) c->prefilter = std::atoi(s) != 0;
   if (const char *s = std::getenv("PDP_KERNEL"))
-    c->kernel_override = !std::strcmp(s, "lookback") ? 1 : (!std::strcmp(s, "frames") ? 2 : 0);
+    c->kernel_override = !std::strcmp(s, "lookback") ? 1 : (!std::strcmp(s, "frames") ? 2 : (!std::strcmp(s, "stream") ? 3 : 0));
   const size_t mb = npix * sizeof(float);
   const size_t lb = (size_t)geo->max_frames_per_batch * c->plan.n_bands * sizeof(unsigned long long);
   cudaError_t errs[] = {cudaMalloc(&c->d_ped, mb),     cudaMalloc(&c->d_gain, mb),      cudaMalloc(&c->d_K, mb),
@@ -466,7 +539,46 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   k.off_accum = pl.off_accum;
   k.off_misc = pl.off_misc;
 
-  // Large batches: frame-owner kernel (every CTA owns a frame range, no inter-CTA exchange).
+  // Large batches: the streaming kernel (frame-owner CTAs, no staging, no barriers).  It needs
+  // BIG = a power of two above twice the largest |v1| the maps allow, small enough to keep ~1e-2 ADU.
+  {
+    const double need = 2.0 * (c->amax + (double)c->prm.cm_adu) + 1.0;
+    double big = 1024.0;
+    while (big < need) big *= 2.0;
+    const bool big_ok = big <= 4194304.0 && (double)c->prm.cm_adu < 0.25 * big;
+    const bool use_stream = c->splan.ok && big_ok &&
+                            (c->kernel_override == 3 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
+    if (c->kernel_override == 3 && !use_stream)
+      return fail(c, PDP_E_GEOMETRY, "PDP_KERNEL=stream: the streaming kernel does not support this geometry/maps");
+    if (use_stream) {
+      const StreamPlan &spl = c->splan;
+      SParams s{};
+      s.k = k;
+      s.k.R = spl.R;
+      s.k.TR = spl.R;
+      s.k.bands_per_panel = spl.bands_per_panel;
+      s.k.n_bands = spl.n_bands;
+      s.rg64 = c->d_rg64;
+      s.big = (float)big;
+      const double ulp_big = big / 8388608.0;
+      s.cand_thr = (float)((double)c->prm.seed_adu - (std::max(1e-3, 4e-6 * std::fabs((double)c->prm.seed_adu)) + 2.0 * ulp_big));
+      s.R = spl.R;
+      s.NW = spl.NW;
+      s.off_cm = spl.off_cm;
+      s.off_bits = spl.off_bits;
+      s.off_cnt = spl.off_cnt;
+      s.off_done = spl.off_done;
+      s.off_pref = spl.off_pref;
+      s.off_phot = spl.off_phot;
+      const int grid_s = std::min(c->num_sms, n);
+      StreamFn sf = stream_kernel(pl.V, pl.G, spl.FL);
+      sf<<<grid_s, spl.NW * 32, spl.smem, st>>>(s);
+      PDP_CUDA(c, cudaGetLastError());
+      c->launches += 1;
+      return PDP_OK;
+    }
+  }
+  // Otherwise: frame-owner kernel with the staged pipeline (every CTA owns a frame range).
   // Small batches do not give every SM a frame range: band x chunk items with decoupled look-back.
   const int pf = (c->prefilter && c->fplan[1].ok) ? 1 : 0;
   const bool use_frames =

@@ -1,0 +1,639 @@
+// pdp_stream.cuh — the throughput kernel (one launch per pdp_process call for large batches).
+//
+// Built around the measured sm_100a issue model: one warp-instruction per cycle and
+// SM sub-partition, FFMA/FADD one cycle on the FMA pipe, every compare/select/permute/logic and
+// every packed-half instruction two cycles, so at 2 B/pixel the HBM roofline leaves ~11 issue
+// slots per pixel-lane.  Consequences:
+//   * no staging through shared memory and no CTA-wide barriers: a warp owns one row segment of a
+//     band (maps in registers), streams the raw pixels of its frames straight from global memory
+//     with 64/128-bit loads, the next frames prefetched into registers while it computes;
+//   * FL frames are processed in lock-step by one warp: their selection searches share every
+//     warp-wide reduction (counts packed into one REDUX) and the pivot logic runs once, each
+//     half-warp steering one search;
+//   * the masked value is ONE FFMA: bq = a + [|a| >= T_cm] * BIG, so pixels outside the mask sort
+//     above every pivot and still carry their value for the seed-candidate test;
+//   * the exact median is found by counting passes (FSET + FADD per pixel) that stop as soon as
+//     a pivot's rank is k, k+1 (or k+2 for an even count) and one push-and-min/max pass
+//     (FSET + FFMA + 1/2 FMNMX3) reads the order statistic itself; everything that does not
+//     converge (ties) goes to the generic bisection of pdp_device.cuh;
+//   * the sparse stage (fp64 seed rule, 3x3 sum, centroid, ordered emission) of a (frame, band) is
+//     run by whichever warp finishes that band of that frame last; nobody waits for it.
+//
+// Decomposition: frame-owner.  CTA b owns frames [fs, fe); it walks them in chunks of kFCH frames,
+// band by band (R rows x all segments = one warp each), frames innermost, so the calibration maps
+// are read from L2 once per (band, chunk) and the per-frame hit-list offsets are a CTA-local
+// running prefix: no inter-CTA exchange at all.
+#pragma once
+#include "pdp_frames.cuh"
+
+namespace pdp {
+
+constexpr int kStreamMaxWarps = 16;
+constexpr int kStreamThreads = kStreamMaxWarps * 32;
+constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
+constexpr int kMaxIt = 9;   // counting passes before the generic bisection takes over
+
+struct SParams {
+  KParams k;
+  const double *rg64;   // 1/gain in double (sparse stage)
+  float big;            // BIG: power of two > 2 * (max |v1| + T_cm); pixels outside the mask get +BIG
+  float cand_thr;       // T_seed - margin (margin covers the rounding of a + BIG)
+  int R, NW;            // rows per band, warps per CTA (= R * nseg)
+  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot;
+};
+
+// ---- small helpers -------------------------------------------------------------------------------
+template <int V>
+struct VecLoadG;  // V uint16 pixels from global memory (read-only path), V*2-byte aligned
+template <>
+struct VecLoadG<2> {
+  __device__ static __forceinline__ void ld(const uint16_t *p, uint32_t (&w)[1]) {
+    w[0] = __ldg(reinterpret_cast<const unsigned *>(p));
+  }
+};
+template <>
+struct VecLoadG<4> {
+  __device__ static __forceinline__ void ld(const uint16_t *p, uint32_t (&w)[2]) {
+    const uint2 t = __ldg(reinterpret_cast<const uint2 *>(p));
+    w[0] = t.x;
+    w[1] = t.y;
+  }
+};
+template <>
+struct VecLoadG<8> {
+  __device__ static __forceinline__ void ld(const uint16_t *p, uint32_t (&w)[4]) {
+    const uint4 t = __ldg(reinterpret_cast<const uint4 *>(p));
+    w[0] = t.x;
+    w[1] = t.y;
+    w[2] = t.z;
+    w[3] = t.w;
+  }
+};
+
+__device__ __forceinline__ float set_ge_abs(float a, float t) {  // 1.0f if |a| >= t else 0.0f
+  float d;
+  asm("set.ge.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(fabsf(a)), "f"(t));
+  return d;
+}
+__device__ __forceinline__ float set_lt_abs(float a, float t) {
+  float d;
+  asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(fabsf(a)), "f"(t));
+  return d;
+}
+__device__ __forceinline__ float set_le(float a, float b) {
+  float d;
+  asm("set.le.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+__device__ __forceinline__ float set_ge(float a, float b) {
+  float d;
+  asm("set.ge.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+
+__device__ __forceinline__ float warp_min_f(float v) { return key2f(warp_min_u(f2key(v))); }
+__device__ __forceinline__ float warp_max_f(float v) { return key2f(warp_max_u(f2key(v))); }
+
+// Order statistics read off with one pass: values on the wrong side of the pivot are pushed out of
+// range by +-big2 (exactly representable move; values on the right side are untouched: r = 0).
+template <int N>
+__device__ __forceinline__ float min_ge(const float (&b)[N], float p, float big2) {  // min{b : b >= p}
+  float m = __int_as_float(0x7f800000);
+#pragma unroll
+  for (int j = 0; j < N; ++j) m = fminf(m, fmaf(set_lt(b[j], p), big2, b[j]));
+  return warp_min_f(m);
+}
+template <int N>
+__device__ __forceinline__ float max_lt(const float (&b)[N], float p, float big2) {  // max{b : b < p}
+  float m = __int_as_float(0xff800000);
+#pragma unroll
+  for (int j = 0; j < N; ++j) m = fmaxf(m, fmaf(set_ge(b[j], p), -big2, b[j]));
+  return warp_max_f(m);
+}
+template <int N>
+__device__ __forceinline__ float min_gt_count(const float (&b)[N], float a, float big2, int &n_le) {
+  float m = __int_as_float(0x7f800000), c = 0.f;  // min{b : b > a}, #{b <= a}
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const float r = set_le(b[j], a);
+    c += r;
+    m = fminf(m, fmaf(r, big2, b[j]));
+  }
+  n_le = warp_sum_i(__float2int_rn(c));
+  return warp_min_f(m);
+}
+template <int N>
+__device__ __forceinline__ float max_lt_count(const float (&b)[N], float a, float big2, int &n_lt) {
+  float m = __int_as_float(0xff800000), c = 0.f;  // max{b : b < a}, #{b < a}
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const float r = set_ge(b[j], a);
+    c += r;
+    m = fmaxf(m, fmaf(r, -big2, b[j]));
+  }
+  n_lt = 32 * N - warp_sum_i(__float2int_rn(c));
+  return warp_max_f(m);
+}
+
+// fp64 evaluation of the 3x3 window of (row, col) of panel p: v2 = (raw - ped) * (1/gain) - c with the
+// common-mode estimates of the three rows passed as pointers (nullptr: the row does not exist).
+__device__ __forceinline__ Exact9 exact9_rows(const KParams &k, const double *rg64, const uint16_t *frame_raw,
+                                              const float *cm_m1, const float *cm_0, const float *cm_p1, int p,
+                                              int row, int col) {
+  const int sgc = col / k.S, cs = col - sgc * k.S;
+  const int sg3[3] = {cs == 0 ? sgc - 1 : sgc, sgc, cs == k.S - 1 ? sgc + 1 : sgc};
+  const float *cmr[3] = {cm_m1, cm_0, cm_p1};
+  double v[9];
+  bool ex[9];
+#pragma unroll
+  for (int dr = -1; dr <= 1; ++dr)
+#pragma unroll
+    for (int dc = -1; dc <= 1; ++dc) {
+      const int i = (dr + 1) * 3 + dc + 1;
+      const int r = row + dr, c = col + dc;
+      ex[i] = (r >= 0 && r < k.H && c >= 0 && c < k.W);
+      v[i] = 0.0;
+      if (ex[i]) {
+        const size_t gi = ((size_t)p * k.H + r) * k.W + c;
+        const unsigned rawv = __ldg(frame_raw + gi);
+        const double cm = (double)cmr[dr + 1][sg3[dc + 1]];
+        v[i] = ((double)rawv - (double)__ldg(k.ped + gi)) * __ldg(rg64 + gi) - cm;
+      }
+    }
+  Exact9 o;
+  const double x = v[4];
+  o.seed = x > k.dT_seed;
+  o.E = 0.0;
+  o.sx = 0.0;
+  o.sy = 0.0;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    if (!ex[i]) continue;
+    const double y = v[i];
+    o.E += y;
+    o.sx += (double)(i % 3 - 1) * y;
+    o.sy += (double)(i / 3 - 1) * y;
+    if (i == 4) continue;
+    // strict maximum; a tie goes to the lower linear index (i < 4 <=> neighbour has lower index)
+    if (!(x > y || (x == y && i > 4))) o.seed = false;
+  }
+  return o;
+}
+
+struct HitRec {
+  float E, dx, dy;
+  int n;
+};
+__device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
+  HitRec h;
+  h.E = (float)e9.E;
+  h.n = photon_count(e9.E, E_ph);
+  h.dx = e9.E > 0.0 ? (float)(e9.sx / e9.E) : 0.f;
+  h.dy = e9.E > 0.0 ? (float)(e9.sy / e9.E) : 0.f;
+  return h;
+}
+
+// ---- sparse stage of one (frame slot, band): run by ONE warp ------------------------------------
+// Evaluates the seed candidates of rows [r0-1, r0+R-2] of the band's panel (from row 0 for the first
+// band, through row H-1 for the last one): every window row then has its common-mode estimate.
+__device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int fl, int gb, int fs) {
+  const KParams &k = sp.k;
+  const int lane = threadIdx.x & 31;
+  const int R = sp.R, ring_rows = 3 * R;
+  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm) + (size_t)fl * ring_rows * k.nseg;
+  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits) + (size_t)fl * ring_rows * k.WPR;
+  volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);
+
+  const int chunk = gb / k.n_bands, band = gb - chunk * k.n_bands;
+  const int f = fs + chunk * kFCH + fl;
+  const int p = band / k.bands_per_panel, bi = band - p * k.bands_per_panel, r0 = bi * R;
+  const int ra = bi == 0 ? 0 : r0 - 1;
+  const int rb = bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
+  const int gb0 = gb - bi;  // running band index of band 0 of this panel
+  auto slot_of = [&](int r) {
+    const int q = r / R;
+    return ((gb0 + q) % 3) * R + (r - q * R);
+  };
+  const uint16_t *frame_raw = k.raw + (size_t)f * k.P * k.H * k.W;
+  const size_t fbase = (size_t)f * k.cap;
+  uint32_t base = pref[fl];
+  int phsum = 0;
+  const int total_words = (rb - ra + 1) * k.WPR;
+  for (int i0 = 0; i0 < total_words; i0 += 32) {
+    const int i = i0 + lane;
+    const bool valid = i < total_words;
+    const int rr = valid ? i / k.WPR : 0, wi = i - rr * k.WPR, row = ra + rr;
+    uint32_t *wp = bits + (size_t)slot_of(row) * k.WPR + wi;
+    uint32_t cand = valid ? *wp : 0u;
+    if (!__any_sync(FULL, cand != 0u)) continue;
+    uint32_t seedword = 0;
+    HitRec rec0{0.f, 0.f, 0.f, 0}, rec1{0.f, 0.f, 0.f, 0};
+    int kk = 0;
+    const float *cm_m1 = nullptr, *cm_0 = nullptr, *cm_p1 = nullptr;
+    if (cand) {
+      *wp = 0u;
+      cm_0 = cmring + (size_t)slot_of(row) * k.nseg;
+      if (row > 0) cm_m1 = cmring + (size_t)slot_of(row - 1) * k.nseg;
+      if (row < k.H - 1) cm_p1 = cmring + (size_t)slot_of(row + 1) * k.nseg;
+      while (cand) {
+        const int b = __ffs(cand) - 1;
+        cand &= cand - 1;
+        const int col = wi * 32 + b;
+        const Exact9 e9 = exact9_rows(k, sp.rg64, frame_raw, cm_m1, cm_0, cm_p1, p, row, col);
+        if (!e9.seed) continue;
+        seedword |= 1u << b;
+        const HitRec h = make_rec(e9, k.dE_ph);
+        phsum += h.n;
+        // accumulated image: one fire-and-forget RED per hit
+        if (h.n) red_add_u32(k.accum + ((size_t)p * k.H + row) * k.W + col, (uint32_t)h.n);
+        if (kk == 0) rec0 = h;
+        if (kk == 1) rec1 = h;
+        ++kk;
+      }
+    }
+    // ordered slots: lanes are in (row, word) order, bits in column order
+    int incl = kk;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += t;
+    }
+    const int tot = __shfl_sync(FULL, incl, 31);
+    uint32_t pos = base + (uint32_t)(incl - kk);
+    int j = 0;
+    while (seedword) {
+      const int b = __ffs(seedword) - 1;
+      seedword &= seedword - 1;
+      if (pos < k.cap) {
+        const int col = wi * 32 + b;
+        HitRec h = j == 0 ? rec0 : rec1;
+        if (j >= 2)  // more than two seeds in one 32-pixel word: evaluate again
+          h = make_rec(exact9_rows(k, sp.rg64, frame_raw, cm_m1, cm_0, cm_p1, p, row, col), k.dE_ph);
+        k.hit_pixel[fbase + pos] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
+        k.hit_charge[fbase + pos] = h.E;
+        k.hit_nphot[fbase + pos] = h.n;
+        k.hit_dx[fbase + pos] = h.dx;
+        k.hit_dy[fbase + pos] = h.dy;
+      }
+      ++pos;
+      ++j;
+    }
+    base += (uint32_t)tot;
+  }
+  phsum = warp_sum_i(phsum);
+  if (lane == 0) {
+    if (band == k.n_bands - 1) {  // the frame is complete
+      k.hit_count[f] = base;
+      k.frame_photons[f] = phot[fl] + (uint32_t)phsum;
+      if (base > k.cap) atomicOr(k.status, 1u);
+      pref[fl] = 0u;
+      phot[fl] = 0u;
+    } else {
+      pref[fl] = base;
+      phot[fl] += (uint32_t)phsum;
+    }
+    __threadfence_block();
+    done[fl] = gb + 1;
+  }
+  __syncwarp();
+}
+
+// ---- the kernel ----------------------------------------------------------------------------------
+// V = pixels per vector load (2/4/8), G = vectors per lane (one warp covers S <= 32*V*G pixels),
+// FL = frames processed in lock-step by a warp (1 or 2).
+template <int V, int G, int FL>
+__global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SParams sp) {
+  constexpr int N = V * G;
+  constexpr int GL = 32 / FL;  // lanes steering one search
+  const KParams &k = sp.k;
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nthreads = blockDim.x, NW = nthreads >> 5;
+  const int R = sp.R, ring_rows = 3 * R;
+  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);          // [kFCH][3R][nseg]
+  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);    // [kFCH][3R][WPR]
+  int *cnt = reinterpret_cast<int *>(smem + sp.off_cnt);                // [3][kFCH]
+  volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);  // [kFCH]
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);    // [kFCH]
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);    // [kFCH]
+
+  const int fs = (int)(((long long)blockIdx.x * k.n_frames) / gridDim.x);
+  const int fe = (int)(((long long)(blockIdx.x + 1) * k.n_frames) / gridDim.x);
+  const int FCn = fe - fs;
+  if (FCn <= 0) return;
+
+  for (int i = tid; i < kFCH * ring_rows * k.WPR; i += nthreads) bits[i] = 0u;
+  for (int i = tid; i < 3 * kFCH; i += nthreads) cnt[i] = 0;
+  for (int i = tid; i < kFCH; i += nthreads) done[i] = 0, pref[i] = 0u, phot[i] = 0u;
+  __syncthreads();
+
+  const int tr = warp / k.nseg, sg = warp - tr * k.nseg;  // this warp's row of the band and segment
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  const float BIG = sp.big, BIG2 = 4.f * sp.big;
+  const int ms = lane / GL;  // the search this lane steers
+  float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
+  float mK[N], mRg[N], mNpf[N];
+  constexpr int NS = (N + 2) / 3;  // pixels per lane sampled for the first pivot (every third)
+
+  int gb = 0;
+  for (int c0 = 0; c0 < FCn; c0 += kFCH) {
+    const int nf = min(kFCH, FCn - c0);
+    for (int band = 0; band < k.n_bands; ++band, ++gb) {
+      const int p = band / k.bands_per_panel, r0 = (band - p * k.bands_per_panel) * R;
+      const int row = r0 + tr;
+      const bool active = row < k.H;
+      const int slot = (gb % 3) * R + tr;
+      const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
+      if (active) {
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+          const int vi = g * 32 + lane;
+          if (vi * V < k.S) {
+            load_map<V>(k.mapK + rowoff + vi * V, &mK[g * V]);
+            load_map<V>(k.mapRg + rowoff + vi * V, &mRg[g * V]);
+            load_map<V>(k.mapNpf + rowoff + vi * V, &mNpf[g * V]);
+          } else {  // padding lanes: a = -BIG/2, i.e. bq = BIG/2: above every pivot, below every candidate
+#pragma unroll
+            for (int e = 0; e < V; ++e) mK[g * V + e] = 8388608.f, mRg[g * V + e] = 0.f, mNpf[g * V + e] = -0.5f * BIG;
+          }
+        }
+      }
+      const uint16_t *rowp = k.raw + (size_t)(fs + c0) * npix + rowoff;
+      uint32_t wn[FL][N / 2];
+      auto fetch = [&](int g0) {
+#pragma unroll
+        for (int q = 0; q < FL; ++q)
+#pragma unroll
+          for (int g = 0; g < G; ++g) {
+            const int vi = g * 32 + lane;
+            uint32_t t[V / 2];
+#pragma unroll
+            for (int e = 0; e < V / 2; ++e) t[e] = 0u;
+            if (active && g0 + q < nf && vi * V < k.S) VecLoadG<V>::ld(rowp + (size_t)(g0 + q) * npix + vi * V, t);
+#pragma unroll
+            for (int e = 0; e < V / 2; ++e) wn[q][g * (V / 2) + e] = t[e];
+          }
+      };
+      fetch(0);
+      for (int g0 = 0; g0 < nf; g0 += FL) {
+        uint32_t w[FL][N / 2];
+#pragma unroll
+        for (int q = 0; q < FL; ++q)
+#pragma unroll
+          for (int e = 0; e < N / 2; ++e) w[q][e] = wn[q][e];
+        if (g0 + FL < nf) fetch(g0 + FL);
+        // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
+#pragma unroll
+        for (int q = 0; q < FL; ++q)
+          if (g0 + q < nf)
+            while (done[g0 + q] < gb - 1) {
+            }
+
+        if (active) {
+          float cq[FL];
+          uint32_t cbits[FL][G];
+          bool anyc[FL];
+          if (k.cm_mode == 0) {
+            // ================= exact median common mode (north_star (a)) =================
+            float bq[FL][N];
+            float nout[FL], ssum[FL];
+#pragma unroll
+            for (int q = 0; q < FL; ++q) {
+              float n0 = 0.f, n1 = 0.f, s0 = 0.f;
+#pragma unroll
+              for (int e = 0; e < N / 2; ++e) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                  const int j = 2 * e + h;
+                  const float x = __uint_as_float(__byte_perm(w[q][e], 0x4B000000u, h ? 0x7632 : 0x7610));
+                  const float a = fmaf(x - mK[j], mRg[j], mNpf[j]);
+                  const float notm = set_ge_abs(a, k.T_cm);   // pixels WITH signal
+                  bq[q][j] = fmaf(notm, BIG, a);
+                  if (h) n1 += notm; else n0 += notm;
+                  if (j % 3 == 0) s0 += fmaf(-notm, a, a);
+                }
+              }
+              nout[q] = n0 + n1;
+              ssum[q] = s0;
+            }
+            // n (exact) and the first pivot (mean of a third of the masked pixels)
+            int nq[FL];
+            float pq[FL];
+            {
+              float pk = nout[0];
+              if constexpr (FL == 2) pk = fmaf(nout[1], 65536.f, pk);
+              const unsigned tot = (unsigned)warp_sum_i(__float2int_rn(pk));
+#pragma unroll
+              for (int q = 0; q < FL; ++q) {
+                nq[q] = 32 * N - (int)((tot >> (16 * q)) & 0xffffu);
+                const int si = warp_sum_i(__float2int_rn(ssum[q] * 256.f));
+                const float est = (float)si * (1.f / 256.f) * ((float)N / (float)NS) / fmaxf((float)nq[q], 1.f);
+                pq[q] = fminf(fmaxf(est, -k.T_cm), k.T_cm);
+              }
+            }
+            // ---- lock-step search; lanes [q*GL, (q+1)*GL) steer search q ----
+            const int n_my = FL == 2 ? (ms ? nq[FL - 1] : nq[0]) : nq[0];
+            const int kl = (n_my - 1) >> 1, kh = n_my >> 1;
+            const int acc_hi = kh + 1;                  // accepted ranks of a pivot: kl .. kh+1
+            const float tgt = 0.5f * (float)(kl + kh + 1);
+            float p_my = FL == 2 ? (ms ? pq[FL - 1] : pq[0]) : pq[0];
+            float lo = 0.f, hi = 0.f;
+            int cl = 0, ch = 0;
+            bool have_lo = false, have_hi = false;
+            bool fin = n_my < k.cm_min_count || n_my <= 0;  // c = 0: nothing to search
+            bool failed = false;
+            int c_fin = 0;
+            for (int it = 0; it < kMaxIt; ++it) {
+              if (__all_sync(FULL, fin || failed)) break;
+              float pv[FL];
+#pragma unroll
+              for (int q = 0; q < FL; ++q) pv[q] = __shfl_sync(FULL, p_my, q * GL);
+              float pk;
+              {
+                float a0[FL], a1[FL], a2[FL];
+#pragma unroll
+                for (int q = 0; q < FL; ++q) {
+                  a0[q] = a1[q] = a2[q] = 0.f;
+#pragma unroll
+                  for (int j = 0; j < N; ++j) {
+                    const float d = set_lt(bq[q][j], pv[q]);
+                    if (j % 3 == 0) a0[q] += d;
+                    else if (j % 3 == 1) a1[q] += d;
+                    else a2[q] += d;
+                  }
+                }
+                pk = a0[0] + a1[0] + a2[0];
+                if constexpr (FL == 2) pk = fmaf(a0[1] + a1[1] + a2[1], 65536.f, pk);
+              }
+              const unsigned tot = (unsigned)warp_sum_i(__float2int_rn(pk));
+              const int c = (int)((tot >> (16 * ms)) & 0xffffu);
+              if (!fin && !failed) {
+                if (c >= kl && c <= acc_hi) {
+                  fin = true;
+                  c_fin = c;
+                } else {
+                  if (c < kl) lo = p_my, cl = c, have_lo = true;
+                  else hi = p_my, ch = c, have_hi = true;
+                  float pn;
+                  if (have_lo && have_hi) {
+                    const float slope = __fdividef(hi - lo, (float)(ch - cl));
+                    pn = fmaf(tgt - (float)cl, slope, lo);
+                    if (ch - cl >= 4) apr = 0.75f * apr + 0.25f * slope;
+                    if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
+                    if (!(pn > lo && pn < hi)) failed = true;   // no float strictly inside: ties
+                  } else {
+                    pn = fmaf(tgt - (float)c, apr, p_my);
+                  }
+                  p_my = pn;
+                }
+              }
+            }
+            if (!fin) failed = true;
+            // ---- read the order statistics ----
+#pragma unroll
+            for (int q = 0; q < FL; ++q) {
+              const int src = q * GL;
+              const bool f_q = __shfl_sync(FULL, (int)failed, src) != 0;
+              const float p_q = __shfl_sync(FULL, p_my, src);
+              const int d_q = __shfl_sync(FULL, c_fin - kl, src);
+              const int n_q = nq[q];
+              const int kl_q = (n_q - 1) >> 1;
+              const bool even = (n_q & 1) == 0;
+              float c = 0.f;
+              if (n_q >= k.cm_min_count && n_q > 0) {
+                if (f_q) {
+                  float apr2 = __shfl_sync(FULL, apr, src);   // one value for the whole warp
+                  c = warp_median<N>(bq[q], n_q, pq[q], k.T_cm, apr2);
+                } else if (!even) {
+                  c = d_q == 0 ? min_ge<N>(bq[q], p_q, BIG2) : max_lt<N>(bq[q], p_q, BIG2);
+                } else if (d_q == 1) {
+                  c = 0.5f * (max_lt<N>(bq[q], p_q, BIG2) + min_ge<N>(bq[q], p_q, BIG2));
+                } else if (d_q == 0) {   // x[kl] = min >= p; x[kh] = the next one (or an equal one)
+                  const float A = min_ge<N>(bq[q], p_q, BIG2);
+                  int n_le;
+                  const float B = min_gt_count<N>(bq[q], A, BIG2, n_le);
+                  c = 0.5f * (A + (n_le >= kl_q + 2 ? A : B));
+                } else {                 // d == 2: x[kh] = max < p; x[kl] = the one before (or an equal one)
+                  const float B = max_lt<N>(bq[q], p_q, BIG2);
+                  int n_lt;
+                  const float A = max_lt_count<N>(bq[q], B, BIG2, n_lt);
+                  c = 0.5f * (B + (n_lt <= kl_q ? B : A));
+                }
+              }
+              cq[q] = c;
+              // seed candidates (exact rule applied in the sparse stage): v1 - c > T_seed - margin
+              const float thr = sp.cand_thr + c;
+              const float thr2 = BIG + thr;
+              bool any = false;
+#pragma unroll
+              for (int j = 0; j < N; ++j) any |= bq[q][j] > thr2;
+              const bool low = thr < k.T_cm;   // (rare) a pixel inside the mask can seed
+              if (low) {
+#pragma unroll
+                for (int j = 0; j < N; ++j) any |= (bq[q][j] > thr && bq[q][j] < k.T_cm);
+              }
+              anyc[q] = __any_sync(FULL, any);
+              if (anyc[q]) {
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                  uint32_t bb = 0;
+#pragma unroll
+                  for (int e = 0; e < V; ++e) {
+                    const float v = bq[q][g * V + e];
+                    bb |= ((v > thr2) || (low && v > thr && v < k.T_cm) ? 1u : 0u) << e;
+                  }
+                  cbits[q][g] = bb;
+                }
+              }
+            }
+          } else {
+            // ================= guarded mean or no common mode =================
+#pragma unroll
+            for (int q = 0; q < FL; ++q) {
+              float a[N];
+              float n0 = 0.f, n1 = 0.f, s0 = 0.f, s1 = 0.f;
+#pragma unroll
+              for (int e = 0; e < N / 2; ++e) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                  const int j = 2 * e + h;
+                  const float x = __uint_as_float(__byte_perm(w[q][e], 0x4B000000u, h ? 0x7632 : 0x7610));
+                  a[j] = fmaf(x - mK[j], mRg[j], mNpf[j]);
+                  if (k.cm_mode == 1) {
+                    const float m = set_lt_abs(a[j], k.T_cm);
+                    if (h) n1 += m, s1 = fmaf(m, a[j], s1);
+                    else n0 += m, s0 = fmaf(m, a[j], s0);
+                  }
+                }
+              }
+              float c = 0.f;
+              if (k.cm_mode == 1) {
+                const int n = warp_sum_i(__float2int_rn(n0 + n1));
+                const float tot = warp_sum_f(s0 + s1);
+                c = __fdiv_rn(tot, fmaxf((float)n, k.sqrtS));
+              }
+              cq[q] = c;
+              const float thr = sp.cand_thr + c;
+              bool any = false;
+#pragma unroll
+              for (int j = 0; j < N; ++j) any |= a[j] > thr;
+              anyc[q] = __any_sync(FULL, any);
+              if (anyc[q]) {
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                  uint32_t bb = 0;
+#pragma unroll
+                  for (int e = 0; e < V; ++e) bb |= (a[g * V + e] > thr ? 1u : 0u) << e;
+                  cbits[q][g] = bb;
+                }
+              }
+            }
+          }
+          // ---- publish: common-mode estimate and candidate bits of (frame slot, row, segment) ----
+#pragma unroll
+          for (int q = 0; q < FL; ++q) {
+            const int fl = g0 + q;
+            if (fl >= nf) continue;
+            if (lane == 0) {
+              cmring[((size_t)fl * ring_rows + slot) * k.nseg + sg] = cq[q];
+              if (k.cm_keep) k.cm_keep[(((size_t)(fs + c0 + fl) * k.P + p) * k.H + row) * k.nseg + sg] = cq[q];
+            }
+            if (anyc[q]) {
+#pragma unroll
+              for (int g = 0; g < G; ++g) {
+                const int vi = g * 32 + lane;
+                if (cbits[q][g] && vi * V < k.S) {
+                  const int col = sg * k.S + vi * V;
+                  atomicOr(&bits[((size_t)fl * ring_rows + slot) * k.WPR + (col >> 5)], cbits[q][g] << (col & 31));
+                }
+              }
+            }
+          }
+        }
+        // ---- arrive; the last warp of a (frame slot, band) runs its sparse stage ----
+        __syncwarp();
+#pragma unroll 1
+        for (int q = 0; q < FL; ++q) {
+          const int fl = g0 + q;
+          if (fl >= nf) continue;
+          int last = 0;
+          if (lane == 0) {
+            __threadfence_block();
+            int *ctr = &cnt[(gb % 3) * kFCH + fl];
+            last = atomicAdd(ctr, 1) == NW - 1;
+            if (last) *ctr = 0;
+          }
+          last = __shfl_sync(FULL, last, 0);
+          if (last) {
+            __threadfence_block();
+            stream_sparse(sp, smem, fl, gb, fs);
+          }
+        }
+      }
+    }
+  }
+}
+
+}  // namespace pdp

@@ -89,7 +89,7 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("kernel", ["frames", "frames_pf", "lookback"])
+@pytest.mark.parametrize("kernel", ["stream", "frames", "frames_pf", "lookback"])
 @pytest.mark.parametrize("cm_mode", [0, 1, 2], ids=["median", "mean", "none"])
 @pytest.mark.parametrize("case", list(CASES), ids=list(CASES))
 def test_parity(oracle, case, cm_mode, kernel):
@@ -134,8 +134,8 @@ def test_integer_exact_suite(oracle):
     sig = sig + ph2 * rng.choice([0, 20, 60], (n, P, H, W))                  # neighbours, ties
     raw = torch.tensor((ped.numpy() + gain.numpy() * sig).astype(np.uint16))
     cfg = small(0, panels=P, rows=H, cols=W, seg_cols=S, seed_adu=50.5, cm_adu=20.5, photon_adu=100.0)
-    for cm_mode, kernel in ((0, "frames"), (0, "frames_pf"), (0, "lookback"), (1, "frames"), (2, "frames_pf"),
-                            (2, "lookback")):
+    for cm_mode, kernel in ((0, "stream"), (1, "stream"), (2, "stream"), (0, "frames"), (0, "frames_pf"), (0, "lookback"),
+                            (1, "frames"), (2, "frames_pf"), (2, "lookback")):
         g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
         rep = compare(o, g, panels=P, rows=H, cols=W)
@@ -148,7 +148,7 @@ def test_integer_exact_suite(oracle):
         assert rep.hits_oracle > 200
 
 
-@pytest.mark.parametrize("kernel", ["frames", "lookback"])
+@pytest.mark.parametrize("kernel", ["stream", "frames", "lookback"])
 def test_overflow_and_empty(oracle, kernel):
     cfg, n = small(0, rows=40, cols=128, seg_cols=64, occupancy=0.03), 3
     raw, ped, gain = make(cfg, n)
@@ -176,8 +176,11 @@ def test_overflow_and_empty(oracle, kernel):
 def test_chunking_determinism_accumulation_and_host_feed(oracle, monkeypatch):
     cfg, n = small(0, rows=50, cols=128, seg_cols=64, occupancy=0.02), 21
     raw, ped, gain = make(cfg, n)
-    ref = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
-    again = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
+    ref = gpu_run(cfg, raw, ped, gain, 0, kernel="stream")
+    again = gpu_run(cfg, raw, ped, gain, 0, kernel="stream")
+    staged = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
+    for k in ref:
+        assert np.array_equal(ref[k], staged[k]), k                          # both large-batch kernels agree bit for bit
     for k in ref:
         assert np.array_equal(ref[k], again[k]), k                           # bit-identical run to run
     monkeypatch.setenv("PDP_CHUNK_FRAMES", "4")                              # 6 chunks, ragged last one
