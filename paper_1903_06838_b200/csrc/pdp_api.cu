@@ -39,7 +39,7 @@ constexpr int kFramesPerCtaMax = 1024;
 struct StreamPlan {
   bool ok = false;
   int R = 0, NW = 0, FL = 1, bands_per_panel = 0, n_bands = 0;
-  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, smem = 0;
+  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, smem = 0;
 };
 
 }  // namespace
@@ -193,7 +193,7 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
 // The streaming kernel: one warp per (band row, segment), R = warps / segments rows per band.
 bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, StreamPlan &pl) {
   const int nseg = g.cols / g.seg_cols;
-  int R = std::min(pdp::kStreamMaxWarps / nseg, (int)g.rows);
+  int R = std::min(pdp::kDenseWarpsMax / nseg, (int)g.rows);
   if (R < 1 || (R < 2 && g.rows > 1)) return false;
   auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
   const uint32_t ring = 3u * (uint32_t)R;
@@ -204,7 +204,9 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
   pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
   pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
   pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
-  if (off > smem_limit) return false;
+  pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
+  pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
+  if (off > smem_limit || WPR > 32 || R > 254) return false;
   pl.R = R;
   pl.NW = R * nseg;
   pl.FL = (V * G <= 16) ? 2 : 1;
@@ -570,9 +572,11 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       s.off_done = spl.off_done;
       s.off_pref = spl.off_pref;
       s.off_phot = spl.off_phot;
+      s.off_list = spl.off_list;
+      s.off_rowmask = spl.off_rowmask;
       const int grid_s = std::min(c->num_sms, n);
       StreamFn sf = stream_kernel(pl.V, pl.G, spl.FL);
-      sf<<<grid_s, spl.NW * 32, spl.smem, st>>>(s);
+      sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);
       PDP_CUDA(c, cudaGetLastError());
       c->launches += 1;
       return PDP_OK;

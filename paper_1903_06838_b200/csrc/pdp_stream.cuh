@@ -28,7 +28,9 @@
 
 namespace pdp {
 
-constexpr int kStreamMaxWarps = 16;
+constexpr int kStreamMaxWarps = 16;      // dense + sparse warps of a CTA
+constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
+constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
 constexpr int kStreamThreads = kStreamMaxWarps * 32;
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
 constexpr int kMaxIt = 9;   // counting passes before the generic bisection takes over
@@ -38,8 +40,9 @@ struct SParams {
   const double *rg64;   // 1/gain in double (sparse stage)
   float big;            // BIG: power of two > 2 * (max |v1| + T_cm); pixels outside the mask get +BIG
   float cand_thr;       // T_seed - margin (margin covers the rounding of a + BIG)
-  int R, NW;            // rows per band, warps per CTA (= R * nseg)
-  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot;
+  int R, NW;            // rows per band, DENSE warps per CTA (= R * nseg)
+  uint32_t off_rowmask;  // [kFCH][3R] which words of a bitmap row are non-zero (WPR <= 32)
+  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list;
 };
 
 // ---- small helpers -------------------------------------------------------------------------------
@@ -193,21 +196,27 @@ __device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
   return h;
 }
 
-// ---- sparse stage of one (frame slot, band): run by ONE warp ------------------------------------
+// ---- sparse stage of one (frame group, band): run by ONE warp -----------------------------------
 // Evaluates the seed candidates of rows [r0-1, r0+R-2] of the band's panel (from row 0 for the first
-// band, through row H-1 for the last one): every window row then has its common-mode estimate.
-__device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int fl, int gb, int fs) {
+// band, through row H-1 for the last one: every window row then has its common-mode estimate) for
+// the nfr frames of the group.  The candidate bits are first compacted, in (frame, row, column)
+// order, into a list in shared memory (batches of kListCap), then every lane evaluates one
+// candidate at a time: all loads of a batch are in flight together and no lane idles.
+constexpr int kListCap = 128;
+
+__device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int g0, int nfr, int gb,
+                                              int fs, uint32_t *list) {
   const KParams &k = sp.k;
   const int lane = threadIdx.x & 31;
   const int R = sp.R, ring_rows = 3 * R;
-  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm) + (size_t)fl * ring_rows * k.nseg;
-  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits) + (size_t)fl * ring_rows * k.WPR;
+  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);
+  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);
   volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);
   uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);
   uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);
 
   const int chunk = gb / k.n_bands, band = gb - chunk * k.n_bands;
-  const int f = fs + chunk * kFCH + fl;
+  const int f0 = fs + chunk * kFCH + g0;
   const int p = band / k.bands_per_panel, bi = band - p * k.bands_per_panel, r0 = bi * R;
   const int ra = bi == 0 ? 0 : r0 - 1;
   const int rb = bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
@@ -216,86 +225,109 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
     const int q = r / R;
     return ((gb0 + q) % 3) * R + (r - q * R);
   };
-  const uint16_t *frame_raw = k.raw + (size_t)f * k.P * k.H * k.W;
-  const size_t fbase = (size_t)f * k.cap;
-  uint32_t base = pref[fl];
-  int phsum = 0;
-  const int total_words = (rb - ra + 1) * k.WPR;
-  for (int i0 = 0; i0 < total_words; i0 += 32) {
-    const int i = i0 + lane;
-    const bool valid = i < total_words;
-    const int rr = valid ? i / k.WPR : 0, wi = i - rr * k.WPR, row = ra + rr;
-    uint32_t *wp = bits + (size_t)slot_of(row) * k.WPR + wi;
-    uint32_t cand = valid ? *wp : 0u;
-    if (!__any_sync(FULL, cand != 0u)) continue;
-    uint32_t seedword = 0;
-    HitRec rec0{0.f, 0.f, 0.f, 0}, rec1{0.f, 0.f, 0.f, 0};
-    int kk = 0;
-    const float *cm_m1 = nullptr, *cm_0 = nullptr, *cm_p1 = nullptr;
-    if (cand) {
-      *wp = 0u;
-      cm_0 = cmring + (size_t)slot_of(row) * k.nseg;
-      if (row > 0) cm_m1 = cmring + (size_t)slot_of(row - 1) * k.nseg;
-      if (row < k.H - 1) cm_p1 = cmring + (size_t)slot_of(row + 1) * k.nseg;
-      while (cand) {
-        const int b = __ffs(cand) - 1;
-        cand &= cand - 1;
-        const int col = wi * 32 + b;
-        const Exact9 e9 = exact9_rows(k, sp.rg64, frame_raw, cm_m1, cm_0, cm_p1, p, row, col);
-        if (!e9.seed) continue;
-        seedword |= 1u << b;
-        const HitRec h = make_rec(e9, k.dE_ph);
-        phsum += h.n;
-        // accumulated image: one fire-and-forget RED per hit
-        if (h.n) red_add_u32(k.accum + ((size_t)p * k.H + row) * k.W + col, (uint32_t)h.n);
-        if (kk == 0) rec0 = h;
-        if (kk == 1) rec1 = h;
-        ++kk;
-      }
-    }
-    // ordered slots: lanes are in (row, word) order, bits in column order
-    int incl = kk;
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  const int nrows = rb - ra + 1;
+  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);
+  uint32_t base0 = pref[g0], base1 = nfr > 1 ? pref[g0 + 1] : 0u;
+  int ph0 = 0, ph1 = 0;
+  // lane <-> (frame of the group, row): the row's summary mask says which words hold candidates
+  const int n_tasks = nrows > 0 ? nfr * nrows : 0;
+  for (int t0 = 0; t0 < n_tasks; t0 += 32) {
+    const int t = t0 + lane;
+    const bool tv = t < n_tasks;
+    const int tq = (tv && t >= nrows) ? 1 : 0, trr = tv ? t - tq * nrows : 0;
+    const size_t rowslot = (size_t)(g0 + tq) * ring_rows + slot_of(ra + trr);
+    const uint32_t rmask = tv ? rowmask[rowslot] : 0u;
+    if (!__any_sync(FULL, rmask != 0u)) continue;
+    uint32_t *rowbits = bits + rowslot * k.WPR;
+    int mine = 0;
+    for (uint32_t m = rmask; m; m &= m - 1) mine += __popc(rowbits[__ffs(m) - 1]);
+    int incl = mine;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int t = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += t;
+      const int u = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += u;
     }
-    const int tot = __shfl_sync(FULL, incl, 31);
-    uint32_t pos = base + (uint32_t)(incl - kk);
-    int j = 0;
-    while (seedword) {
-      const int b = __ffs(seedword) - 1;
-      seedword &= seedword - 1;
-      if (pos < k.cap) {
-        const int col = wi * 32 + b;
-        HitRec h = j == 0 ? rec0 : rec1;
-        if (j >= 2)  // more than two seeds in one 32-pixel word: evaluate again
-          h = make_rec(exact9_rows(k, sp.rg64, frame_raw, cm_m1, cm_0, cm_p1, p, row, col), k.dE_ph);
-        k.hit_pixel[fbase + pos] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
-        k.hit_charge[fbase + pos] = h.E;
-        k.hit_nphot[fbase + pos] = h.n;
-        k.hit_dx[fbase + pos] = h.dx;
-        k.hit_dy[fbase + pos] = h.dy;
+    const int total = __shfl_sync(FULL, incl, 31);
+    const int my_first = incl - mine;
+    for (int b0 = 0; b0 < total; b0 += kListCap) {
+      // ---- compact the candidates [b0, b0 + kListCap) into the list, (frame, row, column) order ----
+      if (my_first < b0 + kListCap && my_first + mine > b0) {
+        int idx = my_first;
+        for (uint32_t m = rmask; m; m &= m - 1) {
+          const int wi = __ffs(m) - 1;
+          for (uint32_t wv = rowbits[wi]; wv; wv &= wv - 1) {
+            if (idx >= b0 && idx < b0 + kListCap)
+              list[idx - b0] = ((uint32_t)tq << 28) | ((uint32_t)trr << 20) | (uint32_t)(wi * 32 + __ffs(wv) - 1);
+            ++idx;
+          }
+        }
       }
-      ++pos;
-      ++j;
+      __syncwarp();
+      const int nb = min(kListCap, total - b0);
+      for (int i0 = 0; i0 < nb; i0 += 32) {
+        const bool have = i0 + lane < nb;
+        const uint32_t e = have ? list[i0 + lane] : 0u;
+        const int q = (int)(e >> 28), row = ra + (int)((e >> 20) & 0xffu), col = (int)(e & 0xfffffu);
+        bool seed = false;
+        HitRec h{0.f, 0.f, 0.f, 0};
+        if (have) {
+          const float *cmf = cmring + (size_t)(g0 + q) * ring_rows * k.nseg;
+          const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
+          const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : nullptr;
+          const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : nullptr;
+          const Exact9 e9 = exact9_rows(k, sp.rg64, k.raw + (size_t)(f0 + q) * npix, cm_m1, cm_0, cm_p1, p, row, col);
+          seed = e9.seed;
+          if (seed) h = make_rec(e9, k.dE_ph);
+        }
+        const unsigned sm = __ballot_sync(FULL, seed);
+        if (!sm) continue;
+        const unsigned m1 = __ballot_sync(FULL, seed && q == 1), m0 = sm & ~m1;
+        const unsigned lt = (1u << lane) - 1u;
+        if (seed) {
+          const uint32_t pos = q ? base1 + __popc(m1 & lt) : base0 + __popc(m0 & lt);
+          if (pos < k.cap) {
+            const size_t o = (size_t)(f0 + q) * k.cap + pos;
+            k.hit_pixel[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
+            k.hit_charge[o] = h.E;
+            k.hit_nphot[o] = h.n;
+            k.hit_dx[o] = h.dx;
+            k.hit_dy[o] = h.dy;
+          }
+          // accumulated image: one fire-and-forget RED per hit
+          if (h.n) red_add_u32(k.accum + ((size_t)p * k.H + row) * k.W + col, (uint32_t)h.n);
+        }
+        base0 += __popc(m0);
+        base1 += __popc(m1);
+        ph0 += warp_sum_i(seed && q == 0 ? h.n : 0);
+        if (m1) ph1 += warp_sum_i(seed && q == 1 ? h.n : 0);
+      }
+      __syncwarp();
     }
-    base += (uint32_t)tot;
+    if (rmask) {   // consumed: clear the words and the summary
+      for (uint32_t m = rmask; m; m &= m - 1) rowbits[__ffs(m) - 1] = 0u;
+      rowmask[rowslot] = 0u;
+    }
   }
-  phsum = warp_sum_i(phsum);
-  if (lane == 0) {
+  if (lane < nfr) {
+    const int fl = g0 + lane;
+    const uint32_t base = lane ? base1 : base0;
+    const uint32_t ph = phot[fl] + (uint32_t)(lane ? ph1 : ph0);
     if (band == k.n_bands - 1) {  // the frame is complete
-      k.hit_count[f] = base;
-      k.frame_photons[f] = phot[fl] + (uint32_t)phsum;
+      k.hit_count[f0 + lane] = base;
+      k.frame_photons[f0 + lane] = ph;
       if (base > k.cap) atomicOr(k.status, 1u);
       pref[fl] = 0u;
       phot[fl] = 0u;
     } else {
       pref[fl] = base;
-      phot[fl] += (uint32_t)phsum;
+      phot[fl] = ph;
     }
+  }
+  __syncwarp();
+  if (lane == 0) {
     __threadfence_block();
-    done[fl] = gb + 1;
+    done[g0] = gb + 1;
   }
   __syncwarp();
 }
@@ -310,7 +342,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const KParams &k = sp.k;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int nthreads = blockDim.x, NW = nthreads >> 5;
+  const int nthreads = blockDim.x, NW = sp.NW;   // NW dense warps, then kSparseWarps sparse warps
   const int R = sp.R, ring_rows = 3 * R;
   float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);          // [kFCH][3R][nseg]
   uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);    // [kFCH][3R][WPR]
@@ -324,11 +356,33 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const int FCn = fe - fs;
   if (FCn <= 0) return;
 
+  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);  // [kFCH][3R]
   for (int i = tid; i < kFCH * ring_rows * k.WPR; i += nthreads) bits[i] = 0u;
+  for (int i = tid; i < kFCH * ring_rows; i += nthreads) rowmask[i] = 0u;
   for (int i = tid; i < 3 * kFCH; i += nthreads) cnt[i] = 0;
   for (int i = tid; i < kFCH; i += nthreads) done[i] = 0, pref[i] = 0u, phot[i] = 0u;
   __syncthreads();
 
+  if (warp >= NW) {
+    // ===== sparse warps: task (band, frame group) -> warp (group index mod kSparseWarps) =====
+    const int sw = warp - NW;
+    uint32_t *list = reinterpret_cast<uint32_t *>(smem + sp.off_list) + sw * kListCap;
+    int gbs = 0;
+    for (int c0 = 0; c0 < FCn; c0 += kFCH) {
+      const int nf = min(kFCH, FCn - c0);
+      for (int band = 0; band < k.n_bands; ++band, ++gbs) {
+        for (int g0 = sw * FL; g0 < nf; g0 += kSparseWarps * FL) {
+          volatile int *ctr = &cnt[(gbs % 3) * kFCH + g0];
+          while (*ctr < NW) __nanosleep(64);   // every dense warp has published (frame group, band)
+          __threadfence_block();
+          __syncwarp();
+          if (lane == 0) *ctr = 0;
+          stream_sparse(sp, smem, g0, min(FL, nf - g0), gbs, fs, list);
+        }
+      }
+    }
+    return;
+  }
   const int tr = warp / k.nseg, sg = warp - tr * k.nseg;  // this warp's row of the band and segment
   const size_t npix = (size_t)k.P * k.H * k.W;
   const float BIG = sp.big, BIG2 = 4.f * sp.big;
@@ -385,11 +439,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           for (int e = 0; e < N / 2; ++e) w[q][e] = wn[q][e];
         if (g0 + FL < nf) fetch(g0 + FL);
         // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
-#pragma unroll
-        for (int q = 0; q < FL; ++q)
-          if (g0 + q < nf)
-            while (done[g0 + q] < gb - 1) {
-            }
+        while (done[g0] < gb - 1) {
+        }
 
         if (active) {
           float cq[FL];
@@ -444,7 +495,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
             bool have_lo = false, have_hi = false;
             bool fin = n_my < k.cm_min_count || n_my <= 0;  // c = 0: nothing to search
             bool failed = false;
-            int c_fin = 0;
+            int c_fin = 0, c_prev = 0;
+            float p_prev = 0.f;
             for (int it = 0; it < kMaxIt; ++it) {
               if (__all_sync(FULL, fin || failed)) break;
               float pv[FL];
@@ -470,6 +522,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
               const unsigned tot = (unsigned)warp_sum_i(__float2int_rn(pk));
               const int c = (int)((tot >> (16 * ms)) & 0xffffu);
               if (!fin && !failed) {
+                // density estimate: only from the first two pivots (wide, unbiased; brackets that
+                // survive later passes are the locally dense ones and would drag it down)
+                if (it == 1 && abs(c - c_prev) >= 8)
+                  apr = 0.75f * apr + 0.25f * fabsf(__fdividef(p_my - p_prev, (float)(c - c_prev)));
+                p_prev = p_my;
+                c_prev = c;
                 if (c >= kl && c <= acc_hi) {
                   fin = true;
                   c_fin = c;
@@ -480,7 +538,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
                   if (have_lo && have_hi) {
                     const float slope = __fdividef(hi - lo, (float)(ch - cl));
                     pn = fmaf(tgt - (float)cl, slope, lo);
-                    if (ch - cl >= 4) apr = 0.75f * apr + 0.25f * slope;
                     if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
                     if (!(pn > lo && pn < hi)) failed = true;   // no float strictly inside: ties
                   } else {
@@ -607,29 +664,17 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
                 if (cbits[q][g] && vi * V < k.S) {
                   const int col = sg * k.S + vi * V;
                   atomicOr(&bits[((size_t)fl * ring_rows + slot) * k.WPR + (col >> 5)], cbits[q][g] << (col & 31));
+                  atomicOr(&rowmask[(size_t)fl * ring_rows + slot], 1u << (col >> 5));
                 }
               }
             }
           }
         }
-        // ---- arrive; the last warp of a (frame slot, band) runs its sparse stage ----
+        // ---- arrive: the group's sparse warp starts once all NW dense warps have published ----
         __syncwarp();
-#pragma unroll 1
-        for (int q = 0; q < FL; ++q) {
-          const int fl = g0 + q;
-          if (fl >= nf) continue;
-          int last = 0;
-          if (lane == 0) {
-            __threadfence_block();
-            int *ctr = &cnt[(gb % 3) * kFCH + fl];
-            last = atomicAdd(ctr, 1) == NW - 1;
-            if (last) *ctr = 0;
-          }
-          last = __shfl_sync(FULL, last, 0);
-          if (last) {
-            __threadfence_block();
-            stream_sparse(sp, smem, fl, gb, fs);
-          }
+        if (lane == 0) {
+          __threadfence_block();
+          atomicAdd(&cnt[(gb % 3) * kFCH + g0], 1);
         }
       }
     }
