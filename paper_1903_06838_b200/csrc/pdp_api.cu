@@ -39,7 +39,7 @@ constexpr int kFramesPerCtaMax = 1024;
 struct StreamPlan {
   bool ok = false;
   int R = 0, NW = 0, FL = 1, bands_per_panel = 0, n_bands = 0;
-  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, smem = 0;
+  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, off_ring = 0, smem = 0;
 };
 
 }  // namespace
@@ -206,11 +206,11 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
   pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
   pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
   pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
+  pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
   if (off > smem_limit || WPR > 32 || R > 254) return false;
   pl.R = R;
   pl.NW = R * nseg;
-  pl.FL = (V * G <= 16) ? 2 : 1;
-  if (const char *e = std::getenv("PDP_STREAM_FL")) pl.FL = std::atoi(e) == 1 ? 1 : pl.FL;
+  pl.FL = 1;
   pl.bands_per_panel = (g.rows + R - 1) / R;
   pl.n_bands = pl.bands_per_panel * g.panels;
   pl.smem = off;
@@ -238,8 +238,9 @@ StreamFn stream_kernel_for(int V, int G) {
   return nullptr;
 }
 StreamFn stream_kernel(int V, int G, int FL) {
-  if (V == 8 && G > 2) return FL == 1 ? (G == 3 ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 4, 1>) : nullptr;
-  return FL == 2 ? stream_kernel_for<2>(V, G) : stream_kernel_for<1>(V, G);
+  if (FL != 1) return nullptr;
+  if (V == 8 && G > 2) return G == 3 ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 4, 1>;
+  return stream_kernel_for<1>(V, G);
 }
 using FramesFn = void (*)(const FParams);
 
@@ -574,6 +575,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       s.off_phot = spl.off_phot;
       s.off_list = spl.off_list;
       s.off_rowmask = spl.off_rowmask;
+      s.off_ring = spl.off_ring;
       const int grid_s = std::min(c->num_sms, n);
       StreamFn sf = stream_kernel(pl.V, pl.G, spl.FL);
       sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);

@@ -33,6 +33,7 @@ constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
 constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
 constexpr int kStreamThreads = kStreamMaxWarps * 32;
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
+constexpr int kRingD = 6;  // frame groups in flight per warp (cp.async ring)
 constexpr int kMaxIt = 9;   // counting passes before the generic bisection takes over
 
 struct SParams {
@@ -42,7 +43,7 @@ struct SParams {
   float cand_thr;       // T_seed - margin (margin covers the rounding of a + BIG)
   int R, NW;            // rows per band, DENSE warps per CTA (= R * nseg)
   uint32_t off_rowmask;  // [kFCH][3R] which words of a bitmap row are non-zero (WPR <= 32)
-  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list;
+  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list, off_ring;
 };
 
 // ---- small helpers -------------------------------------------------------------------------------
@@ -70,6 +71,36 @@ struct VecLoadG<8> {
     w[1] = t.y;
     w[2] = t.z;
     w[3] = t.w;
+  }
+};
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void *dst_smem, const void *src) {  // SASS: LDGSTS
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "n"(BYTES) : "memory");
+}
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async_s(uint32_t dst_smem, const void *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst_smem), "l"(src), "n"(BYTES) : "memory");
+}
+template <int V>
+struct VecLoadS;  // V uint16 pixels from a shared-memory byte address
+template <>
+struct VecLoadS<2> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[1]) {
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w[0]) : "r"(a));
+  }
+};
+template <>
+struct VecLoadS<4> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[2]) {
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(w[0]), "=r"(w[1]) : "r"(a));
+  }
+};
+template <>
+struct VecLoadS<8> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[4]) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(a));
   }
 };
 
@@ -203,39 +234,41 @@ __device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
 // order, into a list in shared memory (batches of kListCap), then every lane evaluates one
 // candidate at a time: all loads of a batch are in flight together and no lane idles.
 constexpr int kListCap = 128;
+constexpr int kGF = 4;   // frame slots per sparse task
 
-__device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int g0, int nfr, int gb,
-                                              int fs, uint32_t *list) {
+struct BandDesc {      // one band of one panel, as the sparse warps see it
+  int gb, band, p, bi; // running band index (over chunks), band of the frame, panel, band of the panel
+};
+
+__device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int g0, int nfr,
+                                              const BandDesc &bd, int f0, uint32_t *list) {
   const KParams &k = sp.k;
   const int lane = threadIdx.x & 31;
   const int R = sp.R, ring_rows = 3 * R;
   float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);
   uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);
+  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);
   volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);
   uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);
   uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);
 
-  const int chunk = gb / k.n_bands, band = gb - chunk * k.n_bands;
-  const int f0 = fs + chunk * kFCH + g0;
-  const int p = band / k.bands_per_panel, bi = band - p * k.bands_per_panel, r0 = bi * R;
-  const int ra = bi == 0 ? 0 : r0 - 1;
-  const int rb = bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
-  const int gb0 = gb - bi;  // running band index of band 0 of this panel
-  auto slot_of = [&](int r) {
-    const int q = r / R;
-    return ((gb0 + q) % 3) * R + (r - q * R);
-  };
-  const size_t npix = (size_t)k.P * k.H * k.W;
+  const int p = bd.p, r0 = bd.bi * R;
+  const int ra = bd.bi == 0 ? 0 : r0 - 1;
+  const int rb = bd.bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
   const int nrows = rb - ra + 1;
-  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);
-  uint32_t base0 = pref[g0], base1 = nfr > 1 ? pref[g0 + 1] : 0u;
-  int ph0 = 0, ph1 = 0;
+  // ring slot of row r in [r0-2, r0+R]: bands gb-1, gb, gb+1 occupy slots (gb-1)%3, gb%3, (gb+1)%3
+  const int s_prev = ((bd.gb + 2) % 3) * R, s_cur = (bd.gb % 3) * R, s_next = ((bd.gb + 1) % 3) * R;
+  auto slot_of = [&](int r) { return r < r0 ? s_prev + (r - r0 + R) : (r < r0 + R ? s_cur + (r - r0) : s_next + (r - r0 - R)); };
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  uint32_t base = lane < nfr ? pref[g0 + lane] : 0u;   // lane q holds the running totals of frame q
+  int ph = 0;
   // lane <-> (frame of the group, row): the row's summary mask says which words hold candidates
   const int n_tasks = nrows > 0 ? nfr * nrows : 0;
   for (int t0 = 0; t0 < n_tasks; t0 += 32) {
     const int t = t0 + lane;
     const bool tv = t < n_tasks;
-    const int tq = (tv && t >= nrows) ? 1 : 0, trr = tv ? t - tq * nrows : 0;
+    int tq = 0, trr = tv ? t : 0;
+    while (trr >= nrows) trr -= nrows, ++tq;
     const size_t rowslot = (size_t)(g0 + tq) * ring_rows + slot_of(ra + trr);
     const uint32_t rmask = tv ? rowmask[rowslot] : 0u;
     if (!__any_sync(FULL, rmask != 0u)) continue;
@@ -280,12 +313,20 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
           seed = e9.seed;
           if (seed) h = make_rec(e9, k.dE_ph);
         }
-        const unsigned sm = __ballot_sync(FULL, seed);
-        if (!sm) continue;
-        const unsigned m1 = __ballot_sync(FULL, seed && q == 1), m0 = sm & ~m1;
+        if (!__any_sync(FULL, seed)) continue;
         const unsigned lt = (1u << lane) - 1u;
+        unsigned mymask = 0u;
+        int add = 0, addph = 0;
+        for (int qq = 0; qq < nfr; ++qq) {
+          const unsigned m = __ballot_sync(FULL, seed && q == qq);
+          if (!m) continue;
+          const int phq = warp_sum_i(seed && q == qq ? h.n : 0);
+          if (q == qq) mymask = m;
+          if (lane == qq) add = __popc(m), addph = phq;
+        }
+        const uint32_t b_q = __shfl_sync(FULL, base, q);
         if (seed) {
-          const uint32_t pos = q ? base1 + __popc(m1 & lt) : base0 + __popc(m0 & lt);
+          const uint32_t pos = b_q + __popc(mymask & lt);
           if (pos < k.cap) {
             const size_t o = (size_t)(f0 + q) * k.cap + pos;
             k.hit_pixel[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
@@ -297,10 +338,8 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
           // accumulated image: one fire-and-forget RED per hit
           if (h.n) red_add_u32(k.accum + ((size_t)p * k.H + row) * k.W + col, (uint32_t)h.n);
         }
-        base0 += __popc(m0);
-        base1 += __popc(m1);
-        ph0 += warp_sum_i(seed && q == 0 ? h.n : 0);
-        if (m1) ph1 += warp_sum_i(seed && q == 1 ? h.n : 0);
+        base += (uint32_t)add;
+        ph += addph;
       }
       __syncwarp();
     }
@@ -311,23 +350,22 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
   }
   if (lane < nfr) {
     const int fl = g0 + lane;
-    const uint32_t base = lane ? base1 : base0;
-    const uint32_t ph = phot[fl] + (uint32_t)(lane ? ph1 : ph0);
-    if (band == k.n_bands - 1) {  // the frame is complete
+    const uint32_t pht = phot[fl] + (uint32_t)ph;
+    if (bd.band == k.n_bands - 1) {  // the frame is complete
       k.hit_count[f0 + lane] = base;
-      k.frame_photons[f0 + lane] = ph;
+      k.frame_photons[f0 + lane] = pht;
       if (base > k.cap) atomicOr(k.status, 1u);
       pref[fl] = 0u;
       phot[fl] = 0u;
     } else {
       pref[fl] = base;
-      phot[fl] = ph;
+      phot[fl] = pht;
     }
   }
   __syncwarp();
   if (lane == 0) {
     __threadfence_block();
-    done[g0] = gb + 1;
+    done[g0] = bd.gb + 1;
   }
   __syncwarp();
 }
@@ -346,7 +384,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const int R = sp.R, ring_rows = 3 * R;
   float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);          // [kFCH][3R][nseg]
   uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);    // [kFCH][3R][WPR]
-  int *cnt = reinterpret_cast<int *>(smem + sp.off_cnt);                // [3][kFCH]
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + sp.off_cnt);      // [3][kFCH/kGF] mbarriers: NW*kGF arrivals
   volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);  // [kFCH]
   uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);    // [kFCH]
   uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);    // [kFCH]
@@ -359,26 +397,29 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);  // [kFCH][3R]
   for (int i = tid; i < kFCH * ring_rows * k.WPR; i += nthreads) bits[i] = 0u;
   for (int i = tid; i < kFCH * ring_rows; i += nthreads) rowmask[i] = 0u;
-  for (int i = tid; i < 3 * kFCH; i += nthreads) cnt[i] = 0;
+  if (tid == 0) {
+    for (int i = 0; i < 3 * (kFCH / kGF); ++i) mbar_init(&bar[i], (uint32_t)(NW * kGF));
+    fence_mbar_init();
+  }
   for (int i = tid; i < kFCH; i += nthreads) done[i] = 0, pref[i] = 0u, phot[i] = 0u;
   __syncthreads();
 
   if (warp >= NW) {
-    // ===== sparse warps: task (band, frame group) -> warp (group index mod kSparseWarps) =====
+    // ===== sparse warps: task (band, group of kGF frame slots) -> warp (group index mod kSparseWarps) =====
     const int sw = warp - NW;
     uint32_t *list = reinterpret_cast<uint32_t *>(smem + sp.off_list) + sw * kListCap;
-    int gbs = 0;
+    BandDesc bd{0, 0, 0, 0};
     for (int c0 = 0; c0 < FCn; c0 += kFCH) {
       const int nf = min(kFCH, FCn - c0);
-      for (int band = 0; band < k.n_bands; ++band, ++gbs) {
-        for (int g0 = sw * FL; g0 < nf; g0 += kSparseWarps * FL) {
-          volatile int *ctr = &cnt[(gbs % 3) * kFCH + g0];
-          while (*ctr < NW) __nanosleep(64);   // every dense warp has published (frame group, band)
-          __threadfence_block();
-          __syncwarp();
-          if (lane == 0) *ctr = 0;
-          stream_sparse(sp, smem, g0, min(FL, nf - g0), gbs, fs, list);
+      bd.band = 0, bd.p = 0, bd.bi = 0;
+      for (; bd.band < k.n_bands; ++bd.band, ++bd.gb) {
+        for (int g0 = sw * kGF; g0 < nf; g0 += kSparseWarps * kGF) {
+          const int nfr = min(kGF, nf - g0);
+          // every dense warp has published (frame group, band): acquire on the group's mbarrier
+          mbar_wait(&bar[(bd.gb % 3) * (kFCH / kGF) + g0 / kGF], (uint32_t)(bd.gb / 3) & 1u);
+          stream_sparse(sp, smem, g0, nfr, bd, fs + c0 + g0, list);
         }
+        if (++bd.bi == k.bands_per_panel) bd.bi = 0, ++bd.p;
       }
     }
     return;
@@ -390,6 +431,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
   float mK[N], mRg[N], mNpf[N];
   constexpr int NS = (N + 2) / 3;  // pixels per lane sampled for the first pivot (every third)
+  static_assert(FL == 1, "the frame loop below advances one frame per iteration");
+  uint32_t vmask = 0;              // which of this lane's G vectors lie inside the segment
+#pragma unroll
+  for (int g = 0; g < G; ++g) vmask |= ((g * 32 + lane) * V < k.S ? 1u : 0u) << g;
+  constexpr uint32_t kSlotBytes = N * 64;   // one frame of one warp in the ring (32 lanes x N pixels)
+  const uint32_t ring_lane = smem_u32(smem + sp.off_ring) + (uint32_t)warp * kRingD * kSlotBytes + (uint32_t)lane * (V * 2);
 
   int gb = 0;
   for (int c0 = 0; c0 < FCn; c0 += kFCH) {
@@ -414,33 +461,46 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           }
         }
       }
-      const uint16_t *rowp = k.raw + (size_t)(fs + c0) * npix + rowoff;
-      uint32_t wn[FL][N / 2];
-      auto fetch = [&](int g0) {
+      // raw pixels: per-warp ring of kRingD frames filled by cp.async (LDGSTS); every lane copies and
+      // later reads only its own vectors, so cp.async.wait_group is all the synchronisation needed
+      const uint16_t *src = k.raw + (size_t)(fs + c0) * npix + rowoff + lane * V;
+      int issued = 0;
+      uint32_t islot = 0, rslot = 0;
+      auto issue = [&]() {
+        if (active && issued < nf) {
 #pragma unroll
-        for (int q = 0; q < FL; ++q)
-#pragma unroll
-          for (int g = 0; g < G; ++g) {
-            const int vi = g * 32 + lane;
-            uint32_t t[V / 2];
-#pragma unroll
-            for (int e = 0; e < V / 2; ++e) t[e] = 0u;
-            if (active && g0 + q < nf && vi * V < k.S) VecLoadG<V>::ld(rowp + (size_t)(g0 + q) * npix + vi * V, t);
-#pragma unroll
-            for (int e = 0; e < V / 2; ++e) wn[q][g * (V / 2) + e] = t[e];
-          }
+          for (int g = 0; g < G; ++g)
+            if ((vmask >> g) & 1u) cp_async_s<V * 2>(ring_lane + islot + g * (64 * V), src + g * (32 * V));
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        src += npix;
+        ++issued;
+        islot = islot + kSlotBytes == kRingD * kSlotBytes ? 0u : islot + kSlotBytes;
       };
-      fetch(0);
-      for (int g0 = 0; g0 < nf; g0 += FL) {
+#pragma unroll 1
+      for (int d = 0; d < kRingD - 1; ++d) issue();
+      // running pointers of what this warp publishes per frame
+      float *cm_p = cmring + (size_t)slot * k.nseg + sg;
+      uint32_t *bits_p = bits + (size_t)slot * k.WPR;
+      uint32_t *rowmask_p = rowmask + slot;
+      uint64_t *bar_p = bar + (gb % 3) * (kFCH / kGF);
+      float *keep_p = k.cm_keep ? k.cm_keep + (((size_t)(fs + c0) * k.P + p) * k.H + row) * k.nseg + sg : nullptr;
+      for (int g0 = 0; g0 < nf; ++g0) {
+        issue();
+        asm volatile("cp.async.wait_group %0;" ::"n"(kRingD - 1) : "memory");
         uint32_t w[FL][N / 2];
 #pragma unroll
-        for (int q = 0; q < FL; ++q)
+        for (int g = 0; g < G; ++g) {
+          uint32_t t[V / 2];
+          VecLoadS<V>::ld(ring_lane + rslot + g * (64 * V), t);
 #pragma unroll
-          for (int e = 0; e < N / 2; ++e) w[q][e] = wn[q][e];
-        if (g0 + FL < nf) fetch(g0 + FL);
-        // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
-        while (done[g0] < gb - 1) {
+          for (int e = 0; e < V / 2; ++e) w[0][g * (V / 2) + e] = t[e];
         }
+        rslot = rslot + kSlotBytes == kRingD * kSlotBytes ? 0u : rslot + kSlotBytes;
+        // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
+        if ((g0 & (kGF - 1)) == 0)
+          while (done[g0] < gb - 1) {
+          }
 
         if (active) {
           float cq[FL];
@@ -649,34 +709,32 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
             }
           }
           // ---- publish: common-mode estimate and candidate bits of (frame slot, row, segment) ----
+          if (lane == 0) {
+            *cm_p = cq[0];
+            if (keep_p) *keep_p = cq[0];
+          }
+          if (anyc[0]) {
 #pragma unroll
-          for (int q = 0; q < FL; ++q) {
-            const int fl = g0 + q;
-            if (fl >= nf) continue;
-            if (lane == 0) {
-              cmring[((size_t)fl * ring_rows + slot) * k.nseg + sg] = cq[q];
-              if (k.cm_keep) k.cm_keep[(((size_t)(fs + c0 + fl) * k.P + p) * k.H + row) * k.nseg + sg] = cq[q];
-            }
-            if (anyc[q]) {
-#pragma unroll
-              for (int g = 0; g < G; ++g) {
-                const int vi = g * 32 + lane;
-                if (cbits[q][g] && vi * V < k.S) {
-                  const int col = sg * k.S + vi * V;
-                  atomicOr(&bits[((size_t)fl * ring_rows + slot) * k.WPR + (col >> 5)], cbits[q][g] << (col & 31));
-                  atomicOr(&rowmask[(size_t)fl * ring_rows + slot], 1u << (col >> 5));
-                }
+            for (int g = 0; g < G; ++g) {
+              if (cbits[0][g] && ((vmask >> g) & 1u)) {
+                const int col = sg * k.S + (g * 32 + lane) * V;
+                atomicOr(bits_p + (col >> 5), cbits[0][g] << (col & 31));
+                atomicOr(rowmask_p, 1u << (col >> 5));
               }
             }
           }
         }
-        // ---- arrive: the group's sparse warp starts once all NW dense warps have published ----
+        cm_p += ring_rows * k.nseg;
+        bits_p += ring_rows * k.WPR;
+        rowmask_p += ring_rows;
+        if (keep_p) keep_p += (size_t)k.P * k.H * k.nseg;
+        // ---- arrive (release, no fence: the prefetch ring stays in flight) ----
         __syncwarp();
-        if (lane == 0) {
-          __threadfence_block();
-          atomicAdd(&cnt[(gb % 3) * kFCH + g0], 1);
-        }
+        if (lane == 0) mbar_arrive(bar_p + (g0 >> 2));
       }
+      // frame slots of the last, partial group that hold no frame still owe their arrivals
+      if (lane == 0)
+        for (int fl = nf; fl < ((nf + kGF - 1) & ~(kGF - 1)); ++fl) mbar_arrive(&bar[(gb % 3) * (kFCH / kGF) + fl / kGF]);
     }
   }
 }
