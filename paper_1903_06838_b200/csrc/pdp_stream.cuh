@@ -544,84 +544,59 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
                 pq[q] = fminf(fmaxf(est, -k.T_cm), k.T_cm);
               }
             }
-            // ---- lock-step search; lanes [q*GL, (q+1)*GL) steer search q ----
-            const int n_my = FL == 2 ? (ms ? nq[FL - 1] : nq[0]) : nq[0];
+            // ---- safeguarded secant search for a pivot whose rank is kl .. kh+1 ----
+            // (all values are warp-uniform; state: 0 searching, 1 found, 2 failed -> generic bisection)
+            const int n_my = nq[0];
             const int kl = (n_my - 1) >> 1, kh = n_my >> 1;
-            const int acc_hi = kh + 1;                  // accepted ranks of a pivot: kl .. kh+1
             const float tgt = 0.5f * (float)(kl + kh + 1);
-            float p_my = FL == 2 ? (ms ? pq[FL - 1] : pq[0]) : pq[0];
-            float lo = 0.f, hi = 0.f;
-            int cl = 0, ch = 0;
-            bool have_lo = false, have_hi = false;
-            bool fin = n_my < k.cm_min_count || n_my <= 0;  // c = 0: nothing to search
-            bool failed = false;
-            int c_fin = 0, c_prev = 0;
-            float p_prev = 0.f;
-            for (int it = 0; it < kMaxIt; ++it) {
-              if (__all_sync(FULL, fin || failed)) break;
-              float pv[FL];
+            float p_my = pq[0], p_prev = 0.f, lo = -k.T_cm, hi = k.T_cm;
+            int c_prev = 0, c_fin = 0;
+            int state = (n_my < k.cm_min_count || n_my <= 0) ? 1 : 0;   // c = 0: nothing to search
+#pragma unroll 1
+            for (int it = 0; it < kMaxIt && state == 0; ++it) {
+              float a0 = 0.f, a1 = 0.f, a2 = 0.f;
 #pragma unroll
-              for (int q = 0; q < FL; ++q) pv[q] = __shfl_sync(FULL, p_my, q * GL);
-              float pk;
-              {
-                float a0[FL], a1[FL], a2[FL];
-#pragma unroll
-                for (int q = 0; q < FL; ++q) {
-                  a0[q] = a1[q] = a2[q] = 0.f;
-#pragma unroll
-                  for (int j = 0; j < N; ++j) {
-                    const float d = set_lt(bq[q][j], pv[q]);
-                    if (j % 3 == 0) a0[q] += d;
-                    else if (j % 3 == 1) a1[q] += d;
-                    else a2[q] += d;
-                  }
-                }
-                pk = a0[0] + a1[0] + a2[0];
-                if constexpr (FL == 2) pk = fmaf(a0[1] + a1[1] + a2[1], 65536.f, pk);
+              for (int j = 0; j < N; ++j) {
+                const float d = set_lt(bq[0][j], p_my);
+                if (j % 3 == 0) a0 += d;
+                else if (j % 3 == 1) a1 += d;
+                else a2 += d;
               }
-              const unsigned tot = (unsigned)warp_sum_i(__float2int_rn(pk));
-              const int c = (int)((tot >> (16 * ms)) & 0xffffu);
-              if (!fin && !failed) {
-                // density estimate: only from the first two pivots (wide, unbiased; brackets that
-                // survive later passes are the locally dense ones and would drag it down)
-                if (it == 1 && abs(c - c_prev) >= 8)
-                  apr = 0.75f * apr + 0.25f * fabsf(__fdividef(p_my - p_prev, (float)(c - c_prev)));
-                p_prev = p_my;
-                c_prev = c;
-                if (c >= kl && c <= acc_hi) {
-                  fin = true;
-                  c_fin = c;
-                } else {
-                  if (c < kl) lo = p_my, cl = c, have_lo = true;
-                  else hi = p_my, ch = c, have_hi = true;
-                  float pn;
-                  if (have_lo && have_hi) {
-                    const float slope = __fdividef(hi - lo, (float)(ch - cl));
-                    pn = fmaf(tgt - (float)cl, slope, lo);
-                    if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
-                    if (!(pn > lo && pn < hi)) failed = true;   // no float strictly inside: ties
-                  } else {
-                    pn = fmaf(tgt - (float)c, apr, p_my);
-                  }
-                  p_my = pn;
-                }
+              const int c = warp_sum_i(__float2int_rn(a0 + a1 + a2));
+              if ((unsigned)(c - kl) <= (unsigned)(kh + 1 - kl)) {
+                state = 1;
+                c_fin = c;
+                break;
               }
+              // secant through the last two points (first step: the running density estimate, which
+              // is refreshed only from the first, wide pair), kept inside the bracket (lo, hi)
+              float slope = apr;
+              if (it > 0 && c != c_prev) {
+                slope = __fdividef(p_my - p_prev, (float)(c - c_prev));
+                if (it == 1 && abs(c - c_prev) >= 8) apr = 0.75f * apr + 0.25f * slope;
+              }
+              if (c < kl) lo = p_my; else hi = p_my;
+              p_prev = p_my;
+              c_prev = c;
+              float pn = fmaf(tgt - (float)c, slope, p_my);
+              if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
+              if (!(pn > lo && pn < hi)) state = 2;   // no float strictly inside: ties
+              p_my = pn;
             }
-            if (!fin) failed = true;
+            const bool failed = state != 1;
             // ---- read the order statistics ----
 #pragma unroll
             for (int q = 0; q < FL; ++q) {
-              const int src = q * GL;
-              const bool f_q = __shfl_sync(FULL, (int)failed, src) != 0;
-              const float p_q = __shfl_sync(FULL, p_my, src);
-              const int d_q = __shfl_sync(FULL, c_fin - kl, src);
+              const bool f_q = failed;
+              const float p_q = p_my;
+              const int d_q = c_fin - kl;
               const int n_q = nq[q];
               const int kl_q = (n_q - 1) >> 1;
               const bool even = (n_q & 1) == 0;
               float c = 0.f;
               if (n_q >= k.cm_min_count && n_q > 0) {
                 if (f_q) {
-                  float apr2 = __shfl_sync(FULL, apr, src);   // one value for the whole warp
+                  float apr2 = apr;
                   c = warp_median<N>(bq[q], n_q, pq[q], k.T_cm, apr2);
                 } else if (!even) {
                   c = d_q == 0 ? min_ge<N>(bq[q], p_q, BIG2) : max_lt<N>(bq[q], p_q, BIG2);
