@@ -28,7 +28,7 @@
 
 namespace pdp {
 
-constexpr int kStreamMaxWarps = 16;      // dense + sparse warps of a CTA
+constexpr int kStreamMaxWarps = 20;      // dense + sparse warps of a CTA
 constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
 constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
 constexpr int kStreamThreads = kStreamMaxWarps * 32;
@@ -77,6 +77,16 @@ struct VecLoadG<8> {
 template <int BYTES>
 __device__ __forceinline__ void cp_async(void *dst_smem, const void *src) {  // SASS: LDGSTS
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "n"(BYTES) : "memory");
+}
+
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // acquire when it succeeds
+  uint32_t ok;
+  asm volatile(
+      "{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+  return ok != 0;
 }
 
 template <int BYTES>
@@ -416,7 +426,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
         for (int g0 = sw * kGF; g0 < nf; g0 += kSparseWarps * kGF) {
           const int nfr = min(kGF, nf - g0);
           // every dense warp has published (frame group, band): acquire on the group's mbarrier
-          mbar_wait(&bar[(bd.gb % 3) * (kFCH / kGF) + g0 / kGF], (uint32_t)(bd.gb / 3) & 1u);
+          while (!mbar_test(&bar[(bd.gb % 3) * (kFCH / kGF) + g0 / kGF], (uint32_t)(bd.gb / 3) & 1u))
+            __nanosleep(256);   // a sleeping warp costs no issue slots; a sparse task lasts microseconds
           stream_sparse(sp, smem, g0, nfr, bd, fs + c0 + g0, list);
         }
         if (++bd.bi == k.bands_per_panel) bd.bi = 0, ++bd.p;
@@ -480,6 +491,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
 #pragma unroll 1
       for (int d = 0; d < kRingD - 1; ++d) issue();
       // running pointers of what this warp publishes per frame
+      const int cm_stride = ring_rows * k.nseg, bits_stride = ring_rows * k.WPR;
+      const size_t keep_stride = (size_t)k.P * k.H * k.nseg;
       float *cm_p = cmring + (size_t)slot * k.nseg + sg;
       uint32_t *bits_p = bits + (size_t)slot * k.WPR;
       uint32_t *rowmask_p = rowmask + slot;
@@ -699,10 +712,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
             }
           }
         }
-        cm_p += ring_rows * k.nseg;
-        bits_p += ring_rows * k.WPR;
+        cm_p += cm_stride;
+        bits_p += bits_stride;
         rowmask_p += ring_rows;
-        if (keep_p) keep_p += (size_t)k.P * k.H * k.nseg;
+        if (keep_p) keep_p += keep_stride;
         // ---- arrive (release, no fence: the prefetch ring stays in flight) ----
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_p + (g0 >> 2));
