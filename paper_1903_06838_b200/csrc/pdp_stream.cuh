@@ -79,6 +79,9 @@ __device__ __forceinline__ void cp_async(void *dst_smem, const void *src) {  // 
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst_smem)), "l"(src), "n"(BYTES) : "memory");
 }
 
+__device__ __forceinline__ void mbar_arrive_n(uint64_t *bar, uint32_t n) {   // release; counts n arrivals
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
+}
 __device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // acquire when it succeeds
   uint32_t ok;
   asm volatile(
@@ -244,14 +247,15 @@ __device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
 // order, into a list in shared memory (batches of kListCap), then every lane evaluates one
 // candidate at a time: all loads of a batch are in flight together and no lane idles.
 constexpr int kListCap = 128;
-constexpr int kGF = 4;   // frame slots per sparse task
+constexpr int kGF = 4;   // frame slots per sparse task (1, 2 or 4, so that every sparse warp has one task per band)
+static_assert(kFCH == kGF * kSparseWarps, "one task per sparse warp and band");
 
 struct BandDesc {      // one band of one panel, as the sparse warps see it
   int gb, band, p, bi; // running band index (over chunks), band of the frame, panel, band of the panel
 };
 
 __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *smem, int g0, int nfr,
-                                              const BandDesc &bd, int f0, uint32_t *list) {
+                                              const BandDesc &bd, int f0, uint32_t *list, int done_idx) {
   const KParams &k = sp.k;
   const int lane = threadIdx.x & 31;
   const int R = sp.R, ring_rows = 3 * R;
@@ -375,7 +379,7 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
   __syncwarp();
   if (lane == 0) {
     __threadfence_block();
-    done[g0] = bd.gb + 1;
+    done[done_idx] = bd.gb + 1;
   }
   __syncwarp();
 }
@@ -408,7 +412,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   for (int i = tid; i < kFCH * ring_rows * k.WPR; i += nthreads) bits[i] = 0u;
   for (int i = tid; i < kFCH * ring_rows; i += nthreads) rowmask[i] = 0u;
   if (tid == 0) {
-    for (int i = 0; i < 3 * (kFCH / kGF); ++i) mbar_init(&bar[i], (uint32_t)(NW * kGF));
+    for (int i = 0; i < 3 * kSparseWarps; ++i) mbar_init(&bar[i], (uint32_t)(NW * kGF));
     fence_mbar_init();
   }
   for (int i = tid; i < kFCH; i += nthreads) done[i] = 0, pref[i] = 0u, phot[i] = 0u;
@@ -422,13 +426,16 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
     for (int c0 = 0; c0 < FCn; c0 += kFCH) {
       const int nf = min(kFCH, FCn - c0);
       bd.band = 0, bd.p = 0, bd.bi = 0;
+      const int gsh = nf <= kSparseWarps ? 0 : (nf <= 2 * kSparseWarps ? 1 : 2);   // log2(frames per task)
       for (; bd.band < k.n_bands; ++bd.band, ++bd.gb) {
-        for (int g0 = sw * kGF; g0 < nf; g0 += kSparseWarps * kGF) {
-          const int nfr = min(kGF, nf - g0);
+        const int g0 = sw << gsh;   // group sw = frame slots [sw*gf, sw*gf + gf)
+        if (g0 < nf) {
           // every dense warp has published (frame group, band): acquire on the group's mbarrier
-          while (!mbar_test(&bar[(bd.gb % 3) * (kFCH / kGF) + g0 / kGF], (uint32_t)(bd.gb / 3) & 1u))
+          while (!mbar_test(&bar[(bd.gb % 3) * kSparseWarps + sw], (uint32_t)(bd.gb / 3) & 1u))
             __nanosleep(256);   // a sleeping warp costs no issue slots; a sparse task lasts microseconds
-          stream_sparse(sp, smem, g0, nfr, bd, fs + c0 + g0, list);
+          stream_sparse(sp, smem, g0, min(1 << gsh, nf - g0), bd, fs + c0 + g0, list, sw);
+        } else if (lane == 0) {
+          done[sw] = bd.gb + 1;
         }
         if (++bd.bi == k.bands_per_panel) bd.bi = 0, ++bd.p;
       }
@@ -452,6 +459,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   int gb = 0;
   for (int c0 = 0; c0 < FCn; c0 += kFCH) {
     const int nf = min(kFCH, FCn - c0);
+    const int gsh = nf <= kSparseWarps ? 0 : (nf <= 2 * kSparseWarps ? 1 : 2);   // log2(frames per sparse task)
     for (int band = 0; band < k.n_bands; ++band, ++gb) {
       const int p = band / k.bands_per_panel, r0 = (band - p * k.bands_per_panel) * R;
       const int row = r0 + tr;
@@ -496,7 +504,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
       float *cm_p = cmring + (size_t)slot * k.nseg + sg;
       uint32_t *bits_p = bits + (size_t)slot * k.WPR;
       uint32_t *rowmask_p = rowmask + slot;
-      uint64_t *bar_p = bar + (gb % 3) * (kFCH / kGF);
+      uint64_t *bar_p = bar + (gb % 3) * kSparseWarps;
       float *keep_p = k.cm_keep ? k.cm_keep + (((size_t)(fs + c0) * k.P + p) * k.H + row) * k.nseg + sg : nullptr;
       for (int g0 = 0; g0 < nf; ++g0) {
         issue();
@@ -511,8 +519,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
         }
         rslot = rslot + kSlotBytes == kRingD * kSlotBytes ? 0u : rslot + kSlotBytes;
         // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
-        if ((g0 & (kGF - 1)) == 0)
-          while (done[g0] < gb - 1) {
+        if ((g0 & ((1 << gsh) - 1)) == 0)
+          while (done[g0 >> gsh] < gb - 1) {
           }
 
         if (active) {
@@ -718,11 +726,11 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
         if (keep_p) keep_p += keep_stride;
         // ---- arrive (release, no fence: the prefetch ring stays in flight) ----
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar_p + (g0 >> 2));
+        if (lane == 0) mbar_arrive_n(bar_p + (g0 >> gsh), (uint32_t)(kGF >> gsh));
       }
       // frame slots of the last, partial group that hold no frame still owe their arrivals
       if (lane == 0)
-        for (int fl = nf; fl < ((nf + kGF - 1) & ~(kGF - 1)); ++fl) mbar_arrive(&bar[(gb % 3) * (kFCH / kGF) + fl / kGF]);
+        for (int fl = nf; fl < (kSparseWarps << gsh); ++fl) mbar_arrive_n(bar_p + (fl >> gsh), (uint32_t)(kGF >> gsh));
     }
   }
 }
