@@ -95,6 +95,20 @@ def oracle_sample(cfg, raw_cpu, ped, gain, cm_mode, threads):
     return time.perf_counter() - t0, res
 
 
+def max_over_ranks(value: float, dist, device) -> float:
+    """The slowest rank's time: every multi-GPU number is the max over ranks (single rank: identity)."""
+    if dist is None:
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def first_frame_of_rank(rank: int, frames_per_rank: int) -> int:
+    """Weak scaling: rank r generates and processes frames [r*n, (r+1)*n) of the synthetic stream."""
+    return rank * frames_per_rank
+
+
 def workload_name(cfg):
     return (f"configs[{cfg.cfg_id}] {cfg.name}: {cfg.n_frames} frames of {cfg.panels}x{cfg.rows}x{cfg.cols} uint16, "
             f"S={cfg.seg_cols}, E_ph={cfg.photon_adu:g}, T_seed={cfg.seed_adu:g}, T_cm={cfg.cm_adu:g}")
@@ -168,7 +182,7 @@ def main():
     ped, gain = synth.make_maps(cfg, dev)
     n = cfg.n_frames
     raw = torch.empty((n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
-    synth.make_frames(cfg, rank * n, n, ped, gain, out=raw)
+    synth.make_frames(cfg, first_frame_of_rank(rank, n), n, ped, gain, out=raw)
     torch.cuda.synchronize()
     gen_s = time.perf_counter() - t0
 
@@ -218,10 +232,8 @@ def main():
         torch.cuda.synchronize()
     total_ms = t_begin.elapsed_time(t_end)
     kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = max_over_ranks(total_ms, dist, dev)
     if dist:
-        t = torch.tensor([total_ms], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
         dist.barrier()
     assert int(out.status.item()) == 0, "hit overflow during the bench"
     hits_per_frame = float(out.hit_count.to(torch.float64).mean().item())
@@ -253,10 +265,7 @@ def main():
             e2e_step()
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
-        if dist:
-            t = torch.tensor([e2e_s], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = max_over_ranks(e2e_s, dist, dev)
         d2h = 8 * n + 4 * cfg.npix + 20 * n * cap
         e2e = {"value": world * n * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * cfg.npix * 2,
                "d2h_bytes_per_step": d2h, "h2d_gbs": n * cfg.npix * 2 * args.e2e_steps / e2e_s / 1e9,
