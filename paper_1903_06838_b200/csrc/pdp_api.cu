@@ -196,11 +196,11 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
   int R = std::min(pdp::kDenseWarpsMax / nseg, (int)g.rows);
   if (R < 1 || (R < 2 && g.rows > 1)) return false;
   auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
-  const uint32_t ring = 3u * (uint32_t)R;
+  const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
   uint32_t off = 0;
   pl.off_cm = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
   pl.off_bits = off;  off = al(off + pdp::kFCH * ring * (uint32_t)WPR * 4u);
-  pl.off_cnt = off;   off = al(off + 3u * pdp::kFCH * 4u);
+  pl.off_cnt = off;   off = al(off + (uint32_t)pdp::kNB * pdp::kSparseWarps * 8u);
   pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
   pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
   pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
@@ -563,6 +563,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       s.k.n_bands = spl.n_bands;
       s.rg64 = c->d_rg64;
       s.big = (float)big;
+      s.magic = 0x4B000000u;
       const double ulp_big = big / 8388608.0;
       s.cand_thr = (float)((double)c->prm.seed_adu - (std::max(1e-3, 4e-6 * std::fabs((double)c->prm.seed_adu)) + 2.0 * ulp_big));
       s.R = spl.R;

@@ -28,11 +28,12 @@
 
 namespace pdp {
 
-constexpr int kStreamMaxWarps = 20;      // dense + sparse warps of a CTA
+constexpr int kStreamMaxWarps = 16;      // dense + sparse warps of a CTA
 constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
 constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
 constexpr int kStreamThreads = kStreamMaxWarps * 32;
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
+constexpr int kNB = 5;     // band slots of the shared-memory rings: a dense warp may run kNB-1 bands ahead of the sparse stage
 constexpr int kRingD = 6;  // frame groups in flight per warp (cp.async ring)
 constexpr int kMaxIt = 9;   // counting passes before the generic bisection takes over
 
@@ -41,8 +42,9 @@ struct SParams {
   const double *rg64;   // 1/gain in double (sparse stage)
   float big;            // BIG: power of two > 2 * (max |v1| + T_cm); pixels outside the mask get +BIG
   float cand_thr;       // T_seed - margin (margin covers the rounding of a + BIG)
+  uint32_t magic;       // 0x4B000000 (2^23 as float bits), passed as data so that PRMT keeps its selector immediate
   int R, NW;            // rows per band, DENSE warps per CTA (= R * nseg)
-  uint32_t off_rowmask;  // [kFCH][3R] which words of a bitmap row are non-zero (WPR <= 32)
+  uint32_t off_rowmask;  // [kFCH][kNB*R] which words of a bitmap row are non-zero (WPR <= 32)
   uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list, off_ring;
 };
 
@@ -83,11 +85,12 @@ __device__ __forceinline__ void mbar_arrive_n(uint64_t *bar, uint32_t n) {   // 
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(n) : "memory");
 }
 __device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // acquire when it succeeds
+  // try_wait suspends the warp in hardware until the phase completes or the hint (ns) expires
   uint32_t ok;
   asm volatile(
-      "{\n.reg .pred p;\nmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
       : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
+      : "r"(smem_u32(bar)), "r"(parity), "r"(20000u)
       : "memory");
   return ok != 0;
 }
@@ -117,6 +120,11 @@ struct VecLoadS<8> {
   }
 };
 
+__device__ __forceinline__ float rcp_approx(float x) {   // one MUFU.RCP
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 __device__ __forceinline__ float set_ge_abs(float a, float t) {  // 1.0f if |a| >= t else 0.0f
   float d;
   asm("set.ge.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(fabsf(a)), "f"(t));
@@ -258,7 +266,7 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
                                               const BandDesc &bd, int f0, uint32_t *list, int done_idx) {
   const KParams &k = sp.k;
   const int lane = threadIdx.x & 31;
-  const int R = sp.R, ring_rows = 3 * R;
+  const int R = sp.R, ring_rows = kNB * R;
   float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);
   uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);
   uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);
@@ -271,7 +279,7 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
   const int rb = bd.bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
   const int nrows = rb - ra + 1;
   // ring slot of row r in [r0-2, r0+R]: bands gb-1, gb, gb+1 occupy slots (gb-1)%3, gb%3, (gb+1)%3
-  const int s_prev = ((bd.gb + 2) % 3) * R, s_cur = (bd.gb % 3) * R, s_next = ((bd.gb + 1) % 3) * R;
+  const int s_prev = ((bd.gb + kNB - 1) % kNB) * R, s_cur = (bd.gb % kNB) * R, s_next = ((bd.gb + 1) % kNB) * R;
   auto slot_of = [&](int r) { return r < r0 ? s_prev + (r - r0 + R) : (r < r0 + R ? s_cur + (r - r0) : s_next + (r - r0 - R)); };
   const size_t npix = (size_t)k.P * k.H * k.W;
   uint32_t base = lane < nfr ? pref[g0 + lane] : 0u;   // lane q holds the running totals of frame q
@@ -395,10 +403,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nthreads = blockDim.x, NW = sp.NW;   // NW dense warps, then kSparseWarps sparse warps
-  const int R = sp.R, ring_rows = 3 * R;
-  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);          // [kFCH][3R][nseg]
-  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);    // [kFCH][3R][WPR]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + sp.off_cnt);      // [3][kFCH/kGF] mbarriers: NW*kGF arrivals
+  const int R = sp.R, ring_rows = kNB * R;
+  float *cmring = reinterpret_cast<float *>(smem + sp.off_cm);          // [kFCH][kNB*R][nseg]
+  uint32_t *bits = reinterpret_cast<uint32_t *>(smem + sp.off_bits);    // [kFCH][kNB*R][WPR]
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + sp.off_cnt);      // [kNB][kSparseWarps] mbarriers: NW*kGF arrivals
   volatile int *done = reinterpret_cast<volatile int *>(smem + sp.off_done);  // [kFCH]
   uint32_t *pref = reinterpret_cast<uint32_t *>(smem + sp.off_pref);    // [kFCH]
   uint32_t *phot = reinterpret_cast<uint32_t *>(smem + sp.off_phot);    // [kFCH]
@@ -408,11 +416,11 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const int FCn = fe - fs;
   if (FCn <= 0) return;
 
-  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);  // [kFCH][3R]
+  uint32_t *rowmask = reinterpret_cast<uint32_t *>(smem + sp.off_rowmask);  // [kFCH][kNB*R]
   for (int i = tid; i < kFCH * ring_rows * k.WPR; i += nthreads) bits[i] = 0u;
   for (int i = tid; i < kFCH * ring_rows; i += nthreads) rowmask[i] = 0u;
   if (tid == 0) {
-    for (int i = 0; i < 3 * kSparseWarps; ++i) mbar_init(&bar[i], (uint32_t)(NW * kGF));
+    for (int i = 0; i < kNB * kSparseWarps; ++i) mbar_init(&bar[i], (uint32_t)(NW * kGF));
     fence_mbar_init();
   }
   for (int i = tid; i < kFCH; i += nthreads) done[i] = 0, pref[i] = 0u, phot[i] = 0u;
@@ -431,8 +439,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
         const int g0 = sw << gsh;   // group sw = frame slots [sw*gf, sw*gf + gf)
         if (g0 < nf) {
           // every dense warp has published (frame group, band): acquire on the group's mbarrier
-          while (!mbar_test(&bar[(bd.gb % 3) * kSparseWarps + sw], (uint32_t)(bd.gb / 3) & 1u))
-            __nanosleep(256);   // a sleeping warp costs no issue slots; a sparse task lasts microseconds
+          while (!mbar_test(&bar[(bd.gb % kNB) * kSparseWarps + sw], (uint32_t)(bd.gb / kNB) & 1u))
+            __nanosleep(2000);  // a sleeping warp costs no issue slots; a band of dense work lasts tens of microseconds
           stream_sparse(sp, smem, g0, min(1 << gsh, nf - g0), bd, fs + c0 + g0, list, sw);
         } else if (lane == 0) {
           done[sw] = bd.gb + 1;
@@ -445,6 +453,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const int tr = warp / k.nseg, sg = warp - tr * k.nseg;  // this warp's row of the band and segment
   const size_t npix = (size_t)k.P * k.H * k.W;
   const float BIG = sp.big, BIG2 = 4.f * sp.big;
+  const uint32_t magic = sp.magic;
   const int ms = lane / GL;  // the search this lane steers
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
   float mK[N], mRg[N], mNpf[N];
@@ -460,11 +469,38 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   for (int c0 = 0; c0 < FCn; c0 += kFCH) {
     const int nf = min(kFCH, FCn - c0);
     const int gsh = nf <= kSparseWarps ? 0 : (nf <= 2 * kSparseWarps ? 1 : 2);   // log2(frames per sparse task)
+    // Raw-pixel prefetch cursor: runs kRingD-1 frames ahead of the frame being processed and crosses
+    // band boundaries inside the chunk, so the DRAM latency is paid once per chunk, not once per band.
+    int i_frame = 0, i_band = 0, i_bi = 0, i_p = 0;
+    bool i_active = tr < k.H;
+    const uint16_t *chunk_raw = k.raw + (size_t)(fs + c0) * npix + (size_t)sg * k.S + lane * V;
+    const uint16_t *src = chunk_raw + (size_t)tr * k.W;
+    uint32_t islot = 0, rslot = 0;
+    auto issue = [&]() {
+      if (i_active && i_frame < nf) {
+#pragma unroll
+        for (int g = 0; g < G; ++g)
+          if ((vmask >> g) & 1u) cp_async_s<V * 2>(ring_lane + islot + g * (64 * V), src + g * (32 * V));
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      src += npix;
+      islot = islot + kSlotBytes == kRingD * kSlotBytes ? 0u : islot + kSlotBytes;
+      if (++i_frame == nf && i_band + 1 < k.n_bands) {   // on to the first frame of the next band
+        ++i_band;
+        if (++i_bi == k.bands_per_panel) i_bi = 0, ++i_p;
+        const int row_n = i_bi * R + tr;
+        i_active = row_n < k.H;
+        src = chunk_raw + ((size_t)i_p * k.H + row_n) * k.W;
+        i_frame = 0;
+      }
+    };
+#pragma unroll 1
+    for (int d = 0; d < kRingD - 1; ++d) issue();
     for (int band = 0; band < k.n_bands; ++band, ++gb) {
       const int p = band / k.bands_per_panel, r0 = (band - p * k.bands_per_panel) * R;
       const int row = r0 + tr;
       const bool active = row < k.H;
-      const int slot = (gb % 3) * R + tr;
+      const int slot = (gb % kNB) * R + tr;
       const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
       if (active) {
 #pragma unroll
@@ -482,30 +518,12 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
       }
       // raw pixels: per-warp ring of kRingD frames filled by cp.async (LDGSTS); every lane copies and
       // later reads only its own vectors, so cp.async.wait_group is all the synchronisation needed
-      const uint16_t *src = k.raw + (size_t)(fs + c0) * npix + rowoff + lane * V;
-      int issued = 0;
-      uint32_t islot = 0, rslot = 0;
-      auto issue = [&]() {
-        if (active && issued < nf) {
-#pragma unroll
-          for (int g = 0; g < G; ++g)
-            if ((vmask >> g) & 1u) cp_async_s<V * 2>(ring_lane + islot + g * (64 * V), src + g * (32 * V));
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-        src += npix;
-        ++issued;
-        islot = islot + kSlotBytes == kRingD * kSlotBytes ? 0u : islot + kSlotBytes;
-      };
-#pragma unroll 1
-      for (int d = 0; d < kRingD - 1; ++d) issue();
       // running pointers of what this warp publishes per frame
       const int cm_stride = ring_rows * k.nseg, bits_stride = ring_rows * k.WPR;
-      const size_t keep_stride = (size_t)k.P * k.H * k.nseg;
       float *cm_p = cmring + (size_t)slot * k.nseg + sg;
       uint32_t *bits_p = bits + (size_t)slot * k.WPR;
       uint32_t *rowmask_p = rowmask + slot;
-      uint64_t *bar_p = bar + (gb % 3) * kSparseWarps;
-      float *keep_p = k.cm_keep ? k.cm_keep + (((size_t)(fs + c0) * k.P + p) * k.H + row) * k.nseg + sg : nullptr;
+      uint64_t *bar_p = bar + (gb % kNB) * kSparseWarps;
       for (int g0 = 0; g0 < nf; ++g0) {
         issue();
         asm volatile("cp.async.wait_group %0;" ::"n"(kRingD - 1) : "memory");
@@ -518,9 +536,9 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           for (int e = 0; e < V / 2; ++e) w[0][g * (V / 2) + e] = t[e];
         }
         rslot = rslot + kSlotBytes == kRingD * kSlotBytes ? 0u : rslot + kSlotBytes;
-        // the ring slot about to be written held band gb-3, last read by the sparse stage of band gb-2
+        // the ring slot about to be written held band gb-kNB, last read by the sparse stage of band gb-kNB+1
         if ((g0 & ((1 << gsh) - 1)) == 0)
-          while (done[g0 >> gsh] < gb - 1) {
+          while (done[g0 >> gsh] < gb - (kNB - 2)) {
           }
 
         if (active) {
@@ -539,7 +557,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                   const int j = 2 * e + h;
-                  const float x = __uint_as_float(__byte_perm(w[q][e], 0x4B000000u, h ? 0x7632 : 0x7610));
+                  const float x = __uint_as_float(__byte_perm(w[q][e], magic, h ? 0x7632 : 0x7610));
                   const float a = fmaf(x - mK[j], mRg[j], mNpf[j]);
                   const float notm = set_ge_abs(a, k.T_cm);   // pixels WITH signal
                   bq[q][j] = fmaf(notm, BIG, a);
@@ -575,9 +593,10 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
             int state = (n_my < k.cm_min_count || n_my <= 0) ? 1 : 0;   // c = 0: nothing to search
 #pragma unroll 1
             for (int it = 0; it < kMaxIt && state == 0; ++it) {
-              float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+              float a0 = set_lt(bq[0][0], p_my), a1 = N > 1 ? set_lt(bq[0][N > 1 ? 1 : 0], p_my) : 0.f,
+                    a2 = N > 2 ? set_lt(bq[0][N > 2 ? 2 : 0], p_my) : 0.f;
 #pragma unroll
-              for (int j = 0; j < N; ++j) {
+              for (int j = 3; j < N; ++j) {
                 const float d = set_lt(bq[0][j], p_my);
                 if (j % 3 == 0) a0 += d;
                 else if (j % 3 == 1) a1 += d;
@@ -593,8 +612,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
               // is refreshed only from the first, wide pair), kept inside the bracket (lo, hi)
               float slope = apr;
               if (it > 0 && c != c_prev) {
-                slope = __fdividef(p_my - p_prev, (float)(c - c_prev));
-                if (it == 1 && abs(c - c_prev) >= 8) apr = 0.75f * apr + 0.25f * slope;
+                slope = (p_my - p_prev) * rcp_approx((float)(c - c_prev));   // |c - c_prev| >= 1: no denormals
+                if (it == 1 && abs(c - c_prev) >= 8) apr = fmaf(0.25f, slope - apr, apr);
               }
               if (c < kl) lo = p_my; else hi = p_my;
               p_prev = p_my;
@@ -672,7 +691,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
                   const int j = 2 * e + h;
-                  const float x = __uint_as_float(__byte_perm(w[q][e], 0x4B000000u, h ? 0x7632 : 0x7610));
+                  const float x = __uint_as_float(__byte_perm(w[q][e], magic, h ? 0x7632 : 0x7610));
                   a[j] = fmaf(x - mK[j], mRg[j], mNpf[j]);
                   if (k.cm_mode == 1) {
                     const float m = set_lt_abs(a[j], k.T_cm);
@@ -707,7 +726,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           // ---- publish: common-mode estimate and candidate bits of (frame slot, row, segment) ----
           if (lane == 0) {
             *cm_p = cq[0];
-            if (keep_p) *keep_p = cq[0];
+            if (k.cm_keep)   // debug only: address computed here, nothing carried through the loop
+              k.cm_keep[(((size_t)(fs + c0 + g0) * k.P + p) * k.H + row) * k.nseg + sg] = cq[0];
           }
           if (anyc[0]) {
 #pragma unroll
@@ -723,7 +743,6 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
         cm_p += cm_stride;
         bits_p += bits_stride;
         rowmask_p += ring_rows;
-        if (keep_p) keep_p += keep_stride;
         // ---- arrive (release, no fence: the prefetch ring stays in flight) ----
         __syncwarp();
         if (lane == 0) mbar_arrive_n(bar_p + (g0 >> gsh), (uint32_t)(kGF >> gsh));
