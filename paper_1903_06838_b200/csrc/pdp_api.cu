@@ -39,7 +39,7 @@ constexpr int kFramesPerCtaMax = 1024;
 struct StreamPlan {
   bool ok = false;
   int R = 0, NW = 0, FL = 1, bands_per_panel = 0, n_bands = 0;
-  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, off_ring = 0, smem = 0;
+  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, off_ring = 0, off_maps = 0, smem = 0;
 };
 
 }  // namespace
@@ -193,29 +193,34 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
 // The streaming kernel: one warp per (band row, segment), R = warps / segments rows per band.
 bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, StreamPlan &pl) {
   const int nseg = g.cols / g.seg_cols;
-  int R = std::min(pdp::kDenseWarpsMax / nseg, (int)g.rows);
-  if (R < 1 || (R < 2 && g.rows > 1)) return false;
+  if (WPR > 32) return false;
   auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
-  const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
-  uint32_t off = 0;
-  pl.off_cm = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
-  pl.off_bits = off;  off = al(off + pdp::kFCH * ring * (uint32_t)WPR * 4u);
-  pl.off_cnt = off;   off = al(off + (uint32_t)pdp::kNB * pdp::kSparseWarps * 8u);
-  pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
-  pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
-  pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
-  pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
-  pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
-  pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
-  if (off > smem_limit || WPR > 32 || R > 254) return false;
-  pl.R = R;
-  pl.NW = R * nseg;
-  pl.FL = 1;
-  pl.bands_per_panel = (g.rows + R - 1) / R;
-  pl.n_bands = pl.bands_per_panel * g.panels;
-  pl.smem = off;
-  pl.ok = true;
-  return true;
+  // the tallest band (most dense warps) whose rings, raw prefetch ring and map tiles fit in shared memory
+  for (int R = std::min(std::min(pdp::kDenseWarpsMax / nseg, (int)g.rows), 254); R >= 1; --R) {
+    if (R < 2 && g.rows > 1) return false;
+    const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
+    uint32_t off = 0;
+    pl.off_cm = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
+    pl.off_bits = off;  off = al(off + pdp::kFCH * ring * (uint32_t)WPR * 4u);
+    pl.off_cnt = off;   off = al(off + (uint32_t)pdp::kNB * pdp::kSparseWarps * 8u);
+    pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
+    pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
+    pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
+    pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
+    pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
+    pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
+    pl.off_maps = off;  off = al(off + (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u);
+    if (off > smem_limit) continue;
+    pl.R = R;
+    pl.NW = R * nseg;
+    pl.FL = 1;
+    pl.bands_per_panel = (g.rows + R - 1) / R;
+    pl.n_bands = pl.bands_per_panel * g.panels;
+    pl.smem = off;
+    pl.ok = true;
+    return true;
+  }
+  return false;
 }
 
 using KernelFn = void (*)(const KParams);
@@ -577,6 +582,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       s.off_list = spl.off_list;
       s.off_rowmask = spl.off_rowmask;
       s.off_ring = spl.off_ring;
+      s.off_maps = spl.off_maps;
       const int grid_s = std::min(c->num_sms, n);
       StreamFn sf = stream_kernel(pl.V, pl.G, spl.FL);
       sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);

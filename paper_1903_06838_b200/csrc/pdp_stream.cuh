@@ -28,7 +28,7 @@
 
 namespace pdp {
 
-constexpr int kStreamMaxWarps = 16;      // dense + sparse warps of a CTA
+constexpr int kStreamMaxWarps = 20;      // dense + sparse warps of a CTA
 constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
 constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
 constexpr int kStreamThreads = kStreamMaxWarps * 32;
@@ -45,7 +45,7 @@ struct SParams {
   uint32_t magic;       // 0x4B000000 (2^23 as float bits), passed as data so that PRMT keeps its selector immediate
   int R, NW;            // rows per band, DENSE warps per CTA (= R * nseg)
   uint32_t off_rowmask;  // [kFCH][kNB*R] which words of a bitmap row are non-zero (WPR <= 32)
-  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list, off_ring;
+  uint32_t off_cm, off_bits, off_cnt, off_done, off_pref, off_phot, off_list, off_ring, off_maps;
 };
 
 // ---- small helpers -------------------------------------------------------------------------------
@@ -93,6 +93,20 @@ __device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // 
       : "r"(smem_u32(bar)), "r"(parity), "r"(20000u)
       : "memory");
   return ok != 0;
+}
+
+template <int V>
+__device__ __forceinline__ void load_smap(const float *src, float *dst) {   // V floats from shared memory
+  if constexpr (V == 2) {
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(dst[0]), "=f"(dst[1]) : "r"(smem_u32(src)));
+  } else {
+#pragma unroll
+    for (int e = 0; e < V; e += 4) {
+      float4 t;
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "r"(smem_u32(src + e)));
+      dst[e] = t.x, dst[e + 1] = t.y, dst[e + 2] = t.z, dst[e + 3] = t.w;
+    }
+  }
 }
 
 template <int BYTES>
@@ -456,7 +470,7 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const uint32_t magic = sp.magic;
   const int ms = lane / GL;  // the search this lane steers
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
-  float mK[N], mRg[N], mNpf[N];
+  float *smap = reinterpret_cast<float *>(smem + sp.off_maps) + (size_t)warp * (3 * N * 32) + lane * V;  // this lane's map vectors
   constexpr int NS = (N + 2) / 3;  // pixels per lane sampled for the first pivot (every third)
   static_assert(FL == 1, "the frame loop below advances one frame per iteration");
   uint32_t vmask = 0;              // which of this lane's G vectors lie inside the segment
@@ -502,19 +516,25 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
       const bool active = row < k.H;
       const int slot = (gb % kNB) * R + tr;
       const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
-      if (active) {
+      if (active) {   // maps of this warp's row segment: global (L2) -> shared memory, once per band and chunk
+        __syncwarp();
 #pragma unroll
         for (int g = 0; g < G; ++g) {
           const int vi = g * 32 + lane;
+          float tK[V], tRg[V], tNpf[V];
           if (vi * V < k.S) {
-            load_map<V>(k.mapK + rowoff + vi * V, &mK[g * V]);
-            load_map<V>(k.mapRg + rowoff + vi * V, &mRg[g * V]);
-            load_map<V>(k.mapNpf + rowoff + vi * V, &mNpf[g * V]);
+            load_map<V>(k.mapK + rowoff + vi * V, tK);
+            load_map<V>(k.mapRg + rowoff + vi * V, tRg);
+            load_map<V>(k.mapNpf + rowoff + vi * V, tNpf);
           } else {  // padding lanes: a = -BIG/2, i.e. bq = BIG/2: above every pivot, below every candidate
 #pragma unroll
-            for (int e = 0; e < V; ++e) mK[g * V + e] = 8388608.f, mRg[g * V + e] = 0.f, mNpf[g * V + e] = -0.5f * BIG;
+            for (int e = 0; e < V; ++e) tK[e] = 8388608.f, tRg[e] = 0.f, tNpf[e] = -0.5f * BIG;
           }
+          store_v1<V>(smap + g * (32 * V), tK);
+          store_v1<V>(smap + N * 32 + g * (32 * V), tRg);
+          store_v1<V>(smap + 2 * N * 32 + g * (32 * V), tNpf);
         }
+        __syncwarp();
       }
       // raw pixels: per-warp ring of kRingD frames filled by cp.async (LDGSTS); every lane copies and
       // later reads only its own vectors, so cp.async.wait_group is all the synchronisation needed
@@ -545,6 +565,13 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           float cq[FL];
           uint32_t cbits[FL][G];
           bool anyc[FL];
+          float mK[N], mRg[N], mNpf[N];
+#pragma unroll
+          for (int g = 0; g < G; ++g) {
+            load_smap<V>(smap + g * (32 * V), &mK[g * V]);
+            load_smap<V>(smap + N * 32 + g * (32 * V), &mRg[g * V]);
+            load_smap<V>(smap + 2 * N * 32 + g * (32 * V), &mNpf[g * V]);
+          }
           if (k.cm_mode == 0) {
             // ================= exact median common mode (north_star (a)) =================
             float bq[FL][N];
