@@ -160,8 +160,17 @@ __device__ __forceinline__ float set_ge(float a, float b) {
   return d;
 }
 
-__device__ __forceinline__ float warp_min_f(float v) { return key2f(warp_min_u(f2key(v))); }
-__device__ __forceinline__ float warp_max_f(float v) { return key2f(warp_max_u(f2key(v))); }
+// sm_100a has warp-wide float min/max (redux.sync.{min,max}.f32): one instruction, no key conversion
+__device__ __forceinline__ float warp_min_f(float v) {
+  float r;
+  asm volatile("redux.sync.min.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+  return r;
+}
+__device__ __forceinline__ float warp_max_f(float v) {
+  float r;
+  asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+  return r;
+}
 
 // Order statistics read off with one pass: values on the wrong side of the pivot are pushed out of
 // range by +-big2 (exactly representable move; values on the right side are untouched: r = 0).
@@ -636,17 +645,20 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
                 break;
               }
               // secant through the last two points (first step: the running density estimate, which
-              // is refreshed only from the first, wide pair), kept inside the bracket (lo, hi)
-              float slope = apr;
-              if (it > 0 && c != c_prev) {
-                slope = (p_my - p_prev) * rcp_approx((float)(c - c_prev));   // |c - c_prev| >= 1: no denormals
-                if (it == 1 && abs(c - c_prev) >= 8) apr = fmaf(0.25f, slope - apr, apr);
-              }
-              if (c < kl) lo = p_my; else hi = p_my;
+              // is refreshed only from the first, wide pair), kept inside the bracket (lo, hi);
+              // written with selects: everything here is warp-uniform and short
+              const float dc = (float)(c - c_prev);
+              const float sec = (p_my - p_prev) * rcp_approx(dc);          // |dc| >= 1 when it is used
+              const bool use_sec = it > 0 && c != c_prev;
+              const float slope = use_sec ? sec : apr;
+              apr = (it == 1 && fabsf(dc) >= 8.f) ? fmaf(0.25f, sec - apr, apr) : apr;
+              const bool below = c < kl;
+              lo = below ? p_my : lo;
+              hi = below ? hi : p_my;
               p_prev = p_my;
               c_prev = c;
               float pn = fmaf(tgt - (float)c, slope, p_my);
-              if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
+              pn = (pn > lo && pn < hi) ? pn : 0.5f * (lo + hi);
               if (!(pn > lo && pn < hi)) state = 2;   // no float strictly inside: ties
               p_my = pn;
             }
