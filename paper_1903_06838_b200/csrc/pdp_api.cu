@@ -58,7 +58,7 @@ struct pdp_ctx {
   int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
   FramesPlan fplan[2];      // [0] without, [1] with the fp16 pre-filter tile
-  StreamPlan splan;         // the streaming kernel (pdp_stream.cuh)
+  StreamPlan splan[2];      // the streaming kernel (pdp_stream.cuh): [0] maps in registers, [1] maps in shared memory
   double amax = 0.0;        // max over pixels of |v1| any uint16 raw value can produce
   int prefilter = 0;        // PDP_PREFILTER=1 selects fplan[1]
   int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel, 3 streaming kernel (PDP_KERNEL)
@@ -191,12 +191,12 @@ bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesP
 }
 
 // The streaming kernel: one warp per (band row, segment), R = warps / segments rows per band.
-bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, StreamPlan &pl) {
+bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, int ms, StreamPlan &pl) {
   const int nseg = g.cols / g.seg_cols;
   if (WPR > 32) return false;
   auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
   // the tallest band (most dense warps) whose rings, raw prefetch ring and map tiles fit in shared memory
-  for (int R = std::min(std::min(pdp::kDenseWarpsMax / nseg, (int)g.rows), 254); R >= 1; --R) {
+  for (int R = std::min(std::min(pdp::kDenseWarpsMaxOf(ms) / nseg, (int)g.rows), 254); R >= 1; --R) {
     if (R < 2 && g.rows > 1) return false;
     const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
     uint32_t off = 0;
@@ -209,11 +209,11 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
     pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
     pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
     pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
-    pl.off_maps = off;  off = al(off + (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u);
+    pl.off_maps = off;  off = al(off + (ms ? (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u : 0u));
     if (off > smem_limit) continue;
     pl.R = R;
     pl.NW = R * nseg;
-    pl.FL = 1;
+    pl.FL = ms;   // the kernel's third template parameter
     pl.bands_per_panel = (g.rows + R - 1) / R;
     pl.n_bands = pl.bands_per_panel * g.panels;
     pl.smem = off;
@@ -242,10 +242,12 @@ StreamFn stream_kernel_for(int V, int G) {
   }
   return nullptr;
 }
-StreamFn stream_kernel(int V, int G, int FL) {
-  if (FL != 1) return nullptr;
-  if (V == 8 && G > 2) return G == 3 ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 4, 1>;
-  return stream_kernel_for<1>(V, G);
+StreamFn stream_kernel(int V, int G, int ms) {
+  if (V == 8 && G > 2) {
+    if (G == 3) return ms ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 3, 0>;
+    return ms ? pdp::pdp_stream_kernel<8, 4, 1> : pdp::pdp_stream_kernel<8, 4, 0>;
+  }
+  return ms ? stream_kernel_for<1>(V, G) : stream_kernel_for<0>(V, G);
 }
 using FramesFn = void (*)(const FParams);
 
@@ -403,16 +405,13 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     }
   }
   c->amax = amax;
-  if (make_plan_stream(*geo, c->plan.V, c->plan.G, c->plan.WPR, prop.sharedMemPerBlockOptin, c->splan)) {
-    StreamFn sf = stream_kernel(c->plan.V, c->plan.G, c->splan.FL);
-    if (!sf) {
-      c->splan.ok = false;
-    } else {
-      e = cudaFuncSetAttribute(sf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->splan.smem);
-      if (e != cudaSuccess) {
-        free_ctx(c);
-        return cuda_fail(nullptr, e, "cudaFuncSetAttribute(stream)");
-      }
+  for (int ms = 0; ms < 2; ++ms) {
+    if (!make_plan_stream(*geo, c->plan.V, c->plan.G, c->plan.WPR, prop.sharedMemPerBlockOptin, ms, c->splan[ms])) continue;
+    StreamFn sf = stream_kernel(c->plan.V, c->plan.G, ms);
+    e = cudaFuncSetAttribute(sf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->splan[ms].smem);
+    if (e != cudaSuccess) {
+      free_ctx(c);
+      return cuda_fail(nullptr, e, "cudaFuncSetAttribute(stream)");
     }
   }
   if (const char *s = std::getenv("PDP_PREFILTER")) c->prefilter = std::atoi(s) != 0;
@@ -554,12 +553,14 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
     double big = 1024.0;
     while (big < need) big *= 2.0;
     const bool big_ok = big <= 4194304.0 && (double)c->prm.cm_adu < 0.25 * big;
-    const bool use_stream = c->splan.ok && big_ok &&
+    // median: maps in shared memory and 16 dense warps; mean / none: maps in registers, 12 dense warps
+    const int ms = (c->prm.cm_mode == PDP_CM_MEDIAN && c->splan[1].ok) ? 1 : (c->splan[0].ok ? 0 : 1);
+    const bool use_stream = c->splan[ms].ok && big_ok &&
                             (c->kernel_override == 3 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
     if (c->kernel_override == 3 && !use_stream)
       return fail(c, PDP_E_GEOMETRY, "PDP_KERNEL=stream: the streaming kernel does not support this geometry/maps");
     if (use_stream) {
-      const StreamPlan &spl = c->splan;
+      const StreamPlan &spl = c->splan[ms];
       SParams s{};
       s.k = k;
       s.k.R = spl.R;
@@ -584,7 +585,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       s.off_ring = spl.off_ring;
       s.off_maps = spl.off_maps;
       const int grid_s = std::min(c->num_sms, n);
-      StreamFn sf = stream_kernel(pl.V, pl.G, spl.FL);
+      StreamFn sf = stream_kernel(pl.V, pl.G, ms);
       sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);
       PDP_CUDA(c, cudaGetLastError());
       c->launches += 1;

@@ -28,10 +28,12 @@
 
 namespace pdp {
 
-constexpr int kStreamMaxWarps = 20;      // dense + sparse warps of a CTA
 constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
-constexpr int kDenseWarpsMax = kStreamMaxWarps - kSparseWarps;
-constexpr int kStreamThreads = kStreamMaxWarps * 32;
+// Two register/occupancy trade-offs, chosen per common-mode estimator (template parameter MS):
+//   MS = 1 (median): calibration maps in shared memory, 102 registers, 16 dense + 4 sparse warps;
+//   MS = 0 (mean / none): maps in registers, 128 registers, 12 dense + 4 sparse warps.
+constexpr int kDenseWarpsMaxOf(int ms) { return ms ? 16 : 12; }
+constexpr int kStreamThreadsOf(int ms) { return (kDenseWarpsMaxOf(ms) + kSparseWarps) * 32; }
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
 constexpr int kNB = 5;     // band slots of the shared-memory rings: a dense warp may run kNB-1 bands ahead of the sparse stage
 constexpr int kRingD = 6;  // frame groups in flight per warp (cp.async ring)
@@ -418,8 +420,9 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
 // ---- the kernel ----------------------------------------------------------------------------------
 // V = pixels per vector load (2/4/8), G = vectors per lane (one warp covers S <= 32*V*G pixels),
 // FL = frames processed in lock-step by a warp (1 or 2).
-template <int V, int G, int FL>
-__global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SParams sp) {
+template <int V, int G, int MS>
+__global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(const SParams sp) {
+  constexpr int FL = 1;   // frames per iteration
   constexpr int N = V * G;
   constexpr int GL = 32 / FL;  // lanes steering one search
   const KParams &k = sp.k;
@@ -479,7 +482,8 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
   const uint32_t magic = sp.magic;
   const int ms = lane / GL;  // the search this lane steers
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
-  float *smap = reinterpret_cast<float *>(smem + sp.off_maps) + (size_t)warp * (3 * N * 32) + lane * V;  // this lane's map vectors
+  float *smap = reinterpret_cast<float *>(smem + sp.off_maps) + (size_t)warp * (3 * N * 32) + lane * V;  // this lane's map vectors (MS)
+  float rK[MS ? 1 : N], rRg[MS ? 1 : N], rNpf[MS ? 1 : N];   // the maps in registers (!MS)
   constexpr int NS = (N + 2) / 3;  // pixels per lane sampled for the first pivot (every third)
   static_assert(FL == 1, "the frame loop below advances one frame per iteration");
   uint32_t vmask = 0;              // which of this lane's G vectors lie inside the segment
@@ -539,9 +543,14 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
 #pragma unroll
             for (int e = 0; e < V; ++e) tK[e] = 8388608.f, tRg[e] = 0.f, tNpf[e] = -0.5f * BIG;
           }
-          store_v1<V>(smap + g * (32 * V), tK);
-          store_v1<V>(smap + N * 32 + g * (32 * V), tRg);
-          store_v1<V>(smap + 2 * N * 32 + g * (32 * V), tNpf);
+          if constexpr (MS) {
+            store_v1<V>(smap + g * (32 * V), tK);
+            store_v1<V>(smap + N * 32 + g * (32 * V), tRg);
+            store_v1<V>(smap + 2 * N * 32 + g * (32 * V), tNpf);
+          } else {
+#pragma unroll
+            for (int e = 0; e < V; ++e) rK[g * V + e] = tK[e], rRg[g * V + e] = tRg[e], rNpf[g * V + e] = tNpf[e];
+          }
         }
         __syncwarp();
       }
@@ -577,9 +586,14 @@ __global__ void __launch_bounds__(kStreamThreads, 1) pdp_stream_kernel(const SPa
           float mK[N], mRg[N], mNpf[N];
 #pragma unroll
           for (int g = 0; g < G; ++g) {
-            load_smap<V>(smap + g * (32 * V), &mK[g * V]);
-            load_smap<V>(smap + N * 32 + g * (32 * V), &mRg[g * V]);
-            load_smap<V>(smap + 2 * N * 32 + g * (32 * V), &mNpf[g * V]);
+            if constexpr (MS) {
+              load_smap<V>(smap + g * (32 * V), &mK[g * V]);
+              load_smap<V>(smap + N * 32 + g * (32 * V), &mRg[g * V]);
+              load_smap<V>(smap + 2 * N * 32 + g * (32 * V), &mNpf[g * V]);
+            } else {
+#pragma unroll
+              for (int e = 0; e < V; ++e) mK[g * V + e] = rK[g * V + e], mRg[g * V + e] = rRg[g * V + e], mNpf[g * V + e] = rNpf[g * V + e];
+            }
           }
           if (k.cm_mode == 0) {
             // ================= exact median common mode (north_star (a)) =================
