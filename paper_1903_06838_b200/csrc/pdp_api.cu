@@ -58,7 +58,7 @@ struct pdp_ctx {
   int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
   FramesPlan fplan[2];      // [0] without, [1] with the fp16 pre-filter tile
-  StreamPlan splan[2];      // the streaming kernel (pdp_stream.cuh): [0] maps in registers, [1] maps in shared memory
+  StreamPlan splan[3];      // the streaming kernel (pdp_stream.cuh): [0] maps in registers, [1] maps in shared memory
   double amax = 0.0;        // max over pixels of |v1| any uint16 raw value can produce
   int prefilter = 0;        // PDP_PREFILTER=1 selects fplan[1]
   int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel, 3 streaming kernel (PDP_KERNEL)
@@ -209,7 +209,7 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
     pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
     pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
     pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
-    pl.off_maps = off;  off = al(off + (ms ? (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u : 0u));
+    pl.off_maps = off;  off = al(off + (ms == 1 ? (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u : 0u));
     if (off > smem_limit) continue;
     pl.R = R;
     pl.NW = R * nseg;
@@ -244,10 +244,10 @@ StreamFn stream_kernel_for(int V, int G) {
 }
 StreamFn stream_kernel(int V, int G, int ms) {
   if (V == 8 && G > 2) {
-    if (G == 3) return ms ? pdp::pdp_stream_kernel<8, 3, 1> : pdp::pdp_stream_kernel<8, 3, 0>;
-    return ms ? pdp::pdp_stream_kernel<8, 4, 1> : pdp::pdp_stream_kernel<8, 4, 0>;
+    if (G == 3) return ms == 1 ? pdp::pdp_stream_kernel<8, 3, 1> : (ms ? pdp::pdp_stream_kernel<8, 3, 2> : pdp::pdp_stream_kernel<8, 3, 0>);
+    return ms == 1 ? pdp::pdp_stream_kernel<8, 4, 1> : (ms ? pdp::pdp_stream_kernel<8, 4, 2> : pdp::pdp_stream_kernel<8, 4, 0>);
   }
-  return ms ? stream_kernel_for<1>(V, G) : stream_kernel_for<0>(V, G);
+  return ms == 1 ? stream_kernel_for<1>(V, G) : (ms ? stream_kernel_for<2>(V, G) : stream_kernel_for<0>(V, G));
 }
 using FramesFn = void (*)(const FParams);
 
@@ -405,7 +405,7 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     }
   }
   c->amax = amax;
-  for (int ms = 0; ms < 2; ++ms) {
+  for (int ms = 0; ms < 3; ++ms) {
     if (!make_plan_stream(*geo, c->plan.V, c->plan.G, c->plan.WPR, prop.sharedMemPerBlockOptin, ms, c->splan[ms])) continue;
     StreamFn sf = stream_kernel(c->plan.V, c->plan.G, ms);
     e = cudaFuncSetAttribute(sf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->splan[ms].smem);
@@ -554,7 +554,8 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
     while (big < need) big *= 2.0;
     const bool big_ok = big <= 4194304.0 && (double)c->prm.cm_adu < 0.25 * big;
     // median: maps in shared memory and 16 dense warps; mean / none: maps in registers, 12 dense warps
-    const int ms = (c->prm.cm_mode == PDP_CM_MEDIAN && c->splan[1].ok) ? 1 : (c->splan[0].ok ? 0 : 1);
+    // variant: 0 mean/none; 1 median, maps in shared memory; 2 median, maps in registers (map tiles do not fit)
+    const int ms = c->prm.cm_mode != PDP_CM_MEDIAN ? 0 : ((c->splan[1].ok && c->splan[1].R >= c->splan[2].R) ? 1 : 2);
     const bool use_stream = c->splan[ms].ok && big_ok &&
                             (c->kernel_override == 3 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
     if (c->kernel_override == 3 && !use_stream)

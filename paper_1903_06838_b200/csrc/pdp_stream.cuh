@@ -31,8 +31,10 @@ namespace pdp {
 constexpr int kSparseWarps = 4;          // warps that only run the sparse stage
 // Two register/occupancy trade-offs, chosen per common-mode estimator (template parameter MS):
 //   MS = 1 (median): calibration maps in shared memory, 102 registers, 16 dense + 4 sparse warps;
-//   MS = 0 (mean / none): maps in registers, 128 registers, 12 dense + 4 sparse warps.
-constexpr int kDenseWarpsMaxOf(int ms) { return ms ? 16 : 12; }
+//   MS = 0 (mean / none) and MS = 2 (median when the map tiles do not fit in shared memory): maps in
+//   registers, 128 registers, 12 dense + 4 sparse warps.
+// Each variant contains only its own estimator's loop body (smaller hot loop in the instruction cache).
+constexpr int kDenseWarpsMaxOf(int ms) { return ms == 1 ? 16 : 12; }
 constexpr int kStreamThreadsOf(int ms) { return (kDenseWarpsMaxOf(ms) + kSparseWarps) * 32; }
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
 constexpr int kNB = 5;     // band slots of the shared-memory rings: a dense warp may run kNB-1 bands ahead of the sparse stage
@@ -417,6 +419,21 @@ __device__ __forceinline__ void stream_sparse(const SParams &sp, unsigned char *
   __syncwarp();
 }
 
+// The generic bracketed bisection (pdp_device.cuh) out of line: it runs only when the fast search does
+// not converge (exact ties), and keeping its ~300 instructions out of the loop body keeps the hot loop small.
+template <int N>
+struct BqPack {
+  float v[N];
+  __device__ __forceinline__ BqPack(const float (&b)[N]) {
+#pragma unroll
+    for (int j = 0; j < N; ++j) v[j] = b[j];
+  }
+};
+template <int N>
+__device__ __noinline__ float median_fallback(BqPack<N> b, int n, float mean, float lim, float apr) {
+  return warp_median<N>(b.v, n, mean, lim, apr);
+}
+
 // ---- the kernel ----------------------------------------------------------------------------------
 // V = pixels per vector load (2/4/8), G = vectors per lane (one warp covers S <= 32*V*G pixels),
 // FL = frames processed in lock-step by a warp (1 or 2).
@@ -483,7 +500,8 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
   const int ms = lane / GL;  // the search this lane steers
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
   float *smap = reinterpret_cast<float *>(smem + sp.off_maps) + (size_t)warp * (3 * N * 32) + lane * V;  // this lane's map vectors (MS)
-  float rK[MS ? 1 : N], rRg[MS ? 1 : N], rNpf[MS ? 1 : N];   // the maps in registers (!MS)
+  constexpr bool kMapsSmem = MS == 1, kMedian = MS != 0;
+  float rK[kMapsSmem ? 1 : N], rRg[kMapsSmem ? 1 : N], rNpf[kMapsSmem ? 1 : N];   // the maps in registers
   constexpr int NS = (N + 2) / 3;  // pixels per lane sampled for the first pivot (every third)
   static_assert(FL == 1, "the frame loop below advances one frame per iteration");
   uint32_t vmask = 0;              // which of this lane's G vectors lie inside the segment
@@ -543,7 +561,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
 #pragma unroll
             for (int e = 0; e < V; ++e) tK[e] = 8388608.f, tRg[e] = 0.f, tNpf[e] = -0.5f * BIG;
           }
-          if constexpr (MS) {
+          if constexpr (kMapsSmem) {
             store_v1<V>(smap + g * (32 * V), tK);
             store_v1<V>(smap + N * 32 + g * (32 * V), tRg);
             store_v1<V>(smap + 2 * N * 32 + g * (32 * V), tNpf);
@@ -586,7 +604,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
           float mK[N], mRg[N], mNpf[N];
 #pragma unroll
           for (int g = 0; g < G; ++g) {
-            if constexpr (MS) {
+            if constexpr (kMapsSmem) {
               load_smap<V>(smap + g * (32 * V), &mK[g * V]);
               load_smap<V>(smap + N * 32 + g * (32 * V), &mRg[g * V]);
               load_smap<V>(smap + 2 * N * 32 + g * (32 * V), &mNpf[g * V]);
@@ -595,7 +613,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
               for (int e = 0; e < V; ++e) mK[g * V + e] = rK[g * V + e], mRg[g * V + e] = rRg[g * V + e], mNpf[g * V + e] = rNpf[g * V + e];
             }
           }
-          if (k.cm_mode == 0) {
+          if constexpr (kMedian) {
             // ================= exact median common mode (north_star (a)) =================
             float bq[FL][N];
             float nout[FL], ssum[FL];
@@ -690,7 +708,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
               if (n_q >= k.cm_min_count && n_q > 0) {
                 if (f_q) {
                   float apr2 = apr;
-                  c = warp_median<N>(bq[q], n_q, pq[q], k.T_cm, apr2);
+                  c = median_fallback<N>(BqPack<N>{bq[q]}, n_q, pq[q], k.T_cm, apr2);
                 } else if (!even) {
                   c = d_q == 0 ? min_ge<N>(bq[q], p_q, BIG2) : max_lt<N>(bq[q], p_q, BIG2);
                 } else if (d_q == 1) {
