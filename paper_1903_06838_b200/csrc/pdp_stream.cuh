@@ -94,7 +94,7 @@ __device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // 
   asm volatile(
       "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
       : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity), "r"(20000u)
+      : "r"(smem_u32(bar)), "r"(parity), "r"(100000u)
       : "memory");
   return ok != 0;
 }
@@ -483,7 +483,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
         if (g0 < nf) {
           // every dense warp has published (frame group, band): acquire on the group's mbarrier
           while (!mbar_test(&bar[(bd.gb % kNB) * kSparseWarps + sw], (uint32_t)(bd.gb / kNB) & 1u))
-            __nanosleep(2000);  // a sleeping warp costs no issue slots; a band of dense work lasts tens of microseconds
+            __nanosleep(6000);  // a sleeping warp costs no issue slots; a band of dense work lasts tens of microseconds
           stream_sparse(sp, smem, g0, min(1 << gsh, nf - g0), bd, fs + c0 + g0, list, sw);
         } else if (lane == 0) {
           done[sw] = bd.gb + 1;
