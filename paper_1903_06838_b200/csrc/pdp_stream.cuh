@@ -1,23 +1,22 @@
 // pdp_stream.cuh — the throughput kernel (one launch per pdp_process call for large batches).
 //
-// Built around the measured sm_100a issue model (DESIGN.md §6): one warp-instruction per cycle and
+// Built around the measured sm_100a issue model (DESIGN.md §5.1): one warp-instruction per cycle and
 // SM sub-partition, FFMA/FADD one cycle on the FMA pipe, every compare/select/permute/logic and
 // every packed-half instruction two cycles, so at 2 B/pixel the HBM roofline leaves ~11 issue
 // slots per pixel-lane.  Consequences:
-//   * no staging through shared memory and no CTA-wide barriers: a warp owns one row segment of a
-//     band (maps in registers), streams the raw pixels of its frames straight from global memory
-//     with 64/128-bit loads, the next frames prefetched into registers while it computes;
-//   * FL frames are processed in lock-step by one warp: their selection searches share every
-//     warp-wide reduction (counts packed into one REDUX) and the pivot logic runs once, each
-//     half-warp steering one search;
+//   * no CTA-wide barriers and no shared tiles: a warp owns one row segment of a band (its
+//     calibration maps in registers or in a private shared-memory tile) and streams the raw pixels
+//     of its frames with 64/128-bit cp.async copies into a private ring, six frames ahead;
+//   * the loop body is kept small (one estimator per kernel variant, rare paths out of line): two
+//     frames per warp in lock-step were measured slower than one, the body outgrows the instruction cache;
 //   * the masked value is ONE FFMA: bq = a + [|a| >= T_cm] * BIG, so pixels outside the mask sort
 //     above every pivot and still carry their value for the seed-candidate test;
 //   * the exact median is found by counting passes (FSET + FADD per pixel) that stop as soon as
 //     a pivot's rank is k, k+1 (or k+2 for an even count) and one push-and-min/max pass
 //     (FSET + FFMA + 1/2 FMNMX3) reads the order statistic itself; everything that does not
 //     converge (ties) goes to the generic bisection of pdp_device.cuh;
-//   * the sparse stage (fp64 seed rule, 3x3 sum, centroid, ordered emission) of a (frame, band) is
-//     run by whichever warp finishes that band of that frame last; nobody waits for it.
+//   * the sparse stage (fp64 seed rule, 3x3 sum, centroid, ordered emission) runs on four dedicated
+//     warps that sleep on mbarriers until all dense warps have published a (band, frame group).
 //
 // Decomposition: frame-owner.  CTA b owns frames [fs, fe); it walks them in chunks of kFCH frames,
 // band by band (R rows x all segments = one warp each), frames innermost, so the calibration maps

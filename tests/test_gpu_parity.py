@@ -230,3 +230,46 @@ def test_many_frames_auto_kernel(oracle, cm_mode):
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
+
+
+def test_full_size_config1_sampled(oracle):
+    """BASELINE.json configs[1] at full size (2000 frames of 704x768), in the launch configuration bench.py
+    times (one pdp_process call over the whole batch, auto kernel choice, capacity like the bench): sampled
+    frames - first, last, around CTA ownership boundaries (2000/148 = 13.5 frames per CTA) and chunk
+    boundaries - are compared hit by hit with the oracle; invariants that hold at any size cover the rest."""
+    cfg, n = small(1), 2000
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, 0, cap=1112)
+    assert g["status"][0] == 0 and g["launches"] == 1
+    sample = sorted({0, 1, 12, 13, 14, 15, 16, 27, 28, 999, 1000, 1013, 1014, 1986, 1987, 1998, 1999})
+    picked = raw.view(torch.int16)[torch.tensor(sample, device=raw.device)].view(torch.uint16)   # uint16 has no index kernel
+    o = oracle_run(oracle, cfg, picked, ped, gain, 0)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, frames=sample, check_accum=False)
+    print(rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 3000 and rep.exempt_hits <= 3
+    # any-size invariants over ALL frames
+    hc = g["hit_count"]
+    assert hc.min() > 100 and hc.max() < 1112
+    k = np.arange(g["hit_pixel"].shape[1])[None, :] < hc[:, None]
+    px = g["hit_pixel"].astype(np.int64) & 0xFFFFFFFF
+    inc = (np.diff(px, axis=1) > 0) | ~k[:, 1:]
+    assert inc.all()                                                       # strictly increasing lists
+    nph = np.where(k, g["hit_nphot"], 0).astype(np.int64)
+    assert np.array_equal(nph.sum(1), g["frame_photons"])                   # totals = sum of listed n
+    acc = np.zeros(cfg.npix, np.int64)
+    np.add.at(acc, px[k], nph[k])
+    assert np.array_equal(acc, g["accum"].astype(np.int64) & 0xFFFFFFFF)    # accum = scatter of all lists
+
+
+def test_full_size_config0(oracle):
+    """configs[0] at full size (100 frames of 185x388, S = 194: padded lanes, 4-byte vectors), every frame."""
+    cfg, n = small(0), 100
+    raw, ped, gain = make(cfg, n)
+    for cm_mode in (0, 1):
+        g = gpu_run(cfg, raw, ped, gain, cm_mode)
+        o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        print(rep.summary())
+        assert rep.ok, rep.failures[:10]
+        assert rep.hits_oracle > 20000 and rep.exempt_hits <= rep.hits_oracle // 200
