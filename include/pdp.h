@@ -119,7 +119,7 @@ typedef struct pdp_output {
  *     the device; the context keeps derived maps, not the host pointers).
  *   out_ctx : receives the context.
  * Errors: PDP_E_NULL, PDP_E_GEOMETRY (also: cols or seg_cols odd, seg_cols > 1024,
- * more than 8 segments per row), PDP_E_VALUE (checked over every map element),
+ * more than 6 segments per row), PDP_E_VALUE (checked over every map element),
  * PDP_E_NO_SM100, PDP_E_CUDA, PDP_E_NOMEM.  On error *out_ctx is set to NULL.
  */
 int pdp_create(const pdp_geometry *geometry, const float *pedestal_host, const float *gain_host,

@@ -440,7 +440,6 @@ template <int V, int G, int MS>
 __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(const SParams sp) {
   constexpr int FL = 1;   // frames per iteration
   constexpr int N = V * G;
-  constexpr int GL = 32 / FL;  // lanes steering one search
   const KParams &k = sp.k;
   extern __shared__ __align__(16) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -496,7 +495,6 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
   const size_t npix = (size_t)k.P * k.H * k.W;
   const float BIG = sp.big, BIG2 = 4.f * sp.big;
   const uint32_t magic = sp.magic;
-  const int ms = lane / GL;  // the search this lane steers
   float apr = 0.375f * k.T_cm / (float)k.S;  // ADU per rank near the median (running estimate)
   float *smap = reinterpret_cast<float *>(smem + sp.off_maps) + (size_t)warp * (3 * N * 32) + lane * V;  // this lane's map vectors (MS)
   constexpr bool kMapsSmem = MS == 1, kMedian = MS != 0;
