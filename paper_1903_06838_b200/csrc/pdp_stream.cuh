@@ -38,6 +38,7 @@ constexpr int kStreamThreadsOf(int ms) { return (kDenseWarpsMaxOf(ms) + kSparseW
 constexpr int kFCH = 16;    // frames per chunk = frame slots of the shared-memory rings
 constexpr int kNB = 5;     // band slots of the shared-memory rings: a dense warp may run kNB-1 bands ahead of the sparse stage
 constexpr int kRingD = 6;  // frame groups in flight per warp (cp.async ring)
+constexpr int kAcc = 1;    // a pivot is accepted when its rank is within kAcc of the wanted ones; the read-out walks the rest
 constexpr int kMaxIt = 9;   // counting passes before the generic bisection takes over
 
 struct SParams {
@@ -668,7 +669,7 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
                 else a2 += d;
               }
               const int c = warp_sum_i(__float2int_rn(a0 + a1 + a2));
-              if ((unsigned)(c - kl) <= (unsigned)(kh + 1 - kl)) {
+              if ((unsigned)(c - kl + kAcc) <= (unsigned)(kh + 1 - kl + 2 * kAcc)) {   // rank in [kl-kAcc, kh+1+kAcc]
                 state = 1;
                 c_fin = c;
                 break;
@@ -706,20 +707,46 @@ __global__ void __launch_bounds__(kStreamThreadsOf(MS), 1) pdp_stream_kernel(con
                 if (f_q) {
                   float apr2 = apr;
                   c = median_fallback<N>(BqPack<N>{bq[q]}, n_q, pq[q], k.T_cm, apr2);
-                } else if (!even) {
-                  c = d_q == 0 ? min_ge<N>(bq[q], p_q, BIG2) : max_lt<N>(bq[q], p_q, BIG2);
-                } else if (d_q == 1) {
-                  c = 0.5f * (max_lt<N>(bq[q], p_q, BIG2) + min_ge<N>(bq[q], p_q, BIG2));
-                } else if (d_q == 0) {   // x[kl] = min >= p; x[kh] = the next one (or an equal one)
-                  const float A = min_ge<N>(bq[q], p_q, BIG2);
-                  int n_le;
-                  const float B = min_gt_count<N>(bq[q], A, BIG2, n_le);
-                  c = 0.5f * (A + (n_le >= kl_q + 2 ? A : B));
-                } else {                 // d == 2: x[kh] = max < p; x[kl] = the one before (or an equal one)
-                  const float B = max_lt<N>(bq[q], p_q, BIG2);
-                  int n_lt;
-                  const float A = max_lt_count<N>(bq[q], B, BIG2, n_lt);
-                  c = 0.5f * (B + (n_lt <= kl_q ? B : A));
+                } else {
+                  // read x[kl] and x[kh] by walking from the pivot (rank c_p = #{b < p}): every pass
+                  // returns one order statistic and, from the second on, how many ranks it covers (ties)
+                  const int c_p = kl_q + d_q, kh_q = n_q >> 1;
+                  float xl, xh;
+                  if (c_p <= kl_q) {                 // walk up: A = x[r0]
+                    float A = min_ge<N>(bq[q], p_q, BIG2);
+                    int r0 = c_p;
+                    bool gotl = false;
+                    xl = xh = A;
+                    for (;;) {
+                      if (!gotl && kl_q == r0) xl = A, gotl = true;
+                      if (kh_q == r0) { xh = A; break; }
+                      int n_le;
+                      const float A2 = min_gt_count<N>(bq[q], A, BIG2, n_le);   // ranks [r0, n_le) hold A
+                      if (!gotl && kl_q < n_le) xl = A, gotl = true;
+                      if (kh_q < n_le) { xh = A; break; }
+                      A = A2;
+                      r0 = n_le;
+                    }
+                  } else if (c_p > kh_q) {           // walk down: B = x[r1]
+                    float B = max_lt<N>(bq[q], p_q, BIG2);
+                    int r1 = c_p - 1;
+                    bool goth = false;
+                    xl = xh = B;
+                    for (;;) {
+                      if (!goth && kh_q == r1) xh = B, goth = true;
+                      if (kl_q == r1) { xl = B; break; }
+                      int n_lt;
+                      const float B2 = max_lt_count<N>(bq[q], B, BIG2, n_lt);   // ranks [n_lt, r1] hold B
+                      if (!goth && kh_q >= n_lt) xh = B, goth = true;
+                      if (kl_q >= n_lt) { xl = B; break; }
+                      B = B2;
+                      r1 = n_lt - 1;
+                    }
+                  } else {                           // even count, the pivot splits the two middle elements
+                    xl = max_lt<N>(bq[q], p_q, BIG2);
+                    xh = min_ge<N>(bq[q], p_q, BIG2);
+                  }
+                  c = 0.5f * (xl + xh);
                 }
               }
               cq[q] = c;
