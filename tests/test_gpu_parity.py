@@ -273,3 +273,30 @@ def test_full_size_config0(oracle):
         print(rep.summary())
         assert rep.ok, rep.failures[:10]
         assert rep.hits_oracle > 20000 and rep.exempt_hits <= rep.hits_oracle // 200
+
+
+@pytest.mark.parametrize("kernel", ["stream", "lookback"])
+def test_seed_threshold_below_mask_threshold(oracle, kernel):
+    """T_seed < T_cm: pixels INSIDE the common-mode mask can seed (the kernels' rare 'low' candidate path)."""
+    cfg, n = small(0, rows=40, cols=256, seg_cols=128, occupancy=0.01, photon_adu=30.0, seed_adu=12.0), 80
+    raw, ped, gain = make(cfg, n)
+    for cm_mode in (0, 1):
+        g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel=kernel)
+        o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        print(rep.summary())
+        assert rep.ok, rep.failures[:10]
+        assert rep.hits_oracle > 2000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
+
+
+def test_wide_gain_range_and_min_count(oracle):
+    """Gains from 0.25 to 4 (BIG grows with max |v1|), and a cm_min_count that most segments miss (c = 0)."""
+    cfg, n = small(4, panels=1, rows=48, gain_lo=0.25, gain_hi=4.0), 90
+    raw, ped, gain = make(cfg, n)
+    for cm_min_count in (0, 250):
+        g = gpu_run(cfg, raw, ped, gain, 0, cm_min_count=cm_min_count, kernel="stream")
+        o = oracle_run(oracle, cfg, raw, ped, gain, 0, cm_min_count=cm_min_count)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        print(cm_min_count, rep.summary())
+        assert rep.ok, rep.failures[:10]
+        assert rep.hits_oracle > 1000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
