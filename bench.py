@@ -33,7 +33,7 @@ NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum of pdp_fused_kernel per launch, from the committed
 # `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"cfg1_median_2000": 2207638632}   # profiles/r1_final_stream_kernel_ncu.md
+NCU_TRAFFIC_BYTES = {"cfg1_median_2000": 2207027512}   # profiles/r1_final_stream_kernel_ncu.md
 CM_MODES = {"median": 0, "mean": 1, "none": 2}
 
 
