@@ -300,3 +300,18 @@ def test_wide_gain_range_and_min_count(oracle):
         print(cm_min_count, rep.summary())
         assert rep.ok, rep.failures[:10]
         assert rep.hits_oracle > 1000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
+
+
+def test_wide_panel_falls_back_to_staged_kernel(oracle):
+    """W = 1280 (> 1024 columns: more than 32 bitmap words per row) is outside the streaming kernel's
+    geometry; a large batch must then run on the staged frame-owner kernel with identical results."""
+    cfg, n = small(0, rows=24, cols=1280, seg_cols=640, occupancy=0.004), 90
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, 0)                 # auto choice
+    o = oracle_run(oracle, cfg, raw, ped, gain, 0)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    print(rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 3000 and g["launches"] == 1
+    with pytest.raises(binding.PdpError):
+        gpu_run(cfg, raw, ped, gain, 0, kernel="stream")   # pinning the streaming kernel must fail loudly
