@@ -73,7 +73,7 @@ static int cmp_double(const void *a, const void *b) {
 
 /* O3: common-mode estimate of one group of S values. */
 static double common_mode(const double *v1, int S, const oracle_params *prm, double *scratch,
-                          int *fragile_mask) {
+                          int *fragile_mask, int *count_out) {
   int k = 0;
   double sum = 0.0;
   *fragile_mask = 0;
@@ -85,6 +85,7 @@ static double common_mode(const double *v1, int S, const oracle_params *prm, dou
       sum += v1[j];
     }
   }
+  *count_out = k; /* "number of segmented pixels"; reported, not used below */
   if (prm->cm_mode == ORACLE_CM_NONE) {
     *fragile_mask = 0;
     return 0.0;
@@ -104,14 +105,16 @@ static double common_mode(const double *v1, int S, const oracle_params *prm, dou
 
 /*
  * One frame.  Outputs (any may be NULL): v2_out[Npix], cm_out[Npix/seg_cols],
- * fragile_out[Npix] (OR of FRAGILE_* bits); hit arrays of `hit_capacity` slots.
+ * cm_count_out[Npix/seg_cols] (number of segmented pixels #M of each group; the comparator bounds
+ * what one flipped mask pixel can do with it), fragile_out[Npix] (OR of FRAGILE_* bits); hit arrays
+ * of `hit_capacity` slots.
  * Returns the TRUE number of seeds (may exceed hit_capacity; only the first
  * hit_capacity are stored).  photons_out receives sum of n over all seeds.
  * accum (may be NULL) gets += n at every seed.
  */
 int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const float *gain,
                          const oracle_params *prm, const uint16_t *raw, double *v2_out,
-                         double *cm_out, uint8_t *fragile_out, int64_t hit_capacity,
+                         double *cm_out, int32_t *cm_count_out, uint8_t *fragile_out, int64_t hit_capacity,
                          uint32_t *hit_pixel, double *hit_charge, int32_t *hit_nphot,
                          double *hit_dx, double *hit_dy, uint64_t *photons_out, uint32_t *accum) {
   const int P = g->panels, H = g->rows, W = g->cols, S = g->seg_cols;
@@ -136,9 +139,10 @@ int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const 
     for (int r = 0; r < H; ++r)
       for (int s = 0; s < nseg; ++s) {
         int64_t base = ((int64_t)p * H + r) * W + (int64_t)s * S;
-        int fmask;
-        double c = common_mode(v2 + base, S, prm, scratch, &fmask);
+        int fmask, k;
+        double c = common_mode(v2 + base, S, prm, scratch, &fmask, &k);
         if (cm_out) cm_out[((int64_t)p * H + r) * nseg + s] = c;
+        if (cm_count_out) cm_count_out[((int64_t)p * H + r) * nseg + s] = k;
         for (int j = 0; j < S; ++j) {
           v2[base + j] -= c;
           if (fmask) frag[base + j] |= FRAGILE_F1;
@@ -214,7 +218,7 @@ int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const 
  * frame_photons[n_frames]; accum[Npix] += n of EVERY seed (also those past
  * hit_capacity; integer atomic adds, so the thread schedule cannot change the
  * result); fragile_out [n_frames][Npix]
- * and cm_out [n_frames][Npix/seg_cols] optional.  Returns 0, or -1 on
+ * and cm_out / cm_count_out [n_frames][Npix/seg_cols] optional.  Returns 0, or -1 on
  * allocation failure.
  */
 int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const float *gain,
@@ -222,7 +226,7 @@ int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const floa
                      int32_t threads, int64_t hit_capacity, int64_t *hit_count,
                      uint32_t *hit_pixel, double *hit_charge, int32_t *hit_nphot, double *hit_dx,
                      double *hit_dy, uint64_t *frame_photons, uint32_t *accum, double *cm_out,
-                     uint8_t *fragile_out) {
+                     int32_t *cm_count_out, uint8_t *fragile_out) {
   const int64_t npix = (int64_t)g->panels * g->rows * g->cols;
   const int64_t nsegs = npix / g->seg_cols;
   int failed = 0;
@@ -233,7 +237,7 @@ int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const floa
     int64_t off = (int64_t)f * hit_capacity;
     int64_t cnt = pdp_oracle_frame(
         g, pedestal, gain, prm, raw + (int64_t)f * npix, NULL, cm_out ? cm_out + f * nsegs : NULL,
-        fragile_out ? fragile_out + f * npix : NULL, hit_capacity, hit_pixel + off,
+        cm_count_out ? cm_count_out + f * nsegs : NULL, fragile_out ? fragile_out + f * npix : NULL, hit_capacity, hit_pixel + off,
         hit_charge + off, hit_nphot + off, hit_dx + off, hit_dy + off, &ph, accum);
     if (cnt < 0) {
 #pragma omp atomic write

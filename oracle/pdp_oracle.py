@@ -68,7 +68,8 @@ class OracleResult:
     frame_photons: np.ndarray  # [n] uint64
     accum: np.ndarray          # [npix] uint32 (this batch only)
     cm: np.ndarray | None      # [n, npix/S] float64
-    fragile: np.ndarray | None  # [n, npix] uint8
+    cm_count: np.ndarray | None = None  # [n, npix/S] int32: #M, number of segmented pixels of each group
+    fragile: np.ndarray | None = None  # [n, npix] uint8
 
 
 def max_hits(panels: int, rows: int, cols: int) -> int:
@@ -102,13 +103,14 @@ def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_a
     accum = np.zeros(npix, np.uint32)
     cm = np.zeros((n, npix // seg_cols), np.float64) if want_cm else None
     frag = np.zeros((n, npix), np.uint8) if want_fragile else None
+    cmn = np.zeros((n, npix // seg_cols), np.int32) if (want_cm or want_fragile) else None
     rc = lib.pdp_oracle_batch(
         ctypes.byref(g), _ptr(pedestal, ctypes.c_float), _ptr(gain, ctypes.c_float),
         ctypes.byref(p), _ptr(raw, ctypes.c_uint16), ctypes.c_int32(n), ctypes.c_int32(threads),
         ctypes.c_int64(cap), _ptr(hit_count, ctypes.c_int64), _ptr(hp, ctypes.c_uint32),
         _ptr(he, ctypes.c_double), _ptr(hn, ctypes.c_int32), _ptr(hx, ctypes.c_double),
         _ptr(hy, ctypes.c_double), _ptr(fp, ctypes.c_uint64), _ptr(accum, ctypes.c_uint32),
-        _ptr(cm, ctypes.c_double), _ptr(frag, ctypes.c_uint8))
+        _ptr(cm, ctypes.c_double), _ptr(cmn, ctypes.c_int32), _ptr(frag, ctypes.c_uint8))
     if rc != 0:
         raise MemoryError("pdp_oracle_batch failed")
     k = np.minimum(hit_count, cap)
@@ -119,7 +121,7 @@ def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_a
         hit_nphot=[hn[f, :k[f]].copy() for f in range(n)],
         hit_dx=[hx[f, :k[f]].copy() for f in range(n)],
         hit_dy=[hy[f, :k[f]].copy() for f in range(n)],
-        frame_photons=fp, accum=accum, cm=cm, fragile=frag)
+        frame_photons=fp, accum=accum, cm=cm, cm_count=cmn, fragile=frag)
 
 
 def frame_v2(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_adu, photon_adu,
@@ -139,7 +141,7 @@ def frame_v2(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_
     cnt = lib.pdp_oracle_frame(
         ctypes.byref(g), _ptr(pedestal, ctypes.c_float), _ptr(gain, ctypes.c_float),
         ctypes.byref(p), _ptr(raw, ctypes.c_uint16), _ptr(v2, ctypes.c_double),
-        _ptr(cm, ctypes.c_double), None, ctypes.c_int64(0), None, None, None, None, None,
+        _ptr(cm, ctypes.c_double), None, None, ctypes.c_int64(0), None, None, None, None, None,
         ctypes.byref(ph), None)
     if cnt < 0:
         raise MemoryError("pdp_oracle_frame failed")

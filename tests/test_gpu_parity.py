@@ -97,7 +97,7 @@ def test_parity(oracle, case, cm_mode, kernel):
     raw, ped, gain = make(cfg, n)
     g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel=kernel)
     o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(case, cm_mode, rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 0
@@ -138,7 +138,7 @@ def test_integer_exact_suite(oracle):
                             (1, "frames"), (2, "frames_pf"), (2, "lookback")):
         g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-        rep = compare(o, g, panels=P, rows=H, cols=W)
+        rep = compare(o, g, panels=P, rows=H, cols=W, seg_cols=S, cm_adu=cfg.cm_adu)
         print(cm_mode, kernel, rep.summary())
         assert rep.ok, rep.failures[:10]
         if cm_mode != 1:
@@ -195,7 +195,7 @@ def test_chunking_determinism_accumulation_and_host_feed(oracle, monkeypatch):
         assert np.array_equal(ref[k], host[k]), k
     assert host["launches"] == 3
     o = oracle_run(oracle, cfg, raw, ped, gain, 0)
-    assert compare(o, ref, panels=1, rows=cfg.rows, cols=cfg.cols).ok
+    assert compare(o, ref, panels=1, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu).ok
 
 
 def test_occupancy_independence_of_lists(oracle):
@@ -212,7 +212,7 @@ def test_many_frames_prefilter(oracle, cm_mode):
     raw, ped, gain = make(cfg, n)
     g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel="frames_pf")
     o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
@@ -226,7 +226,7 @@ def test_many_frames_auto_kernel(oracle, cm_mode):
     raw, ped, gain = make(cfg, n)
     g = gpu_run(cfg, raw, ped, gain, cm_mode)
     o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
@@ -244,7 +244,7 @@ def test_full_size_config1_sampled(oracle):
     sample = sorted({0, 1, 12, 13, 14, 15, 16, 27, 28, 999, 1000, 1013, 1014, 1986, 1987, 1998, 1999})
     picked = raw.view(torch.int16)[torch.tensor(sample, device=raw.device)].view(torch.uint16)   # uint16 has no index kernel
     o = oracle_run(oracle, cfg, picked, ped, gain, 0)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, frames=sample, check_accum=False)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu, frames=sample, check_accum=False)
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 3000 and rep.exempt_hits <= 3
@@ -269,7 +269,7 @@ def test_full_size_config0(oracle):
     for cm_mode in (0, 1):
         g = gpu_run(cfg, raw, ped, gain, cm_mode)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
         print(rep.summary())
         assert rep.ok, rep.failures[:10]
         assert rep.hits_oracle > 20000 and rep.exempt_hits <= rep.hits_oracle // 200
@@ -283,7 +283,7 @@ def test_seed_threshold_below_mask_threshold(oracle, kernel):
     for cm_mode in (0, 1):
         g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel=kernel)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
-        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
         print(rep.summary())
         assert rep.ok, rep.failures[:10]
         assert rep.hits_oracle > 2000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
@@ -296,7 +296,7 @@ def test_wide_gain_range_and_min_count(oracle):
     for cm_min_count in (0, 250):
         g = gpu_run(cfg, raw, ped, gain, 0, cm_min_count=cm_min_count, kernel="stream")
         o = oracle_run(oracle, cfg, raw, ped, gain, 0, cm_min_count=cm_min_count)
-        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
         print(cm_min_count, rep.summary())
         assert rep.ok, rep.failures[:10]
         assert rep.hits_oracle > 1000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
@@ -309,7 +309,7 @@ def test_wide_panel_falls_back_to_staged_kernel(oracle):
     raw, ped, gain = make(cfg, n)
     g = gpu_run(cfg, raw, ped, gain, 0)                 # auto choice
     o = oracle_run(oracle, cfg, raw, ped, gain, 0)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 3000 and g["launches"] == 1

@@ -30,21 +30,25 @@ def _cases():
 
 @pytest.mark.parametrize("case", _cases(), ids=lambda c: c["name"])
 def test_handworked(oracle, case):
-    H, W, S = case["rows"], case["cols"], case["seg_cols"]
+    H, W, S, P = case["rows"], case["cols"], case["seg_cols"], case.get("panels", 1)
     if "raw_rows" in case:
         raw = np.array(case["raw_rows"], np.uint16)
     else:
-        raw = np.full((H, W), case.get("background", 0), np.uint16)
-        for r, c, v in case["nonzero"]:
-            raw[r, c] = v
-    ped = np.full((H, W), case["ped"], np.float32)
-    gain = np.full((H, W), case["gain"], np.float32)
-    res = run(oracle, raw[None], ped, gain, H, W, S, cm_mode=MODES[case["cm_mode"]],
+        raw = np.full((P, H, W), case.get("background", 0), np.uint16)
+        for r, c, v in case.get("nonzero", []):
+            raw[0, r, c] = v
+        for p, r, c, v in case.get("nonzero_p", []):       # [panel, row, col, value]
+            raw[p, r, c] = v
+    ped = np.full((P, H, W), case["ped"], np.float32)
+    gain = np.full((P, H, W), case["gain"], np.float32)
+    res = run(oracle, raw.reshape(1, -1), ped, gain, H, W, S, panels=P, cm_mode=MODES[case["cm_mode"]],
               cm_min_count=case.get("cm_min_count", 0), want_cm=True)
     if "cm" in case:
         np.testing.assert_allclose(res.cm[0], case["cm"], rtol=0, atol=1e-12)
+    if "cm_count" in case:
+        assert res.cm_count[0].tolist() == case["cm_count"]
     if "v2" in case:
-        v2, _ = oracle.frame_v2(raw, ped, gain, panels=1, rows=H, cols=W, seg_cols=S,
+        v2, _ = oracle.frame_v2(raw, ped, gain, panels=P, rows=H, cols=W, seg_cols=S,
                                 cm_mode=MODES[case["cm_mode"]],
                                 cm_min_count=case.get("cm_min_count", 0), **TH)
         np.testing.assert_allclose(v2[0], case["v2"], rtol=0, atol=1e-12)
@@ -84,7 +88,11 @@ def test_dark_gain_closed_form(oracle):
 
 @pytest.mark.parametrize("S,W", [(8, 16), (194, 388), (7, 21), (384, 768)])
 def test_common_mode_matches_numpy(oracle, S, W):
-    """MEDIAN reduces to numpy.median on the masked subset, MEAN_GUARDED to sum/max(k, sqrt(S))."""
+    """MEDIAN reduces to numpy.median on the masked subset (a library routine: a real pin).
+    The MEAN_GUARDED line below RESTATES the oracle's own formula sum/max(k, sqrt(S)): it guards against
+    typos only.  What pins the guard is the hand-worked `guard_mean_1x8` fixture (7/sqrt(8)) and, where
+    k >= sqrt(S), numpy's plain mean at the end of this test; the guard's FORM against the paper is
+    parity unpinned by necessity (Fig. 3 is missing, R4)."""
     rng = np.random.default_rng(S)
     H = 12
     ped = rng.normal(1000, 20, (H, W)).astype(np.float32)
@@ -188,6 +196,40 @@ def test_seed_rule_bruteforce_8x8(oracle):
     assert run(oracle, f[None], ped, gain, 8, 8, 8, cm_mode=2).hit_pixel[0].tolist() == [2 * 8 + 3]
     f = np.zeros((8, 8), np.uint16); f[2, 2] = 60; f[2, 4] = 60        # same window, not adjacent
     assert run(oracle, f[None], ped, gain, 8, 8, 8, cm_mode=2).hit_pixel[0].tolist() == [18, 20]
+
+
+def test_seed_rule_bruteforce_two_panels(oracle):
+    """Panels never neighbour each other (R12): on random 2-panel frames the
+    seeds must equal the independently written rule applied to EACH PANEL ALONE.  Values cluster at the
+    panel seam (last rows of panel 0, first rows of panel 1), so an oracle that let row H-1 of panel 0
+    neighbour row 0 of panel 1 (they are adjacent in memory) fails here."""
+    P, H, W = 2, 4, 5
+    ped = np.zeros((P, H, W), np.float32)
+    gain = np.ones((P, H, W), np.float32)
+    rng = np.random.default_rng(11)
+    frames = []
+    for _ in range(2000):
+        f = np.zeros((P, H, W), np.uint16)
+        for _ in range(rng.integers(2, 7)):
+            p = rng.integers(0, 2)
+            r = (H - 1 - rng.integers(0, 2)) if p == 0 else rng.integers(0, 2)
+            f[p, r, rng.integers(0, W)] = (60, 60, 70, 105)[rng.integers(0, 4)]
+        frames.append(f)
+    raw = np.stack(frames).reshape(len(frames), -1)
+    res = run(oracle, raw, ped, gain, H, W, W, panels=P, cm_mode=2)
+    n_seam = 0
+    for i, f in enumerate(frames):
+        want = []
+        for p in range(P):
+            want += [p * H * W + q for q in _independent_seeds(f[p].astype(np.float64), 50.0)]
+        assert res.hit_pixel[i].tolist() == want, (i, f, res.hit_pixel[i].tolist(), want)
+        # the same frame read as ONE panel of 2H rows would often give a different answer
+        n_seam += want != _independent_seeds(f.reshape(P * H, W).astype(np.float64), 50.0)
+        for k, q in enumerate(want):                      # E only sums pixels of the seed's own panel
+            p, r, c = q // (H * W), (q // W) % H, q % W
+            win = f[p, max(0, r - 1):r + 2, max(0, c - 1):c + 2].astype(np.float64)
+            assert res.hit_charge[i][k] == win.sum()
+    assert n_seam > 300          # the seam mattered in a good share of the frames
 
 
 def test_rounding_table(oracle):
@@ -322,3 +364,53 @@ def test_fragile_flags(oracle):
     gain[0, 2] = np.float32(1.0 / (50.0 + 5e-5))
     res = run(oracle, raw[None], ped, gain, 1, W, 4, cm_mode=2, want_fragile=True)
     assert res.fragile[0][2] & 2 and res.fragile[0][5] == 0
+
+
+def _frame_with_values(vals, W=8):
+    """1 x W frame whose v1 equals `vals` (col -> value) to fp64 rounding of 1/float32(1/v)."""
+    ped = np.zeros((1, W), np.float32)
+    gain = np.ones((1, W), np.float32)
+    raw = np.zeros((1, W), np.uint16)
+    for c, v in vals.items():
+        gain[0, c] = np.float32(1.0 / v)
+        raw[0, c] = 1
+    return raw, ped, gain
+
+
+def test_fragile_flags_f3_f4(oracle):
+    """F3: two 3x3 neighbours closer than the band (1e-4 ADU) while near/above T_seed flag BOTH pixels,
+    2e-4 apart flags nothing.  F4: E within the band of (k + 1/2) E_ph flags the seed, 2e-4 away does not.
+    (BASELINE.json: 'pixels whose fp64 value lies within 1e-4 ADU of a threshold'; R21.)
+    An over-wide F3/F4 would silently widen what tests/compare.py forgives; a missing one would make
+    the parity tests fail on legitimate rounding differences."""
+    F3, F4 = 4, 8
+    # two neighbours 5e-5 apart at 60 ADU (above T_seed = 50)
+    raw, ped, gain = _frame_with_values({2: 60.0, 3: 60.0 + 5e-5})
+    v1 = raw.astype(np.float64) / gain.astype(np.float64)
+    assert 2e-5 < abs(v1[0, 3] - v1[0, 2]) < 9e-5
+    res = run(oracle, raw[None], ped, gain, 1, 8, 8, cm_mode=2, want_fragile=True)
+    fr = res.fragile[0]
+    assert fr[2] & F3 and fr[3] & F3
+    assert not (fr[[0, 1, 4, 5, 6, 7]] & F3).any()           # background pairs (0 == 0) are far below T_seed
+    assert res.hit_pixel[0].tolist() == [3]                   # the larger one seeds
+    # 2e-4 apart: no F3 anywhere
+    raw, ped, gain = _frame_with_values({2: 60.0, 3: 60.0 + 2e-4})
+    res = run(oracle, raw[None], ped, gain, 1, 8, 8, cm_mode=2, want_fragile=True)
+    assert not (res.fragile[0] & F3).any()
+    # near-tie BELOW the seed threshold (30 ADU): irrelevant to any output, not flagged
+    raw, ped, gain = _frame_with_values({2: 30.0, 3: 30.0 + 5e-5})
+    res = run(oracle, raw[None], ped, gain, 1, 8, 8, cm_mode=2, want_fragile=True)
+    assert not (res.fragile[0] & F3).any() and res.hit_count[0] == 0
+    # non-adjacent pixels (columns 2 and 5) 5e-5 apart: not a 3x3 pair, not flagged
+    raw, ped, gain = _frame_with_values({2: 60.0, 5: 60.0 + 5e-5})
+    res = run(oracle, raw[None], ped, gain, 1, 8, 8, cm_mode=2, want_fragile=True)
+    assert not (res.fragile[0] & F3).any() and res.hit_pixel[0].tolist() == [2, 5]
+    # F4: lone pixel with E = 150 +- 5e-5 (rounding boundary 1.5 * E_ph) is flagged, 150 +- 2e-4 is not
+    for e, want in ((150.0 + 5e-5, True), (150.0 - 5e-5, True), (150.0 + 2e-4, False), (150.0 - 2e-4, False),
+                    (250.0 + 5e-5, True), (200.0 + 5e-5, False), (100.0, False)):
+        raw, ped, gain = _frame_with_values({4: e})
+        res = run(oracle, raw[None], ped, gain, 1, 8, 8, cm_mode=2, want_fragile=True)
+        assert res.hit_pixel[0].tolist() == [4]
+        assert bool(res.fragile[0][4] & F4) == want, e
+        assert not (res.fragile[0][[0, 1, 2, 3, 5, 6, 7]] & F4).any()
+        assert res.hit_nphot[0][0] == int(np.rint((1.0 / float(gain[0, 4])) / 100.0))
