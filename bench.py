@@ -1,17 +1,22 @@
 #!/usr/bin/env python
-"""bench.py — throughput of the fused reduction chain on BASELINE.json's headline workload.
+"""bench.py — throughput of the fused reduction chain on BASELINE.json's workloads.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--cm-mode median|mean]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--cm-mode median|mean|none]
     python bench.py --impl reference ...      # the fp64 oracle on the host cores (reference arm)
 
 A step is one pass of the whole hot path (dark, gain, common mode, seed finding, 3x3 charge sum,
 photon count, centroid, ordered hit lists, per-frame totals, accumulated image) over one batch of
-synthetic frames = ALL frames of the config (configs[1]: 2000 frames of 704x768 uint16, 2.16 GB,
-larger than L2).  Prints ONE JSON line (see DESIGN.md §8 for every field).
+synthetic frames = ALL frames of the config, device resident, through one pdp_process call.
+BASELINE.json's metric names no config, so the headline is the largest single-GPU one:
+configs[4], 4000 frames of 16 x 512 x 512 uint16 (33.5 GB, far larger than L2).  The JSON line also
+carries, under config.per_config, the same measurement for configs 0-3 (config 0 rotated over 20
+distinct copies so that it is not L2 resident) and, under e2e, config 4 streamed from pinned host
+memory.  Prints ONE JSON line (DESIGN.md §7 explains every field).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import statistics
@@ -31,10 +36,8 @@ METRIC = "frames/s through the fused pixel-detector reduction chain (also Mpixel
 UNIT = "frames/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "~8 TB/s"
 FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of pdp_fused_kernel per launch, from the committed
-# `ncu --set full` capture (profiles/); None until a capture of the current kernel exists.
-NCU_TRAFFIC_BYTES = {"cfg1_median_2000": 2207027512}   # profiles/r1_final_stream_kernel_ncu.md
 CM_MODES = {"median": 0, "mean": 1, "none": 2}
+ROTATE_COPIES = 20                # config 0 (14 MB per pass) is rotated over this many distinct copies
 
 
 def measured_peak():
@@ -44,6 +47,33 @@ def measured_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def kernel_source_hash() -> str:
+    """sha256 prefix of the CUDA sources: an ncu traffic figure is only quoted for the code it was captured on."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1903_06838_b200", "csrc")
+    for fn in sorted(os.listdir(d)):
+        if fn.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, fn), "rb") as f:
+                h.update(fn.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def recorded_traffic(cfg_id: int, cm_mode: str, n_frames: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed ncu capture
+    (profiles/ncu_traffic.json), or None when no capture of THIS source exists."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            table = json.load(f)["captures"]
+    except Exception:
+        return None
+    src = kernel_source_hash()
+    for e in table:
+        if (e.get("config") == cfg_id and e.get("cm_mode") == cm_mode and e.get("n_frames") == n_frames
+                and e.get("kernel") == kernel and e.get("source_sha16") == src):
+            return e.get("dram_bytes")
+    return None
 
 
 class ClockSampler:
@@ -91,8 +121,20 @@ def oracle_sample(cfg, raw_cpu, ped, gain, cm_mode, threads):
     t0 = time.perf_counter()
     res = pdp_oracle.process(raw_cpu, ped, gain, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols,
                              seg_cols=cfg.seg_cols, seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu,
-                             photon_adu=cfg.photon_adu, cm_mode=cm_mode, threads=threads, hit_capacity=4096)
+                             photon_adu=cfg.photon_adu, cm_mode=cm_mode, threads=threads,
+                             hit_capacity=min(cfg.max_hits, 65536))
     return time.perf_counter() - t0, res
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 def max_over_ranks(value: float, dist, device) -> float:
@@ -114,12 +156,22 @@ def workload_name(cfg):
             f"S={cfg.seg_cols}, E_ph={cfg.photon_adu:g}, T_seed={cfg.seed_adu:g}, T_cm={cfg.cm_adu:g}")
 
 
+def algorithmic_bytes(cfg, n, hits_per_frame):
+    """raw in + hits out + 8 B per frame, maps and accumulated image once per batch."""
+    return n * (cfg.npix * 2 + hits_per_frame * 20 + 8) + cfg.npix * 8 + cfg.npix * 8
+
+
+def ref_sample_frames(cfg, requested):
+    """Frames per oracle sample: about 25 Mpixel unless told otherwise (a few seconds on the host cores)."""
+    return requested or max(4, min(cfg.n_frames, int(25e6 // cfg.npix)))
+
+
 def run_reference(args, cfg, rank, world):
     if rank != 0:
         return
     threads = os.cpu_count() or 1
     ped, gain = synth.make_maps(cfg)
-    m = args.ref_frames
+    m = ref_sample_frames(cfg, args.ref_frames)
     raw = synth.make_frames(cfg, 0, m, ped, gain).numpy()
     cm = CM_MODES[args.cm_mode]
     for _ in range(args.warmup):
@@ -134,11 +186,144 @@ def run_reference(args, cfg, rank, world):
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode,
                        "sample": f"each step = the first {m} frames of the workload"},
-            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": threads, "kind": "oracle", "cpu": cpu_model(),
                              "sample": f"{m} frames x {args.steps} steps, frames over {threads} OpenMP threads"},
             "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "mpixel_per_s": fps * cfg.npix / 1e6}
     print(json.dumps(line))
+
+
+def make_context(binding, cfg, n, ped, gain, cm):
+    return binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
+                           max_frames_per_batch=n, pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu,
+                           cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm)
+
+
+def probe_capacity(binding, ctx, cfg, raw, n, dev, requested=0):
+    """A first pass at the no-overflow bound on a few frames sizes the lists (4x the most seen)."""
+    if requested:
+        return requested
+    probe = binding.alloc_output(min(n, 8), cfg.npix, cfg.max_hits, dev)
+    ctx.process(raw[: min(n, 8)], probe)
+    torch.cuda.synchronize()
+    seen = int(probe.hit_count.max())
+    return min(cfg.max_hits, max(256, 4 * seen))
+
+
+def time_config(binding, cfg, cm_name, dev, rank, steps, warmup, rotate=1, min_warm_s=0.0, dist=None, cap_req=0):
+    """Device-resident timing of one config: returns (result dict, objects kept for the caller)."""
+    cm = CM_MODES[cm_name]
+    n = cfg.n_frames
+    t0 = time.perf_counter()
+    ped, gain = synth.make_maps(cfg, dev)
+    raw = torch.empty((rotate * n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
+    synth.make_frames(cfg, first_frame_of_rank(rank, rotate * n), rotate * n, ped, gain, out=raw, block_pixels=1 << 27)
+    torch.cuda.synchronize()
+    gen_s = time.perf_counter() - t0
+    ctx = make_context(binding, cfg, n, ped, gain, cm)
+    cap = probe_capacity(binding, ctx, cfg, raw, n, dev, cap_req)
+    out = binding.alloc_output(n, cfg.npix, cap, dev)
+    stream = torch.cuda.current_stream()
+    views = [raw[i * n:(i + 1) * n] for i in range(rotate)]
+    calls = [0]
+
+    def step():
+        ctx.process(views[calls[0] % rotate], out, stream)
+        calls[0] += 1
+
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    launches = 0
+    t_w = time.perf_counter()
+    n_warm = 0
+    while n_warm < max(3, warmup) or time.perf_counter() - t_w < min_warm_s:
+        step()
+        n_warm += 1
+        if n_warm % 8 == 0:
+            torch.cuda.synchronize()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_begin.record(stream)
+    for a, b in ev:
+        a.record(stream)
+        step()
+        b.record(stream)
+        launches += ctx.last_launch_count
+    t_end.record(stream)
+    torch.cuda.synchronize()
+    total_ms = max_over_ranks(t_begin.elapsed_time(t_end), dist, dev)
+    k_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
+    assert int(out.status.item()) == 0, "hit overflow during the bench"
+    hits = float((out.hit_count.to(torch.int64) & 0xFFFFFFFF).to(torch.float64).mean().item())
+    peak, peak_src = measured_peak()
+    alg = algorithmic_bytes(cfg, n, hits)
+    res = {"n_frames": n, "ms": total_ms / steps, "kernel_ms": k_ms, "frames_per_s": n * steps / (total_ms * 1e-3),
+           "mpixel_per_s": n * steps * cfg.npix / (total_ms * 1e-3) / 1e6,
+           "raw_gbs": n * cfg.npix * 2 / (k_ms * 1e-3) / 1e9, "alg_gbs": alg / (k_ms * 1e-3) / 1e9,
+           "frac_of_measured": alg / (k_ms * 1e-3) / 1e9 / peak, "frac_of_8000": alg / (k_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+           "hits_per_frame": hits, "hit_capacity": cap, "kernel": ctx.last_kernel_name,
+           "launches_per_step": launches / steps, "generation_s": gen_s, "warmup_steps_run": n_warm,
+           "l2": ("rotated over %d distinct copies (%.0f MB) so that a pass is not L2 resident" % (rotate, rotate * n * cfg.npix * 2 / 1e6))
+                 if rotate > 1 else "inputs larger than L2 (%.2f GB per step)" % (n * cfg.npix * 2 / 1e9)}
+    keep = {"ctx": ctx, "out": out, "raw": raw, "ped": ped, "gain": gain, "cap": cap, "launches": launches,
+            "alg_bytes": alg, "peak": peak, "peak_src": peak_src, "total_ms": total_ms}
+    return res, keep
+
+
+def e2e_streamed(binding, cfg, keep, dev, steps, dist, world):
+    """The same batch through pdp_process_host from pinned host memory: chunked H2D copies on a side stream and
+    the D2H read of every output inside the timed region."""
+    ctx, out, raw, cap = keep["ctx"], keep["out"], keep["raw"], keep["cap"]
+    n = cfg.n_frames
+    stream = torch.cuda.current_stream()
+    note = "whole batch pinned"
+    try:
+        ring = n
+        raw_host = torch.empty((n,) + tuple(raw.shape[1:]), dtype=torch.uint16).pin_memory()
+    except RuntimeError:
+        ring = max(1, min(n, (4 << 30) // (cfg.npix * 2)))        # the box cannot pin the whole batch: cycle 4 GB
+        raw_host = torch.empty((ring,) + tuple(raw.shape[1:]), dtype=torch.uint16).pin_memory()
+        note = f"box cannot pin the whole batch: a pinned ring of {ring} frames is cycled"
+    raw_host.copy_(raw[:ring])
+    hc = torch.empty((n,), dtype=torch.int32).pin_memory()
+    fp = torch.empty((n,), dtype=torch.int32).pin_memory()
+    acc = torch.empty((cfg.npix,), dtype=torch.int32).pin_memory()
+    lists = [torch.empty((n, cap), dtype=dt).pin_memory() for dt in
+             (torch.int32, torch.float32, torch.int32, torch.float32, torch.float32)]
+    chunk = max(1, min(ring, (256 << 20) // (cfg.npix * 2)))      # ~256 MB per copy
+    launches = [0]
+
+    def e2e_step():
+        for f0 in range(0, n, ring):
+            m = min(ring, n - f0)
+            o = binding.Output(cap, out.hit_count[f0:], out.hit_pixel[f0:], out.hit_charge[f0:], out.hit_nphot[f0:],
+                               out.hit_dx[f0:], out.hit_dy[f0:], out.frame_photons[f0:], out.accum, out.status)
+            ctx.process_host(raw_host[:m], o, chunk, stream)
+            launches[0] += ctx.last_launch_count
+        hc.copy_(out.hit_count, non_blocking=True)
+        fp.copy_(out.frame_photons, non_blocking=True)
+        acc.copy_(out.accum, non_blocking=True)
+        for h, d in zip(lists, (out.hit_pixel, out.hit_charge, out.hit_nphot, out.hit_dx, out.hit_dy)):
+            h.copy_(d, non_blocking=True)
+
+    e2e_step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    launches[0] = 0
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+    d2h = 8 * n + 4 * cfg.npix + 20 * n * cap
+    return {"value": world * n * steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * cfg.npix * 2,
+            "d2h_bytes_per_step": d2h, "h2d_gbs": n * cfg.npix * 2 * steps / e2e_s / 1e9,
+            "d2h_gbs": d2h * steps / e2e_s / 1e9, "chunk_frames": chunk, "steps": steps, "pinned": note,
+            "launches_per_step": launches[0] / steps, "bound": "PCIe (host to device)",
+            "api": "pdp_process_host (pinned host frames, double-buffered side-stream copies)"}
 
 
 def main():
@@ -147,13 +332,16 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs")
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (headline: 4)")
     ap.add_argument("--frames", type=int, default=0, help="override the frame count (debug; 0 = the config's)")
     ap.add_argument("--cm-mode", default="median", choices=list(CM_MODES))
     ap.add_argument("--hit-capacity", type=int, default=0, help="slots per frame (0 = 4x the expected hits)")
-    ap.add_argument("--ref-frames", type=int, default=48, help="frames per step of the reference arm / cpu_baseline")
+    ap.add_argument("--ref-frames", type=int, default=0, help="frames per oracle sample (0 = about 25 Mpixel)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--per-config", default="0,1,2,3,4", help="configs for the per_config table ('' = none)")
+    ap.add_argument("--per-config-modes", default="median", help="comma list of cm modes for the per_config table")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -177,140 +365,92 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
 
-    # ---- synthetic workload, generated on the device, each rank its own frames (weak scaling) ----
-    t0 = time.perf_counter()
-    ped, gain = synth.make_maps(cfg, dev)
-    n = cfg.n_frames
-    raw = torch.empty((n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
-    synth.make_frames(cfg, first_frame_of_rank(rank, n), n, ped, gain, out=raw)
-    torch.cuda.synchronize()
-    gen_s = time.perf_counter() - t0
-
-    cm = CM_MODES[args.cm_mode]
-    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
-                          max_frames_per_batch=n, pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu,
-                          cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm)
-    # capacity: a first pass at the no-overflow bound on a few frames sizes the lists (4x the max seen)
-    probe = binding.alloc_output(min(n, 8), cfg.npix, cfg.max_hits, dev)
-    ctx.process(raw[: min(n, 8)], probe)
-    torch.cuda.synchronize()
-    seen = int(probe.hit_count.max())
-    cap = args.hit_capacity or min(cfg.max_hits, max(256, 4 * seen))
-    del probe
-    out = binding.alloc_output(n, cfg.npix, cap, dev)
-    stream = torch.cuda.current_stream()
-
-    def step():
-        ctx.process(raw, out, stream)
-
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    launches = 0
-    # The clock sampler runs from the warm-up on: a timed region of K steps lasts milliseconds, one
-    # nvidia-smi query ~100 ms, so the warm-up repeats the same step for >= 0.7 s (and >= W steps) and
-    # the samples cover warm-up + timed region, i.e. the same kernel under the same load.
+    # ---- headline: the whole config, device resident, one pdp_process call per step ----
+    # The clock sampler runs from the warm-up on: one nvidia-smi query takes ~100 ms, so the warm-up repeats the
+    # same step for >= 0.7 s (and >= W steps) and the samples cover warm-up + timed region under the same load.
+    rotate = ROTATE_COPIES if cfg.n_frames * cfg.npix * 2 < (200 << 20) else 1
     with ClockSampler(local) as clocks:
-        t_w = time.perf_counter()
-        n_warm = 0
-        while n_warm < max(3, args.warmup) or time.perf_counter() - t_w < 0.7:
-            step()
-            n_warm += 1
-            if n_warm % 8 == 0:
-                torch.cuda.synchronize()
-        torch.cuda.synchronize()
-        if dist:
-            dist.barrier()
-        torch.cuda.synchronize()
-        t_begin = torch.cuda.Event(enable_timing=True)
-        t_end = torch.cuda.Event(enable_timing=True)
-        t_begin.record(stream)
-        for a, b in ev:
-            a.record(stream)
-            step()
-            b.record(stream)
-            launches += ctx.last_launch_count
-        t_end.record(stream)
-        torch.cuda.synchronize()
-    total_ms = t_begin.elapsed_time(t_end)
-    kernel_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = max_over_ranks(total_ms, dist, dev)
+        res, keep = time_config(binding, cfg, args.cm_mode, dev, rank, args.steps, args.warmup, rotate=rotate,
+                                min_warm_s=0.7, dist=dist, cap_req=args.hit_capacity)
+    n = cfg.n_frames
     if dist:
         dist.barrier()
-    assert int(out.status.item()) == 0, "hit overflow during the bench"
-    hits_per_frame = float(out.hit_count.to(torch.float64).mean().item())
 
-    # ---- end to end through the C ABI with HOST buffers (pinned), H2D + D2H inside the timed region ----
     e2e = None
-    try:
-        raw_host = torch.empty(raw.shape, dtype=torch.uint16).pin_memory()
-        raw_host.copy_(raw)
-        hc = torch.empty((n,), dtype=torch.int32).pin_memory()
-        fp = torch.empty((n,), dtype=torch.int32).pin_memory()
-        acc = torch.empty((cfg.npix,), dtype=torch.int32).pin_memory()
-        lists = [torch.empty((n, cap), dtype=dt).pin_memory() for dt in
-                 (torch.int32, torch.float32, torch.int32, torch.float32, torch.float32)]
-        chunk = max(1, min(n, (256 << 20) // (cfg.npix * 2)))      # ~256 MB per copy
-        def e2e_step():
-            ctx.process_host(raw_host, out, chunk, stream)
-            hc.copy_(out.hit_count, non_blocking=True)
-            fp.copy_(out.frame_photons, non_blocking=True)
-            acc.copy_(out.accum, non_blocking=True)
-            for h, d in zip(lists, (out.hit_pixel, out.hit_charge, out.hit_nphot, out.hit_dx, out.hit_dy)):
-                h.copy_(d, non_blocking=True)
-        e2e_step()
-        torch.cuda.synchronize()
-        if dist:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            e2e_step()
-        torch.cuda.synchronize()
-        e2e_s = time.perf_counter() - t0
-        e2e_s = max_over_ranks(e2e_s, dist, dev)
-        d2h = 8 * n + 4 * cfg.npix + 20 * n * cap
-        e2e = {"value": world * n * args.e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": n * cfg.npix * 2,
-               "d2h_bytes_per_step": d2h, "h2d_gbs": n * cfg.npix * 2 * args.e2e_steps / e2e_s / 1e9,
-               "chunk_frames": chunk, "api": "pdp_process_host (pinned host frames, double-buffered side-stream copies)"}
-    except Exception as exc:  # e.g. the box cannot pin the whole batch
-        e2e = {"value": None, "unit": UNIT, "error": str(exc)[:200]}
+    if not args.no_e2e:
+        try:
+            e2e = e2e_streamed(binding, cfg, keep, dev, args.e2e_steps, dist, world)
+        except Exception as exc:
+            e2e = {"value": None, "unit": UNIT, "error": str(exc)[:200]}
 
-    # ---- roofline of the (single) kernel of a step ----
-    alg_bytes = n * (cfg.npix * 2 + hits_per_frame * 20 + 8) + cfg.npix * 8 + cfg.npix * 8
-    k_ms = statistics.mean(kernel_ms)
-    peak, peak_src = measured_peak()
-    achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-    key = f"cfg{cfg.cfg_id}_{args.cm_mode}_{n}"
-    kernel_name = "pdp_stream_kernel" if 2 * n >= torch.cuda.get_device_properties(dev).multi_processor_count else "pdp_fused_kernel"
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(key), "peak_source": peak_src, "kernel": kernel_name,
-                "kernel_ms": k_ms, "algorithmic_bytes_per_launch": alg_bytes,
-                "raw_gbs": n * cfg.npix * 2 / (k_ms * 1e-3) / 1e9,
-                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+    traffic = recorded_traffic(cfg.cfg_id, args.cm_mode, n, res["kernel"])
+    roofline = {"bound": "hbm", "achieved": res["alg_gbs"], "peak": keep["peak"], "unit": "GB/s",
+                "frac": res["frac_of_measured"], "traffic": traffic,
+                "traffic_source": "profiles/ncu_traffic.json (ncu --set full capture of this source)" if traffic else
+                                  "no ncu capture of the current kernel source",
+                "peak_source": keep["peak_src"], "kernel": res["kernel"], "kernel_ms": res["kernel_ms"],
+                "algorithmic_bytes_per_launch": keep["alg_bytes"], "raw_gbs": res["raw_gbs"],
+                "frac_of_nominal_8TBs": res["frac_of_8000"], "source_sha16": kernel_source_hash()}
 
-    fps = world * n * args.steps / (total_ms * 1e-3)
+    fps = world * n * args.steps / (keep["total_ms"] * 1e-3)
     line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "warmup": max(3, args.warmup), "ms_per_step": keep["total_ms"] / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 dense pass, f64 on seed candidates",
             "data": "synthetic", "mpixel_per_s": fps * cfg.npix / 1e6,
-            "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode, "hit_capacity": cap,
-                       "hits_per_frame": hits_per_frame, "l2": "inputs larger than L2 (%.2f GB per step)" % (n * cfg.npix * 2 / 1e9),
+            "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode, "hit_capacity": keep["cap"],
+                       "hits_per_frame": res["hits_per_frame"], "l2": res["l2"],
                        "sharding": "each rank processes its own full set of frames; no collective on the data path",
-                       "generation_s": gen_s, "warmup_steps_run": n_warm,
+                       "generation_s": res["generation_s"], "warmup_steps_run": res["warmup_steps_run"],
                        "clock_sampling": "nvidia-smi every 100 ms over warm-up (>= 0.7 s of the same step) + timed region"},
-            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline}
+            "clocks": clocks.summary(), "e2e": e2e, "gpu_launches": keep["launches"], "roofline": roofline}
 
     if rank == 0 and not args.no_cpu_baseline:
         threads = os.cpu_count() or 1
-        m = min(n, args.ref_frames)
-        sample = raw[:m].cpu().numpy()
-        dt, res = oracle_sample(cfg, sample, ped.cpu().numpy(), gain.cpu().numpy(), cm, threads)
-        line["cpu_baseline"] = {"value": m / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                "sample": f"first {m} frames of the workload, {dt:.1f} s, {threads} OpenMP threads over frames"}
+        m = ref_sample_frames(cfg, args.ref_frames)
+        sample = keep["raw"][:m].cpu().numpy()
+        pedn, gainn = keep["ped"].cpu().numpy(), keep["gain"].cpu().numpy()
+        cm = CM_MODES[args.cm_mode]
+        oracle_sample(cfg, sample[: max(1, m // 4)], pedn, gainn, cm, threads)          # warm-up
+        runs = [oracle_sample(cfg, sample, pedn, gainn, cm, threads) for _ in range(3)]
+        dt = statistics.median(r[0] for r in runs)
+        m1 = max(1, m // 8)
+        dt1, _ = oracle_sample(cfg, sample[:m1], pedn, gainn, cm, 1)
+        res_o = runs[0][1]
+        line["cpu_baseline"] = {"value": m / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "cpu": cpu_model(),
+                                "single_thread_value": m1 / dt1,
+                                "sample": f"first {m} frames of the workload, median of 3 runs after a warm-up "
+                                          f"({dt:.2f} s each), {threads} OpenMP threads over frames; single thread on {m1} frames"}
         # cheap cross-check of the timed run against the oracle on the sample (counts must agree)
         line["cpu_baseline"]["hit_count_equal"] = bool(
-            (torch.as_tensor(res.hit_count) == out.hit_count[:m].cpu().to(torch.int64)).all())
+            (torch.as_tensor(res_o.hit_count) == (keep["out"].hit_count[:m].cpu().to(torch.int64) & 0xFFFFFFFF)).all()) \
+            if rotate == 1 else None
+    keep["ctx"].close()
+    del keep
+
+    # ---- the other configs, same protocol with fewer steps (rank 0 of a single-GPU run only) ----
+    if rank == 0 and world == 1 and args.per_config:
+        table = {}
+        for mode in [m for m in args.per_config_modes.split(",") if m]:
+            for ci in [int(x) for x in args.per_config.split(",") if x != ""]:
+                key = f"cfg{ci}_{mode}"
+                if ci == cfg.cfg_id and mode == args.cm_mode and not args.frames:
+                    r = dict(res)
+                else:
+                    torch.cuda.empty_cache()
+                    c2 = synth.CONFIGS[ci]
+                    rot = ROTATE_COPIES if c2.n_frames * c2.npix * 2 < (200 << 20) else 1
+                    try:
+                        r, k2 = time_config(binding, c2, mode, dev, 0, 5, 3, rotate=rot)
+                        k2["ctx"].close()
+                        del k2
+                    except Exception as exc:
+                        r = {"error": str(exc)[:200]}
+                for drop in ("generation_s", "warmup_steps_run", "launches_per_step"):
+                    r.pop(drop, None)
+                table[key] = r
+        line["config"]["per_config"] = table
     if rank == 0:
         print(json.dumps(line))
-    ctx.close()
     if dist:
         dist.destroy_process_group()
 

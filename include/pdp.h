@@ -165,6 +165,10 @@ int pdp_destroy(pdp_ctx *ctx);
  * pdp_process_host call on this context enqueued. */
 int pdp_last_launch_count(const pdp_ctx *ctx);
 
+/* Name of the kernel that did the dense pass of the last pdp_process / pdp_process_host call
+ * ("" before the first call).  Static string owned by the library; for benchmarks and profiles. */
+const char *pdp_last_kernel_name(const pdp_ctx *ctx);
+
 /* Debug/diagnostic: copy the per-segment common-mode estimates of the last
  * pdp_process call into `cm_device` (DEVICE float32,
  * [n_frames][P][H][W/seg_cols]).  Only valid when the context was told to keep

@@ -19,7 +19,7 @@ CM_MEDIAN, CM_MEAN_GUARDED, CM_NONE = 0, 1, 2
 STATUS_HIT_OVERFLOW = 1
 
 EXPORTS = ("pdp_create", "pdp_process", "pdp_process_host", "pdp_set_params", "pdp_destroy",
-           "pdp_last_launch_count", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
+           "pdp_last_launch_count", "pdp_last_kernel_name", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
            "pdp_last_error", "pdp_version")
 
 
@@ -72,6 +72,8 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.pdp_set_params.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_params)]
     lib.pdp_destroy.argtypes = [ctypes.c_void_p]
     lib.pdp_last_launch_count.argtypes = [ctypes.c_void_p]
+    lib.pdp_last_kernel_name.argtypes = [ctypes.c_void_p]
+    lib.pdp_last_kernel_name.restype = ctypes.c_char_p
     lib.pdp_keep_common_mode.argtypes = [ctypes.c_void_p, ctypes.c_int32]
     lib.pdp_get_common_mode.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p]
     lib.pdp_strerror.argtypes = [ctypes.c_int]
@@ -194,6 +196,10 @@ class Context:
     @property
     def last_launch_count(self) -> int:
         return int(self._lib.pdp_last_launch_count(self._h))
+
+    @property
+    def last_kernel_name(self) -> str:
+        return self._lib.pdp_last_kernel_name(self._h).decode()
 
     def close(self):
         if self._h:

@@ -69,6 +69,7 @@ struct pdp_ctx {
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   int launches = 0;
+  const char *last_kernel = "";   // name of the dominant kernel of the last call (pdp_last_kernel_name)
   std::string last_error;
 };
 
@@ -461,6 +462,8 @@ int pdp_destroy(pdp_ctx *ctx) {
 
 int pdp_last_launch_count(const pdp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
+const char *pdp_last_kernel_name(const pdp_ctx *ctx) { return ctx ? ctx->last_kernel : ""; }
+
 int pdp_keep_common_mode(pdp_ctx *ctx, int32_t enable) {
   if (!ctx) return fail(nullptr, PDP_E_NULL, "pdp_keep_common_mode: null ctx");
   ctx->keep_cm = enable ? 1 : 0;
@@ -590,6 +593,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);
       PDP_CUDA(c, cudaGetLastError());
       c->launches += 1;
+      c->last_kernel = "pdp_stream_kernel";
       return PDP_OK;
     }
   }
@@ -627,6 +631,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
     ff<<<grid_f, fpl.threads, fpl.smem, st>>>(f);
     PDP_CUDA(c, cudaGetLastError());
     c->launches += 1;
+    c->last_kernel = "pdp_frames_kernel";
     return PDP_OK;
   }
   PDP_CUDA(c, cudaMemsetAsync(c->d_lookback, 0, (size_t)n * pl.n_bands * sizeof(unsigned long long), st));
@@ -636,6 +641,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   fn<<<grid, pl.threads, pl.smem, st>>>(k);
   PDP_CUDA(c, cudaGetLastError());
   c->launches += 1;
+  c->last_kernel = "pdp_fused_kernel";
   return PDP_OK;
 }
 

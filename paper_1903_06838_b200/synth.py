@@ -148,29 +148,38 @@ def _phi(z: torch.Tensor) -> torch.Tensor:
     return 0.5 * (1.0 + torch.special.erf(z * (1.0 / math.sqrt(2.0))))
 
 
-def _signal(cfg: DetectorConfig, frame: int, device) -> torch.Tensor:
-    """Deposited photon charge of one frame, gain-corrected ADU, float64 [P, H, W]."""
+def _keys(cfg: DetectorConfig, purpose: int, frames, device) -> torch.Tensor:
+    """One key per frame as an int64 column [F, 1] (broadcasts against per-element counters)."""
+    return torch.tensor([_key(cfg, purpose, f) for f in frames], dtype=torch.int64, device=device).reshape(-1, 1)
+
+
+def _signal(cfg: DetectorConfig, frames, device) -> torch.Tensor:
+    """Deposited photon charge of the given frames, gain-corrected ADU, float64 [F, P*H*W]."""
     P, H, W = cfg.panels, cfg.rows, cfg.cols
+    F = len(frames)
     idx = torch.arange(cfg.npix, dtype=torch.int64, device=device)
-    key = _key(cfg, 3, frame)
-    k = _photon_counts(cfg, _uniform(key, idx, 0), _uniform(key, idx, 1))
-    sig = torch.zeros(cfg.npix, dtype=torch.float64, device=device)
-    pix = torch.nonzero(k > 0).flatten()
-    if pix.numel() == 0:
-        return sig.reshape(P, H, W)
-    reps = k[pix]
-    ph_pix = torch.repeat_interleave(pix, reps)
+    key = _keys(cfg, 3, frames, device)
+    k = _photon_counts(cfg, _uniform(key, idx, 0), _uniform(key, idx, 1))      # [F, npix]
+    sig = torch.zeros(F * cfg.npix, dtype=torch.float64, device=device)
+    hit = torch.nonzero(k.reshape(-1) > 0).flatten()            # flat (frame, pixel), frame-major
+    if hit.numel() == 0:
+        return sig.reshape(F, cfg.npix)
+    reps = k.reshape(-1)[hit]
+    ph = torch.repeat_interleave(hit, reps)
     # ordinal of the photon inside its pixel
     start = torch.cumsum(reps, 0) - reps
-    ordinal = torch.arange(ph_pix.numel(), device=device) - torch.repeat_interleave(start, reps)
+    ordinal = torch.arange(ph.numel(), device=device) - torch.repeat_interleave(start, reps)
+    ph_frame = ph // cfg.npix
+    ph_pix = ph - ph_frame * cfg.npix
     ctr = ph_pix * 16 + ordinal
-    pkey = _key(cfg, 4, frame)
+    pkey = _keys(cfg, 4, frames, device).flatten()[ph_frame]
     col = ph_pix % W
     row = (ph_pix // W) % H
     pan = ph_pix // (W * H)
     x0 = col.to(torch.float64) + _uniform(pkey, ctr, 0)   # pixel j covers [j, j+1)
     y0 = row.to(torch.float64) + _uniform(pkey, ctr, 1)
     s = cfg.cloud_sigma
+    base = ph_frame * cfg.npix
     for dr in range(-3, 4):
         rr = row + dr
         wy = _phi((rr.to(torch.float64) + 1.0 - y0) / s) - _phi((rr.to(torch.float64) - y0) / s)
@@ -179,33 +188,42 @@ def _signal(cfg: DetectorConfig, frame: int, device) -> torch.Tensor:
             cc = col + dc
             wx = _phi((cc.to(torch.float64) + 1.0 - x0) / s) - _phi((cc.to(torch.float64) - x0) / s)
             ok = okr & (cc >= 0) & (cc < W)          # charge falling off the panel is lost
-            tgt = (pan * H + rr) * W + cc
+            tgt = base + (pan * H + rr) * W + cc
             sig.index_put_((tgt[ok],), (cfg.photon_adu * wy * wx)[ok], accumulate=True)
-    return sig.reshape(P, H, W)
+    return sig.reshape(F, cfg.npix)
+
+
+def _make_block(cfg: DetectorConfig, frames, ped: torch.Tensor, gain: torch.Tensor) -> torch.Tensor:
+    """Raw frames `frames` (a list of frame numbers) as int32 values in [0, 65535]; shape [F, P, H, W]."""
+    device = ped.device
+    P, H, W, S = cfg.panels, cfg.rows, cfg.cols, cfg.seg_cols
+    F = len(frames)
+    idx = torch.arange(cfg.npix, dtype=torch.int64, device=device)
+    noise = cfg.noise_sigma * _normal(_keys(cfg, 1, frames, device), idx)          # [F, npix]
+    nseg = W // S
+    sidx = torch.arange(P * H * nseg, dtype=torch.int64, device=device)
+    cm = cfg.cm_sigma * _normal(_keys(cfg, 2, frames, device), sidx).reshape(F, P * H * nseg, 1)
+    s = (_signal(cfg, frames, device) + noise).reshape(F, P * H * nseg, S) + cm
+    raw = torch.round(ped.to(torch.float64).reshape(1, -1) + gain.to(torch.float64).reshape(1, -1) * s.reshape(F, -1))
+    return raw.clamp_(0.0, 65535.0).to(torch.int32).reshape(F, P, H, W)   # round: half-to-even
 
 
 def make_frame(cfg: DetectorConfig, frame: int, ped: torch.Tensor, gain: torch.Tensor) -> torch.Tensor:
     """One raw frame, uint16 stored as int32 tensor values in [0, 65535]; shape [P, H, W]."""
-    device = ped.device
-    P, H, W, S = cfg.panels, cfg.rows, cfg.cols, cfg.seg_cols
-    idx = torch.arange(cfg.npix, dtype=torch.int64, device=device)
-    noise = cfg.noise_sigma * _normal(_key(cfg, 1, frame), idx).reshape(P, H, W)
-    nseg = W // S
-    sidx = torch.arange(P * H * nseg, dtype=torch.int64, device=device)
-    cm = cfg.cm_sigma * _normal(_key(cfg, 2, frame), sidx).reshape(P, H, nseg)
-    cm = cm.repeat_interleave(S, dim=2)
-    s = _signal(cfg, frame, device) + cm + noise
-    raw = torch.round(ped.to(torch.float64) + gain.to(torch.float64) * s)   # half-to-even
-    return raw.clamp_(0.0, 65535.0).to(torch.int32)
+    return _make_block(cfg, [frame], ped, gain)[0]
 
 
 def make_frames(cfg: DetectorConfig, first: int, count: int, ped: torch.Tensor, gain: torch.Tensor,
-                out: torch.Tensor | None = None) -> torch.Tensor:
-    """raw[count, P, H, W] as torch.uint16 on ped.device (frames first .. first+count-1)."""
+                out: torch.Tensor | None = None, block_pixels: int = 1 << 25) -> torch.Tensor:
+    """raw[count, P, H, W] as torch.uint16 on ped.device (frames first .. first+count-1).  Frames are
+    generated in blocks of ~block_pixels pixels (every frame depends only on its own number, so the
+    block size never changes a value)."""
     if out is None:
         out = torch.empty((count, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=ped.device)
-    for i in range(count):
-        out[i].copy_(make_frame(cfg, first + i, ped, gain).to(torch.uint16))
+    B = max(1, block_pixels // cfg.npix)
+    for i in range(0, count, B):
+        m = min(B, count - i)
+        out[i:i + m].copy_(_make_block(cfg, list(range(first + i, first + i + m)), ped, gain).to(torch.uint16))
     return out
 
 

@@ -19,6 +19,7 @@ from paper_1903_06838_b200 import binding, build, synth  # noqa: E402
 
 build.build()
 DEV = "cuda"
+LAUNCHES_PER_CALL = 1      # kernels one pdp_process call enqueues
 
 
 def small(cfg_id, **kw):
@@ -232,34 +233,121 @@ def test_many_frames_auto_kernel(oracle, cm_mode):
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
 
 
-def test_full_size_config1_sampled(oracle):
-    """BASELINE.json configs[1] at full size (2000 frames of 704x768), in the launch configuration bench.py
-    times (one pdp_process call over the whole batch, auto kernel choice, capacity like the bench): sampled
-    frames - first, last, around CTA ownership boundaries (2000/148 = 13.5 frames per CTA) and chunk
-    boundaries - are compared hit by hit with the oracle; invariants that hold at any size cover the rest."""
-    cfg, n = small(1), 2000
+def _gpu_invariants(out, cfg, n):
+    """Any-size invariants over ALL frames, evaluated on the device (the lists of the big configs are GBs):
+    strictly increasing pixel lists, frame_photons == sum of listed n, accum == scatter of all lists."""
+    cap = out.hit_capacity
+    hc = out.hit_count.to(torch.int64) & 0xFFFFFFFF
+    assert int(hc.max()) <= cap and int(out.status.item()) == 0
+    for f0 in range(0, n, 64):                                  # blocks of frames bound the temporaries
+        f1 = min(n, f0 + 64)
+        k = torch.arange(cap, device=hc.device)[None, :] < hc[f0:f1, None]
+        px = out.hit_pixel[f0:f1].to(torch.int64) & 0xFFFFFFFF
+        assert bool(((px[:, 1:] > px[:, :-1]) | ~k[:, 1:]).all()), "lists not strictly increasing"
+        assert bool((px[k] < cfg.npix).all())
+        nph = torch.where(k, out.hit_nphot[f0:f1], 0).to(torch.int64)
+        assert torch.equal(nph.sum(1), out.frame_photons[f0:f1].to(torch.int64) & 0xFFFFFFFF)
+        if f0 == 0:
+            acc = torch.zeros(cfg.npix, dtype=torch.int64, device=hc.device)
+        acc.index_add_(0, px[k], nph[k])
+    assert torch.equal(acc, out.accum.to(torch.int64) & 0xFFFFFFFF), "accum != scatter of all lists"
+    return hc
+
+
+def _full_size_sampled(oracle, cfg_id, cm_mode, min_hits, *, host_chunk=None, extra_sample=()):
+    """One BASELINE.json config at FULL size in the launch configuration bench.py times (one pdp_process
+    call over all frames, auto kernel choice, capacity chosen like the bench does): frames sampled at the
+    start, the end and around CTA / chunk ownership boundaries are compared hit by hit with the oracle;
+    invariants that hold at any size cover every frame."""
+    cfg = synth.CONFIGS[cfg_id]
+    n = cfg.n_frames
     raw, ped, gain = make(cfg, n)
-    g = gpu_run(cfg, raw, ped, gain, 0, cap=1112)
-    assert g["status"][0] == 0 and g["launches"] == 1
-    sample = sorted({0, 1, 12, 13, 14, 15, 16, 27, 28, 999, 1000, 1013, 1014, 1986, 1987, 1998, 1999})
-    picked = raw.view(torch.int16)[torch.tensor(sample, device=raw.device)].view(torch.uint16)   # uint16 has no index kernel
-    o = oracle_run(oracle, cfg, picked, ped, gain, 0)
-    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu, frames=sample, check_accum=False)
-    print(rep.summary())
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
+                          max_frames_per_batch=n, pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu,
+                          cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm_mode)
+    probe = binding.alloc_output(8, cfg.npix, cfg.max_hits, DEV)
+    ctx.process(raw[:8], probe)
+    torch.cuda.synchronize()
+    cap = min(cfg.max_hits, max(256, 4 * int(probe.hit_count.max())))
+    del probe
+    out = binding.alloc_output(n, cfg.npix, cap, DEV)
+    if host_chunk:
+        try:
+            host = torch.empty(raw.shape, dtype=torch.uint16).pin_memory()
+        except RuntimeError:                                     # the box cannot pin the whole batch
+            host = torch.empty(raw.shape, dtype=torch.uint16)
+        host.copy_(raw)
+        ctx.process_host(host, out, host_chunk)
+    else:
+        ctx.process(raw, out)
+    torch.cuda.synchronize()
+    launches = ctx.last_launch_count
+    assert launches == (-(-n // host_chunk) if host_chunk else 1) * LAUNCHES_PER_CALL
+    hc = _gpu_invariants(out, cfg, n)
+    per_cta = n / 148.0
+    sample = {0, 1, n // 2, n - 2, n - 1}
+    for b in (1, 2, 74, 147):                                    # last/first frames of neighbouring CTAs
+        e = int(b * per_cta)
+        sample |= {max(0, e - 1), e, min(n - 1, e + 1)}
+    sample |= {15, 16, 17} if per_cta > 16 else set()            # chunk boundary inside a CTA's range
+    sample = sorted(x for x in sample | set(extra_sample) if 0 <= x < n)
+    assert len(sample) >= 12
+    idx = torch.tensor(sample, device=raw.device)
+    picked = raw.view(torch.int16)[idx].view(torch.uint16)       # uint16 has no index kernel
+    o = oracle_run(oracle, cfg, picked, ped, gain, cm_mode)
+    g = {k: getattr(out, k)[idx].cpu().numpy() for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot",
+                                                          "hit_dx", "hit_dy", "frame_photons")}
+    g["hit_count"] = g["hit_count"].astype(np.int64) & 0xFFFFFFFF
+    g["frame_photons"] = g["frame_photons"].astype(np.int64) & 0xFFFFFFFF
+    g["accum"] = np.zeros(1, np.int32)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu,
+                  check_accum=False)
+    print(cfg.name, "cm", cm_mode, "cap", cap, "hits/frame %.0f" % float(hc.double().mean()), rep.summary())
+    ctx.close()
     assert rep.ok, rep.failures[:10]
-    assert rep.hits_oracle > 3000 and rep.exempt_hits <= 3
-    # any-size invariants over ALL frames
-    hc = g["hit_count"]
-    assert hc.min() > 100 and hc.max() < 1112
-    k = np.arange(g["hit_pixel"].shape[1])[None, :] < hc[:, None]
-    px = g["hit_pixel"].astype(np.int64) & 0xFFFFFFFF
-    inc = (np.diff(px, axis=1) > 0) | ~k[:, 1:]
-    assert inc.all()                                                       # strictly increasing lists
-    nph = np.where(k, g["hit_nphot"], 0).astype(np.int64)
-    assert np.array_equal(nph.sum(1), g["frame_photons"])                   # totals = sum of listed n
-    acc = np.zeros(cfg.npix, np.int64)
-    np.add.at(acc, px[k], nph[k])
-    assert np.array_equal(acc, g["accum"].astype(np.int64) & 0xFFFFFFFF)    # accum = scatter of all lists
+    assert rep.hits_oracle > min_hits and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
+
+
+def test_full_size_config1_sampled(oracle):
+    """configs[1]: 2000 frames of 704x768 (13.5 frames per CTA)."""
+    _full_size_sampled(oracle, 1, 0, 3000)
+
+
+def test_full_size_config2_sampled(oracle):
+    """configs[2]: 500 frames of 32 panels x 185x388 (S = 194: 4-byte vectors, frames only 8-byte aligned,
+    3.4 frames per CTA, panel edges every 185 rows)."""
+    _full_size_sampled(oracle, 2, 0, 30000)
+
+
+def test_full_size_config3_sampled(oracle):
+    """configs[3]: 500 frames of 1024x1024 at 10 % occupancy (42 k hits per frame: the sparse stage and the
+    ordered emission under real load)."""
+    _full_size_sampled(oracle, 3, 0, 400000)
+
+
+@pytest.mark.parametrize("host", [False, True], ids=["device", "streamed"])
+def test_full_size_config4_sampled(oracle, host):
+    """configs[4]: 4000 frames of 16 panels x 512x512 (33.5 GB, 27 frames per CTA: multi-chunk path), device
+    resident and streamed from (pinned) host memory in 64-frame chunks through the double-buffered side stream."""
+    _full_size_sampled(oracle, 4, 0, 150000, host_chunk=64 if host else None)
+
+
+@pytest.mark.parametrize("n", [148 * 6 + 3, 148 * 17, 148 * 20, 148 * 24 + 5, 148 * 33],
+                         ids=["6perCTA", "17perCTA", "20perCTA", "24perCTA", "33perCTA"])
+def test_frames_per_cta_paths(oracle, n):
+    """Every frame against the oracle on a small, DENSE geometry with 6 ... 33 frames per CTA: partial
+    frame groups, a second and third chunk of frame slots per CTA (ring reuse, barrier phase carry-over),
+    a short last chunk (slot ownership must not change between chunks), with the sparse
+    stage as the bottleneck (5 % of the pixels are photon centres)."""
+    cfg = small(0, panels=2, rows=21, cols=128, seg_cols=64, occupancy=0.05)
+    raw, ped, gain = make(cfg, n)
+    for cm_mode in (0, 1):
+        g = gpu_run(cfg, raw, ped, gain, cm_mode)
+        o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+        rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
+        print(n, cm_mode, rep.summary())
+        assert rep.ok, rep.failures[:10]
+        assert rep.hits_oracle > 100 * n and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
 
 
 def test_full_size_config0(oracle):
