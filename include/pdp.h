@@ -85,7 +85,9 @@ typedef struct pdp_params {
 } pdp_params;
 
 /* One batch of raw frames: DEVICE pointer, contiguous [n_frames][P][H][W]
- * uint16, 16-byte aligned.  Caller-owned; only read. */
+ * uint16, 16-byte aligned (rows are moved with 16-byte asynchronous copies; any cudaMalloc'ed or torch
+ * buffer is; a misaligned pointer returns PDP_E_ALIGN instead of taking a slow path silently).
+ * Caller-owned; only read. */
 typedef struct pdp_batch {
   const uint16_t *data;
   int32_t n_frames;
@@ -118,9 +120,11 @@ typedef struct pdp_output {
  *   pedestal_host, gain_host : HOST float32 arrays of P*H*W elements (copied to
  *     the device; the context keeps derived maps, not the host pointers).
  *   out_ctx : receives the context.
- * Errors: PDP_E_NULL, PDP_E_GEOMETRY (also: cols or seg_cols odd, seg_cols > 1024,
- * more than 6 segments per row), PDP_E_VALUE (checked over every map element),
- * PDP_E_NO_SM100, PDP_E_CUDA, PDP_E_NOMEM.  On error *out_ctx is set to NULL.
+ * Geometry limits (all return PDP_E_GEOMETRY): cols and seg_cols even (pixels are moved in pairs or wider),
+ * seg_cols <= 1024, at most 6 segments per row, panels*rows*cols < 2^32.  Any such geometry runs; 16-byte
+ * vectors need cols and seg_cols to be multiples of 8, otherwise 8- or 4-byte ones are used.
+ * Errors: PDP_E_NULL, PDP_E_GEOMETRY, PDP_E_VALUE (checked over every map element: finite, gain != 0,
+ * |pedestal| <= 4e6), PDP_E_NO_SM100, PDP_E_CUDA, PDP_E_NOMEM.  On error *out_ctx is set to NULL.
  */
 int pdp_create(const pdp_geometry *geometry, const float *pedestal_host, const float *gain_host,
                const pdp_params *params, pdp_ctx **out_ctx);
@@ -141,16 +145,22 @@ int pdp_process(pdp_ctx *ctx, const pdp_batch *raw_u16_batch, void *cuda_stream,
                 const pdp_output *out);
 
 /*
- * pdp_process_host — the same chain fed from HOST memory (pinned for real
- * overlap): the n_frames frames at `raw_host` are copied to the device in
- * chunks of `chunk_frames` on an internal copy stream into two device buffers
- * owned by the context (allocated on first use, sized chunk_frames), and each
- * chunk is processed on `cuda_stream` while the next one is in flight
+ * pdp_process_pinned — the same chain fed from HOST memory (pinned for real
+ * overlap): the n_frames frames at `pinned_host` are copied to the device in
+ * chunks of `chunk_frames` on `copy_stream` (a cudaStream_t as void*; NULL =
+ * a side stream owned by the context) into two device buffers owned by the
+ * context (allocated on first use, sized chunk_frames), and each chunk is
+ * processed on `compute_stream` while the next one is in flight
  * (BASELINE.json config 4 "streamed from pinned host memory with
- * double-buffered copies on a side stream").  `out` buffers are DEVICE
- * pointers sized for all n_frames; chunk_frames <= max_frames_per_batch.
- * Returns after everything has been enqueued; synchronise `cuda_stream`.
+ * double-buffered copies on a side stream"; "similar to real time
+ * DAQ").  `out` buffers are DEVICE pointers sized for all n_frames;
+ * chunk_frames <= max_frames_per_batch.  Returns after everything has been
+ * enqueued; synchronise `compute_stream`.  Errors as pdp_process.
+ *
+ * pdp_process_host — the same with the context's own copy stream.
  */
+int pdp_process_pinned(pdp_ctx *ctx, const uint16_t *pinned_host, int32_t n_frames, int32_t chunk_frames,
+                       void *compute_stream, void *copy_stream, const pdp_output *out);
 int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
                      int32_t chunk_frames, void *cuda_stream, const pdp_output *out);
 
@@ -162,12 +172,28 @@ int pdp_set_params(pdp_ctx *ctx, const pdp_params *params);
 int pdp_destroy(pdp_ctx *ctx);
 
 /* Number of kernel launches (ours, not memsets/copies) the last pdp_process /
- * pdp_process_host call on this context enqueued. */
+ * pdp_process_pinned call on this context enqueued: 2 per batch on the throughput path (the chain
+ * kernel and the accumulated-image pass), 1 on the small-batch path. */
 int pdp_last_launch_count(const pdp_ctx *ctx);
 
 /* Name of the kernel that did the dense pass of the last pdp_process / pdp_process_host call
  * ("" before the first call).  Static string owned by the library; for benchmarks and profiles. */
 const char *pdp_last_kernel_name(const pdp_ctx *ctx);
+
+/*
+ * pdp_debug_set — diagnostic switches for tests and profiling (never needed for normal use; the library reads
+ * no environment variables).  Keys:
+ *   "kernel"        0 automatic (default), 1 the small-batch kernel (band x chunk items, decoupled look-back),
+ *                   2 the throughput kernel (frame-owner CTAs); PDP_E_GEOMETRY at the next pdp_process if the
+ *                   geometry does not fit it;
+ *   "chunk_frames"  frames per work item of the small-batch kernel (0 = automatic);
+ *   "sparse_warps"  0 automatic (from the hit density of earlier calls), 4 or 8: warps of the throughput
+ *                   kernel that evaluate seed candidates;
+ *   "variant"       V*10000 + NV*100 + LPS: pin the throughput kernel's layout (pixels per vector, vectors per
+ *                   lane, lanes per row segment), 0 = automatic; PDP_E_GEOMETRY if it does not cover seg_cols.
+ * None of them changes any output.  Errors: PDP_E_NULL, PDP_E_VALUE (unknown key / value).
+ */
+int pdp_debug_set(pdp_ctx *ctx, const char *key, int64_t value);
 
 /* Debug/diagnostic: copy the per-segment common-mode estimates of the last
  * pdp_process call into `cm_device` (DEVICE float32,

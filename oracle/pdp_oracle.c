@@ -28,6 +28,9 @@
  *                                                         PAPER.md:L89, L95
  *   O9  hit list ordered by pixel index
  *   O10 frame_photons = sum n ; accum[idx] += n
+ *   O11 histograms of the summarization (E spectrum, dx/dy)
+ *   O12 dense photon counting round(v2/E_ph) per pixel
+ *   O3' stacked common-mode stages on other group shapes
  *   OF  fragile flags: which decisions sit within `band` ADU of a threshold
  *       (BASELINE.json: "pixels whose fp64 value lies within 1e-4 ADU of a
  *       threshold; these are counted and reported")
@@ -60,10 +63,26 @@ typedef struct {
   int32_t panels, rows, cols, seg_cols;
 } oracle_geometry;
 
+/* One common-mode stage ("other types of common mode (row, column, block) can be easily
+ * extracted by reshaping tensors accordingly"; L117 "3 stacked common mode stages"): the panel is tiled by
+ * groups of gh rows x gw columns (row segment: 1 x S, column segment: S x 1, block: bh x bw, frame-wise on
+ * a panel: H x W; gh | H and gw | W), every group gets its own estimate with the stage's estimator, and the
+ * stages are applied one after the other, each on the output of the previous one. */
+typedef struct {
+  int32_t gh, gw;        /* group shape */
+  int32_t mode;          /* ORACLE_CM_* */
+  int32_t min_count;     /* MEDIAN: c = 0 below this count; 0 -> ceil(sqrt(gh*gw)) */
+} oracle_cm_stage;
+
+#define ORACLE_MAX_STAGES 3
+
 typedef struct {
   double seed_adu, cm_adu, photon_adu;
   int32_t cm_mode, cm_min_count; /* cm_min_count 0 -> ceil(sqrt(seg_cols)) */
   double band;                   /* fragile band in ADU (1e-4) */
+  int32_t n_stages;              /* 0: ONE stage of 1 x seg_cols groups with cm_mode / cm_min_count (the hot path) */
+  oracle_cm_stage stage[ORACLE_MAX_STAGES];
+  double zero_below_adu;         /* dense photon counting only: pixels with v2 below it count 0 */
 } oracle_params;
 
 static int cmp_double(const void *a, const void *b) {
@@ -72,8 +91,8 @@ static int cmp_double(const void *a, const void *b) {
 }
 
 /* O3: common-mode estimate of one group of S values. */
-static double common_mode(const double *v1, int S, const oracle_params *prm, double *scratch,
-                          int *fragile_mask, int *count_out) {
+static double common_mode(const double *v1, int S, const oracle_params *prm, int mode, int min_count_in,
+                          double *scratch, int *fragile_mask, int *count_out) {
   int k = 0;
   double sum = 0.0;
   *fragile_mask = 0;
@@ -86,21 +105,77 @@ static double common_mode(const double *v1, int S, const oracle_params *prm, dou
     }
   }
   *count_out = k; /* "number of segmented pixels"; reported, not used below */
-  if (prm->cm_mode == ORACLE_CM_NONE) {
+  if (mode == ORACLE_CM_NONE) {
     *fragile_mask = 0;
     return 0.0;
   }
-  if (prm->cm_mode == ORACLE_CM_MEAN_GUARDED) {
+  if (mode == ORACLE_CM_MEAN_GUARDED) {
     double guard = sqrt((double)S);
     double denom = (double)k > guard ? (double)k : guard;
     return sum / denom;
   }
   /* MEDIAN */
-  int min_count = prm->cm_min_count > 0 ? prm->cm_min_count : (int)ceil(sqrt((double)S));
+  int min_count = min_count_in > 0 ? min_count_in : (int)ceil(sqrt((double)S));
   if (k < min_count || k == 0) return 0.0;
   qsort(scratch, (size_t)k, sizeof(double), cmp_double);
   if (k & 1) return scratch[(k - 1) / 2];
   return 0.5 * (scratch[k / 2 - 1] + scratch[k / 2]);
+}
+
+/*
+ * O1-O4 for one frame: v2[Npix] = ((raw - dark) / gain) with the common-mode stage(s) subtracted.
+ * frag (Npix, may be NULL) gets FRAGILE_F1 on every pixel of a group whose mask is within band of
+ * flipping (any stage); cm_out / cm_count_out (may be NULL) receive the estimate and the number of
+ * segmented pixels of every group of the LAST stage, in (panel, group row, group column) order.
+ */
+static int calibrate_and_common_mode(const oracle_geometry *g, const float *pedestal, const float *gain,
+                                     const oracle_params *prm, const uint16_t *raw, double *v2,
+                                     uint8_t *frag, double *cm_out, int32_t *cm_count_out) {
+  const int P = g->panels, H = g->rows, W = g->cols;
+  const int64_t npix = (int64_t)P * H * W;
+  /* O1, O2 */
+  for (int64_t i = 0; i < npix; ++i) {
+    double d = (double)raw[i] - (double)pedestal[i];
+    v2[i] = d / (double)gain[i];
+  }
+  /* O3, O4: stage by stage, each on the output of the previous one */
+  oracle_cm_stage one = {1, g->seg_cols, prm->cm_mode, prm->cm_min_count};
+  const int n_stages = prm->n_stages > 0 ? prm->n_stages : 1;
+  for (int st = 0; st < n_stages; ++st) {
+    const oracle_cm_stage *sg = prm->n_stages > 0 ? &prm->stage[st] : &one;
+    const int gh = sg->gh, gw = sg->gw, G = gh * gw;
+    if (gh < 1 || gw < 1 || H % gh || W % gw) return -1;
+    double *vals = (double *)malloc((size_t)G * sizeof(double));
+    double *scratch = (double *)malloc((size_t)G * sizeof(double));
+    if (!vals || !scratch) {
+      free(vals);
+      free(scratch);
+      return -1;
+    }
+    const int ngr = H / gh, ngc = W / gw;
+    const int last = st == n_stages - 1;
+    for (int p = 0; p < P; ++p)
+      for (int br = 0; br < ngr; ++br)
+        for (int bc = 0; bc < ngc; ++bc) {
+          int k = 0;
+          for (int r = 0; r < gh; ++r)
+            for (int c = 0; c < gw; ++c)
+              vals[k++] = v2[((int64_t)p * H + br * gh + r) * W + bc * gw + c];
+          int fmask, cnt;
+          double cm = common_mode(vals, G, prm, sg->mode, sg->min_count, scratch, &fmask, &cnt);
+          if (last && cm_out) cm_out[((int64_t)p * ngr + br) * ngc + bc] = cm;
+          if (last && cm_count_out) cm_count_out[((int64_t)p * ngr + br) * ngc + bc] = cnt;
+          for (int r = 0; r < gh; ++r)
+            for (int c = 0; c < gw; ++c) {
+              int64_t i = ((int64_t)p * H + br * gh + r) * W + bc * gw + c;
+              v2[i] -= cm; /* "subtracted from the input signal": from ALL pixels of the group */
+              if (fmask && frag) frag[i] |= FRAGILE_F1;
+            }
+        }
+    free(vals);
+    free(scratch);
+  }
+  return 0;
 }
 
 /*
@@ -117,37 +192,20 @@ int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const 
                          double *cm_out, int32_t *cm_count_out, uint8_t *fragile_out, int64_t hit_capacity,
                          uint32_t *hit_pixel, double *hit_charge, int32_t *hit_nphot,
                          double *hit_dx, double *hit_dy, uint64_t *photons_out, uint32_t *accum) {
-  const int P = g->panels, H = g->rows, W = g->cols, S = g->seg_cols;
+  const int P = g->panels, H = g->rows, W = g->cols;
   const int64_t npix = (int64_t)P * H * W;
   double *v2 = (double *)malloc((size_t)npix * sizeof(double));
-  double *scratch = (double *)malloc((size_t)S * sizeof(double));
   uint8_t *frag = (uint8_t *)calloc((size_t)npix, 1);
-  if (!v2 || !scratch || !frag) {
+  if (!v2 || !frag) {
     free(v2);
-    free(scratch);
     free(frag);
     return -1;
   }
-  /* O1, O2 */
-  for (int64_t i = 0; i < npix; ++i) {
-    double d = (double)raw[i] - (double)pedestal[i];
-    v2[i] = d / (double)gain[i];
+  if (calibrate_and_common_mode(g, pedestal, gain, prm, raw, v2, frag, cm_out, cm_count_out) != 0) {
+    free(v2);
+    free(frag);
+    return -1;
   }
-  /* O3, O4 */
-  const int nseg = W / S;
-  for (int p = 0; p < P; ++p)
-    for (int r = 0; r < H; ++r)
-      for (int s = 0; s < nseg; ++s) {
-        int64_t base = ((int64_t)p * H + r) * W + (int64_t)s * S;
-        int fmask, k;
-        double c = common_mode(v2 + base, S, prm, scratch, &fmask, &k);
-        if (cm_out) cm_out[((int64_t)p * H + r) * nseg + s] = c;
-        if (cm_count_out) cm_count_out[((int64_t)p * H + r) * nseg + s] = k;
-        for (int j = 0; j < S; ++j) {
-          v2[base + j] -= c;
-          if (fmask) frag[base + j] |= FRAGILE_F1;
-        }
-      }
   /* O5..O10 */
   int64_t count = 0;
   uint64_t photons = 0;
@@ -206,7 +264,6 @@ int64_t pdp_oracle_frame(const oracle_geometry *g, const float *pedestal, const 
   if (v2_out) memcpy(v2_out, v2, (size_t)npix * sizeof(double));
   if (fragile_out) memcpy(fragile_out, frag, (size_t)npix);
   free(v2);
-  free(scratch);
   free(frag);
   return count;
 }
@@ -228,7 +285,9 @@ int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const floa
                      double *hit_dy, uint64_t *frame_photons, uint32_t *accum, double *cm_out,
                      int32_t *cm_count_out, uint8_t *fragile_out) {
   const int64_t npix = (int64_t)g->panels * g->rows * g->cols;
-  const int64_t nsegs = npix / g->seg_cols;
+  const int64_t nsegs = prm->n_stages > 0
+                            ? npix / ((int64_t)prm->stage[prm->n_stages - 1].gh * prm->stage[prm->n_stages - 1].gw)
+                            : npix / g->seg_cols; /* groups of the last stage */
   int failed = 0;
   if (threads < 1) threads = 1;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(threads)
@@ -248,4 +307,65 @@ int pdp_oracle_batch(const oracle_geometry *g, const float *pedestal, const floa
     frame_photons[f] = ph;
   }
   return failed ? -1 : 0;
+}
+
+/*
+ * O11  Histogram summarization ("functions for histogramming"; L109 Fig. 7: spectrum of the summed
+ * charge; L113 Fig. 8: histogram of the centroids): bin b = floor((x - lo) / width) counts x when 0 <= b < nbins
+ * (uniform bins [lo + b*width, lo + (b+1)*width), values outside are dropped).  hist[nbins] += counts.
+ */
+void pdp_oracle_histogram(const double *x, int64_t n, double lo, double width, int32_t nbins,
+                          uint64_t *hist) {
+  for (int64_t i = 0; i < n; ++i) {
+    double b = floor((x[i] - lo) / width);
+    if (b >= 0.0 && b < (double)nbins) hist[(int64_t)b] += 1;
+  }
+}
+
+/*
+ * O12  Dense photon counting for areas of high flux ("division with the expected single photon
+ * gain followed by rounding to the nearest integer"), on v2 (after dark, gain and common mode):
+ *   n_px = max(0, rint(v2 / E_ph))  (half-to-even), and n_px = 0 where v2 < zero_below_adu (PAPER.md:L91
+ *   "zeroing the signal of pixels within noise"; zero_below_adu = -infinity switches it off).
+ * image[Npix] += n_px over the frames (the photon-counting image of PAPER.md:L99), totals[f] = sum over the
+ * frame.  fragile_out (optional, [n_frames][Npix]) flags pixels whose v2/E_ph is within band of a rounding
+ * boundary or whose v2 is within band of zero_below_adu (FRAGILE_F4), and groups with a fragile mask (F1).
+ * Returns 0, -1 on allocation failure or an invalid stage.
+ */
+int pdp_oracle_dense_batch(const oracle_geometry *g, const float *pedestal, const float *gain,
+                           const oracle_params *prm, const uint16_t *raw, int32_t n_frames,
+                           uint32_t *image, uint64_t *totals, uint8_t *fragile_out) {
+  const int64_t npix = (int64_t)g->panels * g->rows * g->cols;
+  double *v2 = (double *)malloc((size_t)npix * sizeof(double));
+  uint8_t *frag = (uint8_t *)malloc((size_t)npix);
+  if (!v2 || !frag) {
+    free(v2);
+    free(frag);
+    return -1;
+  }
+  for (int32_t f = 0; f < n_frames; ++f) {
+    memset(frag, 0, (size_t)npix);
+    if (calibrate_and_common_mode(g, pedestal, gain, prm, raw + (int64_t)f * npix, v2, frag, NULL, NULL) != 0) {
+      free(v2);
+      free(frag);
+      return -1;
+    }
+    uint64_t tot = 0;
+    for (int64_t i = 0; i < npix; ++i) {
+      double x = v2[i];
+      double ratio = x / prm->photon_adu;
+      if (fabs(ratio - (floor(ratio) + 0.5)) * prm->photon_adu < prm->band) frag[i] |= FRAGILE_F4;
+      if (fabs(x - prm->zero_below_adu) < prm->band) frag[i] |= FRAGILE_F4;
+      double rn = nearbyint(ratio);
+      uint32_t n = 0;
+      if (!(x < prm->zero_below_adu) && rn > 0.0) n = rn > 4294967295.0 ? 4294967295u : (uint32_t)rn;
+      image[i] += n;
+      tot += n;
+    }
+    if (totals) totals[f] = tot;
+    if (fragile_out) memcpy(fragile_out + (int64_t)f * npix, frag, (size_t)npix);
+  }
+  free(v2);
+  free(frag);
+  return 0;
 }

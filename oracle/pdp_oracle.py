@@ -27,10 +27,34 @@ class _Geometry(ctypes.Structure):
                 ("cols", ctypes.c_int32), ("seg_cols", ctypes.c_int32)]
 
 
+class _Stage(ctypes.Structure):
+    _fields_ = [("gh", ctypes.c_int32), ("gw", ctypes.c_int32), ("mode", ctypes.c_int32),
+                ("min_count", ctypes.c_int32)]
+
+
 class _Params(ctypes.Structure):
     _fields_ = [("seed_adu", ctypes.c_double), ("cm_adu", ctypes.c_double),
                 ("photon_adu", ctypes.c_double), ("cm_mode", ctypes.c_int32),
-                ("cm_min_count", ctypes.c_int32), ("band", ctypes.c_double)]
+                ("cm_min_count", ctypes.c_int32), ("band", ctypes.c_double),
+                ("n_stages", ctypes.c_int32), ("stage", _Stage * 3), ("zero_below_adu", ctypes.c_double)]
+
+
+def _params(seed_adu, cm_adu, photon_adu, cm_mode, cm_min_count, band, stages=None, zero_below_adu=-np.inf):
+    """thresholds reach the library as float32; the oracle promotes those to double.
+    stages: optional list of up to 3 (gh, gw, mode[, min_count]) common-mode stages."""
+    p = _Params(float(np.float32(seed_adu)), float(np.float32(cm_adu)), float(np.float32(photon_adu)),
+                cm_mode, cm_min_count, band)
+    stages = list(stages or [])
+    assert len(stages) <= 3
+    p.n_stages = len(stages)
+    for i, st in enumerate(stages):
+        p.stage[i] = _Stage(int(st[0]), int(st[1]), int(st[2]), int(st[3]) if len(st) > 3 else 0)
+    p.zero_below_adu = float(np.float32(zero_below_adu)) if np.isfinite(zero_below_adu) else float(zero_below_adu)
+    return p
+
+
+def _n_groups(npix, seg_cols, stages):
+    return npix // (stages[-1][0] * stages[-1][1]) if stages else npix // seg_cols
 
 
 def build(force: bool = False) -> str:
@@ -50,6 +74,8 @@ def _load():
         _lib = ctypes.CDLL(build())
         _lib.pdp_oracle_frame.restype = ctypes.c_int64
         _lib.pdp_oracle_batch.restype = ctypes.c_int
+        _lib.pdp_oracle_dense_batch.restype = ctypes.c_int
+        _lib.pdp_oracle_histogram.restype = None
     return _lib
 
 
@@ -79,8 +105,8 @@ def max_hits(panels: int, rows: int, cols: int) -> int:
 
 def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_adu, photon_adu,
             cm_mode=CM_MEDIAN, cm_min_count=0, band=1e-4, threads=1, hit_capacity=None,
-            want_cm=False, want_fragile=False) -> OracleResult:
-    """Run the oracle over raw[n, panels*rows*cols] (uint16)."""
+            want_cm=False, want_fragile=False, stages=None) -> OracleResult:
+    """Run the oracle over raw[n, panels*rows*cols] (uint16).  stages: see _params."""
     lib = _load()
     npix = panels * rows * cols
     raw = np.ascontiguousarray(raw, dtype=np.uint16).reshape(-1, npix)
@@ -90,9 +116,8 @@ def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_a
     assert cols % seg_cols == 0
     cap = int(hit_capacity) if hit_capacity is not None else max_hits(panels, rows, cols)
     g = _Geometry(panels, rows, cols, seg_cols)
-    # thresholds reach the library as float32; the oracle promotes those to double
-    p = _Params(float(np.float32(seed_adu)), float(np.float32(cm_adu)),
-                float(np.float32(photon_adu)), cm_mode, cm_min_count, band)
+    p = _params(seed_adu, cm_adu, photon_adu, cm_mode, cm_min_count, band, stages)
+    ngr = _n_groups(npix, seg_cols, stages)
     hit_count = np.zeros(n, np.int64)
     hp = np.zeros((n, cap), np.uint32)
     he = np.zeros((n, cap), np.float64)
@@ -101,9 +126,9 @@ def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_a
     hy = np.zeros((n, cap), np.float64)
     fp = np.zeros(n, np.uint64)
     accum = np.zeros(npix, np.uint32)
-    cm = np.zeros((n, npix // seg_cols), np.float64) if want_cm else None
+    cm = np.zeros((n, ngr), np.float64) if want_cm else None
     frag = np.zeros((n, npix), np.uint8) if want_fragile else None
-    cmn = np.zeros((n, npix // seg_cols), np.int32) if (want_cm or want_fragile) else None
+    cmn = np.zeros((n, ngr), np.int32) if (want_cm or want_fragile) else None
     rc = lib.pdp_oracle_batch(
         ctypes.byref(g), _ptr(pedestal, ctypes.c_float), _ptr(gain, ctypes.c_float),
         ctypes.byref(p), _ptr(raw, ctypes.c_uint16), ctypes.c_int32(n), ctypes.c_int32(threads),
@@ -125,18 +150,17 @@ def process(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_a
 
 
 def frame_v2(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_adu, photon_adu,
-             cm_mode=CM_MEDIAN, cm_min_count=0, band=1e-4):
-    """v2 (after dark, gain, common mode) and the per-segment c of ONE frame, fp64."""
+             cm_mode=CM_MEDIAN, cm_min_count=0, band=1e-4, stages=None):
+    """v2 (after dark, gain, common mode) and the per-group c (last stage) of ONE frame, fp64."""
     lib = _load()
     npix = panels * rows * cols
     raw = np.ascontiguousarray(raw, dtype=np.uint16).reshape(npix)
     pedestal = np.ascontiguousarray(pedestal, dtype=np.float32).reshape(npix)
     gain = np.ascontiguousarray(gain, dtype=np.float32).reshape(npix)
     g = _Geometry(panels, rows, cols, seg_cols)
-    p = _Params(float(np.float32(seed_adu)), float(np.float32(cm_adu)),
-                float(np.float32(photon_adu)), cm_mode, cm_min_count, band)
+    p = _params(seed_adu, cm_adu, photon_adu, cm_mode, cm_min_count, band, stages)
     v2 = np.zeros(npix, np.float64)
-    cm = np.zeros(npix // seg_cols, np.float64)
+    cm = np.zeros(_n_groups(npix, seg_cols, stages), np.float64)
     ph = ctypes.c_uint64(0)
     cnt = lib.pdp_oracle_frame(
         ctypes.byref(g), _ptr(pedestal, ctypes.c_float), _ptr(gain, ctypes.c_float),
@@ -145,4 +169,39 @@ def frame_v2(raw, pedestal, gain, *, panels, rows, cols, seg_cols, seed_adu, cm_
         ctypes.byref(ph), None)
     if cnt < 0:
         raise MemoryError("pdp_oracle_frame failed")
+    if stages:
+        return v2.reshape(panels, rows, cols), cm.reshape(panels, rows // stages[-1][0], cols // stages[-1][1])
     return v2.reshape(panels, rows, cols), cm.reshape(panels, rows, cols // seg_cols)
+
+
+def histogram(values, lo, width, nbins, hist=None):
+    """O11: uniform-bin histogram of `values` (float64), out-of-range dropped; hist (uint64[nbins]) += counts."""
+    lib = _load()
+    x = np.ascontiguousarray(values, dtype=np.float64).reshape(-1)
+    if hist is None:
+        hist = np.zeros(nbins, np.uint64)
+    lib.pdp_oracle_histogram(_ptr(x, ctypes.c_double), ctypes.c_int64(x.size), ctypes.c_double(float(np.float32(lo))),
+                             ctypes.c_double(float(np.float32(width))), ctypes.c_int32(nbins), _ptr(hist, ctypes.c_uint64))
+    return hist
+
+
+def dense(raw, pedestal, gain, *, panels, rows, cols, seg_cols, cm_adu, photon_adu, cm_mode=CM_MEDIAN,
+          cm_min_count=0, band=1e-4, stages=None, zero_below_adu=-np.inf, want_fragile=False):
+    """O12: dense photon-counting image (uint32[npix], summed over the frames), per-frame totals, fragile flags."""
+    lib = _load()
+    npix = panels * rows * cols
+    raw = np.ascontiguousarray(raw, dtype=np.uint16).reshape(-1, npix)
+    n = raw.shape[0]
+    pedestal = np.ascontiguousarray(pedestal, dtype=np.float32).reshape(npix)
+    gain = np.ascontiguousarray(gain, dtype=np.float32).reshape(npix)
+    g = _Geometry(panels, rows, cols, seg_cols)
+    p = _params(0.0, cm_adu, photon_adu, cm_mode, cm_min_count, band, stages, zero_below_adu)
+    image = np.zeros(npix, np.uint32)
+    totals = np.zeros(n, np.uint64)
+    frag = np.zeros((n, npix), np.uint8) if want_fragile else None
+    rc = lib.pdp_oracle_dense_batch(ctypes.byref(g), _ptr(pedestal, ctypes.c_float), _ptr(gain, ctypes.c_float),
+                                    ctypes.byref(p), _ptr(raw, ctypes.c_uint16), ctypes.c_int32(n),
+                                    _ptr(image, ctypes.c_uint32), _ptr(totals, ctypes.c_uint64), _ptr(frag, ctypes.c_uint8))
+    if rc != 0:
+        raise ValueError("pdp_oracle_dense_batch failed (allocation, or a stage that does not tile the panel)")
+    return image, totals, frag

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpdp.so")
 CM_MEDIAN, CM_MEAN_GUARDED, CM_NONE = 0, 1, 2
 STATUS_HIT_OVERFLOW = 1
 
-EXPORTS = ("pdp_create", "pdp_process", "pdp_process_host", "pdp_set_params", "pdp_destroy",
+EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_set_params", "pdp_destroy",
            "pdp_last_launch_count", "pdp_last_kernel_name", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
            "pdp_last_error", "pdp_version")
 
@@ -69,6 +69,9 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
                                 ctypes.POINTER(pdp_output)]
     lib.pdp_process_host.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
                                      ctypes.c_void_p, ctypes.POINTER(pdp_output)]
+    lib.pdp_process_pinned.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(pdp_output)]
+    lib.pdp_debug_set.argtypes = [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]
     lib.pdp_set_params.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_params)]
     lib.pdp_destroy.argtypes = [ctypes.c_void_p]
     lib.pdp_last_launch_count.argtypes = [ctypes.c_void_p]
@@ -172,15 +175,21 @@ class Context:
                     "pdp_process")
 
     def process_host(self, raw_host: torch.Tensor, out: Output, chunk_frames: int,
-                     stream: torch.cuda.Stream | None = None):
-        """raw_host: CPU (pinned) 16-bit tensor [n, P, H, W]; chunks are copied on a side stream."""
+                     stream: torch.cuda.Stream | None = None, copy_stream: torch.cuda.Stream | None = None):
+        """raw_host: CPU (pinned) 16-bit tensor [n, P, H, W]; chunks are copied on `copy_stream` (default: the
+        context's own side stream) while `stream` computes (pdp_process_pinned)."""
         if raw_host.is_cuda or not raw_host.is_contiguous() or raw_host.element_size() != 2:
             raise ValueError("raw_host must be a contiguous CPU tensor of 16-bit elements")
         n = raw_host.numel() // self.npix
         s = stream if stream is not None else torch.cuda.current_stream()
         o = out.c_struct()
-        self._check(self._lib.pdp_process_host(self._h, raw_host.data_ptr(), n, chunk_frames,
-                                               ctypes.c_void_p(s.cuda_stream), ctypes.byref(o)), "pdp_process_host")
+        cs = ctypes.c_void_p(copy_stream.cuda_stream) if copy_stream is not None else None
+        self._check(self._lib.pdp_process_pinned(self._h, raw_host.data_ptr(), n, chunk_frames,
+                                                 ctypes.c_void_p(s.cuda_stream), cs, ctypes.byref(o)), "pdp_process_pinned")
+
+    def debug_set(self, key: str, value: int):
+        """Diagnostic switches of include/pdp.h (kernel, chunk_frames, sparse_warps, variant)."""
+        self._check(self._lib.pdp_debug_set(self._h, key.encode(), int(value)), "pdp_debug_set")
 
     def keep_common_mode(self, enable: bool = True):
         self._check(self._lib.pdp_keep_common_mode(self._h, int(enable)), "pdp_keep_common_mode")

@@ -1,18 +1,25 @@
-"""Build libpdp.so (the C-ABI library of include/pdp.h) in-tree with nvcc for sm_100a."""
+"""Build libpdp.so (the C-ABI library of include/pdp.h) in-tree with nvcc for sm_100a.
+
+The translation units (host API + small-batch kernel, and one unit per vector width of the throughput
+kernel's instantiations) are compiled in parallel and linked into one shared object.
+"""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpdp.so")
-SOURCES = ["pdp_api.cu"]
-HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_frames.cuh", "pdp_stream.cuh", os.path.join("..", "..", "include", "pdp.h")]
+OBJDIR = os.path.join(HERE, "build")
+SOURCES = ["pdp_api.cu", "pdp_chain_v8.cu", "pdp_chain_v4.cu", "pdp_chain_v2.cu"]
+HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_chain.cuh", "pdp_chain_inst.cuh", "pdp_post.cuh",
+           os.path.join("..", "..", "include", "pdp.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
+              "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -33,10 +40,18 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
-    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")]
-    cmd = [_nvcc(), *flags, *(["-Xptxas", "-v"] if verbose else []),
-           *[os.path.join(CSRC, s) for s in SOURCES], "-o", LIB]
-    subprocess.check_call(cmd)
+    os.makedirs(OBJDIR, exist_ok=True)
+    nvcc = _nvcc()
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(src: str) -> str:
+        obj = os.path.join(OBJDIR, os.path.splitext(src)[0] + ".o")
+        subprocess.check_call([nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj])
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as pool:
+        objs = list(pool.map(compile_one, SOURCES))
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", *objs, "-o", LIB])
     return LIB
 
 

@@ -1,5 +1,6 @@
-// pdp_api.cu — host side of the C ABI declared in include/pdp.h: validation, derived maps,
-// launch configuration, the single fused launch per batch, and the double-buffered host feed.
+// pdp_api.cu — host side of the C ABI declared in include/pdp.h: validation, derived maps, launch
+// configuration, the launches of one batch, and the double-buffered host feed.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -9,38 +10,65 @@
 #include <vector>
 
 #include "../../include/pdp.h"
-#include "pdp_frames.cuh"
-#include "pdp_stream.cuh"
+#include "pdp_chain.cuh"
+#include "pdp_fused.cuh"
+#include "pdp_post.cuh"
 
-using pdp::FParams;
+using pdp::CParams;
 using pdp::KParams;
-using pdp::SParams;
+using pdp::PostParams;
+
+namespace pdp {
+using ChainFn = void (*)(const CParams);
+ChainFn chain_lookup_v8(int nv, int lps, int mode);   // pdp_chain_v8.cu
+ChainFn chain_lookup_v4(int nv, int lps, int mode);   // pdp_chain_v4.cu
+ChainFn chain_lookup_v2(int nv, int lps, int mode);   // pdp_chain_v2.cu
+}  // namespace pdp
 
 namespace {
 
 thread_local std::string g_last_error;  // errors raised before a context exists
 
+constexpr int kStatsSlots = 1 + 256 * pdp::kMaxSparseWarps;   // pixels, then seeds per (CTA, sparse warp)
+constexpr size_t kStatsBytes = kStatsSlots * sizeof(unsigned long long);
+
+// small-batch kernel (pdp_fused.cuh): band x chunk items with decoupled look-back
 struct LaunchPlan {
+  bool ok = false;
   int V = 0, G = 0;      // kernel variant
   int R = 0, TR = 0, WPR = 0, bands_per_panel = 0, n_bands = 0;
   int threads = 0;
   uint32_t stage_bytes = 0, off_v1 = 0, off_ctab = 0, off_cand = 0, off_accum = 0, off_misc = 0, smem = 0;
 };
 
-struct FramesPlan {
-  bool ok = false;
-  int R = 0, TR = 0, bands_per_panel = 0, n_bands = 0, threads = 0;
-  uint32_t stage_bytes = 0, smem = 0;
-  uint32_t off_v2h = 0, off_ctab = 0, off_cand = 0, off_wcnt = 0, off_rowcnt = 0, off_rowphot = 0, off_rowbase = 0,
-           off_swh = 0, off_stg = 0, off_pref = 0, off_phot = 0, off_desc = 0, off_bar = 0;
+// throughput kernel (pdp_chain.cuh)
+struct ChainVariant {
+  int V, NV, LPS;
 };
-constexpr int kFramesPerCtaMax = 1024;
+struct ChainPlan {
+  bool ok = false;
+  ChainVariant v{0, 0, 0};
+  int R = 0, NWD = 0, NWS = 0, WPR = 0, bands_per_panel = 0, n_bands = 0;
+  uint32_t off_cm = 0, off_flag = 0, off_bar = 0, off_done = 0, off_pref = 0, off_phot = 0, off_sparse = 0,
+           sparse_stride = 0, off_ring = 0, off_maps = 0, ring_warp_bytes = 0, maps_warp_bytes = 0, smem = 0;
+};
 
-struct StreamPlan {
-  bool ok = false;
-  int R = 0, NW = 0, FL = 1, bands_per_panel = 0, n_bands = 0;
-  uint32_t off_cm = 0, off_bits = 0, off_cnt = 0, off_done = 0, off_pref = 0, off_phot = 0, off_list = 0, off_rowmask = 0, off_ring = 0, off_maps = 0, smem = 0;
+// Preference order per vector width: the first entry that covers S with at most 25 % padding wins, otherwise
+// the one with the least padding.  Entries with LPS < 32 put several frames side by side in a warp.
+const ChainVariant kVariants[] = {
+    {8, 6, 8}, {8, 4, 8}, {8, 4, 16}, {8, 3, 16}, {8, 2, 16}, {8, 1, 32}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32},
+    {4, 1, 32}, {4, 2, 32}, {4, 4, 32}, {4, 8, 32},
+    {2, 13, 8}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
 };
+
+pdp::ChainFn chain_kernel(const ChainVariant &v, int mode) {
+  switch (v.V) {
+    case 8: return pdp::chain_lookup_v8(v.NV, v.LPS, mode);
+    case 4: return pdp::chain_lookup_v4(v.NV, v.LPS, mode);
+    case 2: return pdp::chain_lookup_v2(v.NV, v.LPS, mode);
+  }
+  return nullptr;
+}
 
 }  // namespace
 
@@ -48,28 +76,33 @@ struct pdp_ctx {
   pdp_geometry geo{};
   pdp_params prm{};
   int device = 0, num_sms = 0;
+  size_t smem_limit = 0;
   size_t npix = 0;
-  float *d_ped = nullptr, *d_gain = nullptr, *d_K = nullptr, *d_rg = nullptr, *d_npf = nullptr;
+  float *d_ped = nullptr, *d_gain = nullptr, *d_rg = nullptr;
+  float *d_K = nullptr, *d_npf = nullptr;   // small-batch kernel: 2^23 + rint(ped), -(ped - rint(ped))/gain
   double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
-  float *d_cm = nullptr;  // optional kept common-mode estimates
+  unsigned long long *d_stats = nullptr;    // written by the throughput kernel: [0] pixels, [1..] seeds per sparse warp
+  unsigned long long *h_stats = nullptr;    // pinned copy, refreshed asynchronously after every launch
+  double density = 0.0;                     // seeds per pixel of the last launch whose statistics have arrived
+  float *d_cm = nullptr;                    // optional kept common-mode estimates
   int keep_cm = 0;
-  int64_t cm_frames = 0;  // frames of the last call whose estimates are in d_cm
+  int64_t cm_frames = 0;                    // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
-  FramesPlan fplan[2];      // [0] without, [1] with the fp16 pre-filter tile
-  StreamPlan splan[3];      // the streaming kernel (pdp_stream.cuh): [0] maps in registers, [1] maps in shared memory
-  double amax = 0.0;        // max over pixels of |v1| any uint16 raw value can produce
-  int prefilter = 0;        // PDP_PREFILTER=1 selects fplan[1]
-  int kernel_override = 0;  // 0 auto, 1 look-back kernel, 2 frames kernel, 3 streaming kernel (PDP_KERNEL)
-  int chunk_frames_override = 0;
+  ChainPlan cplan[2];                       // [0] 4 sparse warps (sparse data), [1] 8 sparse warps (dense data)
+  ChainVariant forced{0, 0, 0};             // pdp_debug_set("variant")
+  int kernel_override = 0;                  // pdp_debug_set("kernel"): 0 auto, 1 look-back kernel, 2 throughput kernel
+  int chunk_frames_override = 0;            // pdp_debug_set("chunk_frames")
+  int sparse_override = 0;                  // pdp_debug_set("sparse_warps"): 0 auto, 4, 8
   // host-feed state
   uint16_t *d_feed[2] = {nullptr, nullptr};
   int64_t feed_frames = 0;
   cudaStream_t copy_stream = nullptr;
   cudaEvent_t ev_ready[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
   int launches = 0;
-  const char *last_kernel = "";   // name of the dominant kernel of the last call (pdp_last_kernel_name)
+  const char *last_kernel = "";             // name of the dense-pass kernel of the last call
+  char last_kernel_buf[64] = {0};
   std::string last_error;
 };
 
@@ -98,8 +131,8 @@ int validate_params(const pdp_params *p) {
   return PDP_OK;
 }
 
-// Pick the kernel variant (V pixels per vector, G vectors per lane) with the fewest register
-// slots per lane, and the tallest band that fits the warp and shared-memory budgets.
+// Small-batch kernel: the variant (V pixels per vector, G vectors per lane) with the fewest register slots
+// per lane, and the tallest band that fits the warp and shared-memory budgets.
 bool make_plan(const pdp_geometry &g, size_t smem_limit, LaunchPlan &pl) {
   const int S = g.seg_cols, W = g.cols, nseg = W / S;
   int bestN = 1 << 30;
@@ -146,75 +179,72 @@ bool make_plan(const pdp_geometry &g, size_t smem_limit, LaunchPlan &pl) {
     pl.off_accum = off_accum;
     pl.off_misc = off_misc;
     pl.smem = off;
-    return true;
-  }
-  return false;
-}
-
-// Same choice for the frame-owner kernel (pdp_frames.cuh), whose shared-memory needs differ.
-template <bool PF>
-bool make_plan_frames(const pdp_geometry &g, int WPR, size_t smem_limit, FramesPlan &pl) {
-  using P = pdp::Pipe<PF>;
-  const int S = g.seg_cols, W = g.cols, nseg = W / S;
-  auto al = [](uint32_t x) { return (x + 127u) & ~127u; };
-  for (int R = pdp::kMaxWarps / nseg - 2; R >= 1; --R) {
-    if (R > g.rows) continue;
-    const int TR = R + 2, n_words = R * WPR;
-    if (n_words > pdp::kThreads) continue;
-    uint32_t off = 0;
-    const uint32_t stage = al((uint32_t)TR * W * 2u + 32u);
-    off += stage * P::kRing;
-    pl.off_v2h = off;      off = al(off + (PF ? P::D * (uint32_t)TR * W * 2u : 0u));
-    pl.off_ctab = off;     off = al(off + P::NB * (uint32_t)TR * nseg * 4u);
-    pl.off_cand = off;     off = al(off + P::NB * (uint32_t)n_words * 4u);
-    pl.off_wcnt = off;     off = al(off + P::NB * (uint32_t)n_words * 4u);
-    pl.off_rowcnt = off;   off = al(off + P::NB * (uint32_t)R * 4u);
-    pl.off_rowphot = off;  off = al(off + P::NB * (uint32_t)R * 4u);
-    pl.off_rowbase = off;  off = al(off + P::NB * (uint32_t)R * 4u);
-    pl.off_swh = off;      off = al(off + P::D * (uint32_t)n_words * 4u);
-    pl.off_stg = off;      off = al(off + P::D * 4u * (uint32_t)n_words * 4u);
-    pl.off_pref = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
-    pl.off_phot = off;     off = al(off + (uint32_t)kFramesPerCtaMax * 4u);
-    pl.off_desc = off;     off = al(off + P::NB * 16u);
-    pl.off_bar = off;      off = al(off + (P::kRing + 2 * P::NB) * 8u + (P::kRing + P::NB) * 4u);
-    if (off > smem_limit) continue;
-    pl.R = R;
-    pl.TR = TR;
-    pl.bands_per_panel = (g.rows + R - 1) / R;
-    pl.n_bands = pl.bands_per_panel * g.panels;
-    pl.threads = std::max(TR * nseg, (n_words + 31) / 32) * 32;
-    pl.stage_bytes = stage;
-    pl.smem = off;
     pl.ok = true;
     return true;
   }
   return false;
 }
 
-// The streaming kernel: one warp per (band row, segment), R = warps / segments rows per band.
-bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_limit, int ms, StreamPlan &pl) {
+bool pick_variant(const pdp_geometry &g, ChainVariant &out) {
+  const int S = g.seg_cols, W = g.cols;
+  int V = 0;
+  for (int v : {8, 4, 2})
+    if (S % v == 0 && W % v == 0) {
+      V = v;
+      break;
+    }
+  if (!V) return false;
+  const ChainVariant *best = nullptr;
+  int best_pad = 1 << 30;
+  for (const ChainVariant &c : kVariants) {
+    if (c.V != V) continue;
+    const int cap = c.V * c.NV * c.LPS, pad = cap - S;
+    if (pad < 0) continue;
+    if (4 * pad <= cap) {   // first preferred entry with at most 25 % padding
+      out = c;
+      return true;
+    }
+    if (pad < best_pad) best_pad = pad, best = &c;
+  }
+  if (!best) return false;
+  out = *best;
+  return true;
+}
+
+// The throughput kernel: one dense warp per (band row, segment), R = dense warps / segments rows per band.
+bool make_plan_chain(const pdp_geometry &g, const ChainVariant &v, int dense_warps_max, int nws, size_t smem_limit,
+                     ChainPlan &pl) {
   const int nseg = g.cols / g.seg_cols;
-  if (WPR > 32) return false;
-  auto al = [](uint32_t x) { return (x + 15u) & ~15u; };
-  // the tallest band (most dense warps) whose rings, raw prefetch ring and map tiles fit in shared memory
-  for (int R = std::min(std::min(pdp::kDenseWarpsMaxOf(ms) / nseg, (int)g.rows), 254); R >= 1; --R) {
-    if (R < 2 && g.rows > 1) return false;
+  const int N = v.V * v.NV;
+  if (v.V * v.NV * v.LPS < g.seg_cols || nseg > dense_warps_max) return false;
+  const int WPR = (g.cols + 31) / 32;
+  if (WPR > 64) return false;   // the per-row summary of non-zero bitmap words is one 64-bit word
+  auto al = [](uint32_t x) { return (x + 127u) & ~127u; };
+  for (int R = std::min(std::min(dense_warps_max / nseg, (int)g.rows), 254); R >= 1; --R) {
+    if (R < 2 && g.rows > 1) return false;   // the sparse stage needs the previous band's last two rows in the ring
     const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
+    const int NWD = R * nseg;
+    const uint32_t gfmax = (uint32_t)((pdp::kFCH + nws - 1) / nws);
     uint32_t off = 0;
-    pl.off_cm = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
-    pl.off_bits = off;  off = al(off + pdp::kFCH * ring * (uint32_t)WPR * 4u);
-    pl.off_cnt = off;   off = al(off + (uint32_t)pdp::kNB * pdp::kSparseWarps * 8u);
-    pl.off_done = off;  off = al(off + pdp::kFCH * 4u);
-    pl.off_pref = off;  off = al(off + pdp::kFCH * 4u);
-    pl.off_phot = off;  off = al(off + pdp::kFCH * 4u);
-    pl.off_list = off;  off = al(off + (uint32_t)pdp::kSparseWarps * pdp::kListCap * 4u);
-    pl.off_rowmask = off;  off = al(off + pdp::kFCH * ring * 4u);
-    pl.off_ring = off;  off = al(off + (uint32_t)(R * nseg) * pdp::kRingD * (uint32_t)(V * G * 64));
-    pl.off_maps = off;  off = al(off + (ms == 1 ? (uint32_t)(R * nseg) * 3u * (uint32_t)(V * G * 32) * 4u : 0u));
+    pl.off_cm = off;      off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
+    pl.off_flag = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
+    pl.off_bar = off;     off = al(off + (uint32_t)pdp::kNB * (uint32_t)nws * 8u);
+    pl.off_done = off;    off = al(off + (uint32_t)nws * 4u);
+    pl.off_pref = off;    off = al(off + pdp::kFCH * 4u);
+    pl.off_phot = off;    off = al(off + pdp::kFCH * 4u);
+    pl.sparse_stride = al((uint32_t)(pdp::kListCap + pdp::kItemCap) * 4u + gfmax * (uint32_t)(R + 1) * 8u +
+                          gfmax * (uint32_t)(R + 1) * (uint32_t)WPR * 4u);
+    pl.off_sparse = off;  off = al(off + (uint32_t)nws * pl.sparse_stride);
+    pl.ring_warp_bytes = (uint32_t)pdp::kRingD * 32u * (uint32_t)N * 2u;
+    pl.off_ring = off;    off = al(off + (uint32_t)NWD * pl.ring_warp_bytes);
+    pl.maps_warp_bytes = 2u * (uint32_t)v.LPS * (uint32_t)N * 4u;
+    pl.off_maps = off;    off = al(off + (uint32_t)NWD * pl.maps_warp_bytes);
     if (off > smem_limit) continue;
+    pl.v = v;
     pl.R = R;
-    pl.NW = R * nseg;
-    pl.FL = ms;   // the kernel's third template parameter
+    pl.NWD = NWD;
+    pl.NWS = nws;
+    pl.WPR = WPR;
     pl.bands_per_panel = (g.rows + R - 1) / R;
     pl.n_bands = pl.bands_per_panel * g.panels;
     pl.smem = off;
@@ -225,32 +255,6 @@ bool make_plan_stream(const pdp_geometry &g, int V, int G, int WPR, size_t smem_
 }
 
 using KernelFn = void (*)(const KParams);
-using StreamFn = void (*)(const SParams);
-
-template <int FL>
-StreamFn stream_kernel_for(int V, int G) {
-  switch (V * 10 + G) {
-    case 21: return pdp::pdp_stream_kernel<2, 1, FL>;
-    case 22: return pdp::pdp_stream_kernel<2, 2, FL>;
-    case 23: return pdp::pdp_stream_kernel<2, 3, FL>;
-    case 24: return pdp::pdp_stream_kernel<2, 4, FL>;
-    case 41: return pdp::pdp_stream_kernel<4, 1, FL>;
-    case 42: return pdp::pdp_stream_kernel<4, 2, FL>;
-    case 43: return pdp::pdp_stream_kernel<4, 3, FL>;
-    case 44: return pdp::pdp_stream_kernel<4, 4, FL>;
-    case 81: return pdp::pdp_stream_kernel<8, 1, FL>;
-    case 82: return pdp::pdp_stream_kernel<8, 2, FL>;
-  }
-  return nullptr;
-}
-StreamFn stream_kernel(int V, int G, int ms) {
-  if (V == 8 && G > 2) {
-    if (G == 3) return ms == 1 ? pdp::pdp_stream_kernel<8, 3, 1> : (ms ? pdp::pdp_stream_kernel<8, 3, 2> : pdp::pdp_stream_kernel<8, 3, 0>);
-    return ms == 1 ? pdp::pdp_stream_kernel<8, 4, 1> : (ms ? pdp::pdp_stream_kernel<8, 4, 2> : pdp::pdp_stream_kernel<8, 4, 0>);
-  }
-  return ms == 1 ? stream_kernel_for<1>(V, G) : (ms ? stream_kernel_for<2>(V, G) : stream_kernel_for<0>(V, G));
-}
-using FramesFn = void (*)(const FParams);
 
 KernelFn kernel_for(int V, int G) {
   switch (V * 10 + G) {
@@ -270,25 +274,6 @@ KernelFn kernel_for(int V, int G) {
   return nullptr;
 }
 
-template <bool PF>
-FramesFn frames_kernel_for(int V, int G) {
-  switch (V * 10 + G) {
-    case 21: return pdp::pdp_frames_kernel<2, 1, PF>;
-    case 22: return pdp::pdp_frames_kernel<2, 2, PF>;
-    case 23: return pdp::pdp_frames_kernel<2, 3, PF>;
-    case 24: return pdp::pdp_frames_kernel<2, 4, PF>;
-    case 41: return pdp::pdp_frames_kernel<4, 1, PF>;
-    case 42: return pdp::pdp_frames_kernel<4, 2, PF>;
-    case 43: return pdp::pdp_frames_kernel<4, 3, PF>;
-    case 44: return pdp::pdp_frames_kernel<4, 4, PF>;
-    case 81: return pdp::pdp_frames_kernel<8, 1, PF>;
-    case 82: return pdp::pdp_frames_kernel<8, 2, PF>;
-    case 83: return pdp::pdp_frames_kernel<8, 3, PF>;
-    case 84: return pdp::pdp_frames_kernel<8, 4, PF>;
-  }
-  return nullptr;
-}
-
 void free_ctx(pdp_ctx *c) {
   if (!c) return;
   cudaFree(c->d_ped);
@@ -299,7 +284,9 @@ void free_ctx(pdp_ctx *c) {
   cudaFree(c->d_rg64);
   cudaFree(c->d_lookback);
   cudaFree(c->d_ticket);
+  cudaFree(c->d_stats);
   cudaFree(c->d_cm);
+  if (c->h_stats) cudaFreeHost(c->h_stats);
   for (int i = 0; i < 2; ++i) {
     cudaFree(c->d_feed[i]);
     if (c->ev_ready[i]) cudaEventDestroy(c->ev_ready[i]);
@@ -307,6 +294,31 @@ void free_ctx(pdp_ctx *c) {
   }
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   delete c;
+}
+
+// (Re)build the throughput-kernel plans for the current variant choice.
+int build_chain_plans(pdp_ctx *c) {
+  ChainVariant v{0, 0, 0};
+  c->cplan[0] = ChainPlan{};
+  c->cplan[1] = ChainPlan{};
+  if (c->forced.V) v = c->forced;
+  else if (!pick_variant(c->geo, v)) return PDP_OK;   // no variant: the small-batch kernel serves every batch
+  make_plan_chain(c->geo, v, 16, 4, c->smem_limit, c->cplan[0]);
+  make_plan_chain(c->geo, v, 12, 8, c->smem_limit, c->cplan[1]);
+  for (int i = 0; i < 2; ++i) {
+    if (!c->cplan[i].ok) continue;
+    for (int mode = 0; mode < 3; ++mode) {
+      pdp::ChainFn fn = chain_kernel(v, mode);
+      if (!fn) {
+        c->cplan[i].ok = false;
+        break;
+      }
+      PDP_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)std::max(c->cplan[0].smem, c->cplan[1].smem)));
+    }
+  }
+  if (c->forced.V && !c->cplan[0].ok) return fail(c, PDP_E_GEOMETRY, "pdp_debug_set: variant does not fit this geometry");
+  return PDP_OK;
 }
 
 }  // namespace
@@ -352,11 +364,10 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceProperties");
   if (prop.major != 10) return fail(nullptr, PDP_E_NO_SM100, "pdp_create: device is not compute capability 10.x");
 
-  // derived dense-pass maps, evaluated in double: K = 2^23 + rint(ped), rg = 1/gain,
-  // npf = -(ped - rint(ped))/gain, so that v1 = fma((2^23 + raw) - K, rg, npf)
+  // derived maps, evaluated in double: rg = 1/gain (float and double); for the small-batch kernel
+  // K = 2^23 + rint(ped), npf = -(ped - rint(ped))/gain, so that v1 = fma((2^23 + raw) - K, rg, npf)
   std::vector<float> K, rg, npf;
   std::vector<double> rg64;
-  double amax = 0.0;
   try {
     rg64.resize(npix);
     K.resize(npix);
@@ -370,7 +381,6 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
     if (!std::isfinite(p) || !std::isfinite(g) || g == 0.0 || std::fabs(p) > 4.0e6)
       return fail(nullptr, PDP_E_VALUE, "pdp_create: non-finite or out-of-range pedestal/gain");
     const double pi = std::nearbyint(p), r = 1.0 / g;
-    amax = std::max(amax, (65535.0 + std::fabs(p)) * std::fabs(r));
     K[i] = (float)(8388608.0 + pi);
     rg[i] = (float)r;
     rg64[i] = r;
@@ -383,67 +393,47 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   c->prm = *prm;
   c->device = dev;
   c->num_sms = prop.multiProcessorCount;
+  c->smem_limit = prop.sharedMemPerBlockOptin;
   c->npix = npix;
-  if (!make_plan(*geo, prop.sharedMemPerBlockOptin, c->plan)) {
+  if (!make_plan(*geo, c->smem_limit, c->plan)) {
     free_ctx(c);
     return fail(nullptr, PDP_E_GEOMETRY, "pdp_create: no kernel variant fits this geometry");
   }
   KernelFn fn = kernel_for(c->plan.V, c->plan.G);
   e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->plan.smem);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(pdp::pdp_accum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
   if (e != cudaSuccess) {
     free_ctx(c);
     return cuda_fail(nullptr, e, "cudaFuncSetAttribute");
   }
-  make_plan_frames<false>(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan[0]);
-  make_plan_frames<true>(*geo, c->plan.WPR, prop.sharedMemPerBlockOptin, c->fplan[1]);
-  for (int pf = 0; pf < 2; ++pf) {
-    if (!c->fplan[pf].ok) continue;
-    FramesFn ff = pf ? frames_kernel_for<true>(c->plan.V, c->plan.G) : frames_kernel_for<false>(c->plan.V, c->plan.G);
-    e = cudaFuncSetAttribute(ff, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->fplan[pf].smem);
-    if (e != cudaSuccess) {
-      free_ctx(c);
-      return cuda_fail(nullptr, e, "cudaFuncSetAttribute(frames)");
-    }
+  if (int rc = build_chain_plans(c)) {
+    free_ctx(c);
+    return rc;
   }
-  c->amax = amax;
-  for (int ms = 0; ms < 3; ++ms) {
-    if (!make_plan_stream(*geo, c->plan.V, c->plan.G, c->plan.WPR, prop.sharedMemPerBlockOptin, ms, c->splan[ms])) continue;
-    StreamFn sf = stream_kernel(c->plan.V, c->plan.G, ms);
-    e = cudaFuncSetAttribute(sf, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->splan[ms].smem);
-    if (e != cudaSuccess) {
-      free_ctx(c);
-      return cuda_fail(nullptr, e, "cudaFuncSetAttribute(stream)");
-    }
-  }
-  if (const char *s = std::getenv("PDP_PREFILTER")) c->prefilter = std::atoi(s) != 0;
-  if (const char *s = std::getenv("PDP_KERNEL"))
-    c->kernel_override = !std::strcmp(s, "lookback") ? 1 : (!std::strcmp(s, "frames") ? 2 : (!std::strcmp(s, "stream") ? 3 : 0));
   const size_t mb = npix * sizeof(float);
   const size_t lb = (size_t)geo->max_frames_per_batch * c->plan.n_bands * sizeof(unsigned long long);
-  cudaError_t errs[] = {cudaMalloc(&c->d_ped, mb),     cudaMalloc(&c->d_gain, mb),      cudaMalloc(&c->d_K, mb),
-                        cudaMalloc(&c->d_rg, mb),      cudaMalloc(&c->d_npf, mb),       cudaMalloc(&c->d_lookback, lb),
-                        cudaMalloc(&c->d_ticket, 256)};
+  cudaError_t errs[] = {cudaMalloc(&c->d_ped, mb),      cudaMalloc(&c->d_gain, mb),
+                        cudaMalloc(&c->d_K, mb),        cudaMalloc(&c->d_rg, mb),
+                        cudaMalloc(&c->d_npf, mb),      cudaMalloc(&c->d_lookback, lb),
+                        cudaMalloc(&c->d_ticket, 256),  cudaMalloc(&c->d_stats, kStatsBytes),
+                        cudaMalloc(&c->d_rg64, npix * sizeof(double)),
+                        cudaHostAlloc(&c->h_stats, kStatsBytes, cudaHostAllocDefault)};
   for (cudaError_t x : errs)
     if (x != cudaSuccess) {
       free_ctx(c);
       return cuda_fail(nullptr, x, "cudaMalloc");
     }
-  e = cudaMalloc(&c->d_rg64, npix * sizeof(double));
+  std::memset(c->h_stats, 0, kStatsBytes);
+  e = cudaMemset(c->d_stats, 0, kStatsBytes);
   if (e == cudaSuccess) e = cudaMemcpy(c->d_rg64, rg64.data(), npix * sizeof(double), cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) {
-    free_ctx(c);
-    return cuda_fail(nullptr, e, "cudaMalloc/cudaMemcpy(rg64)");
-  }
   const void *srcs[] = {ped, gain, K.data(), rg.data(), npf.data()};
   float *dsts[] = {c->d_ped, c->d_gain, c->d_K, c->d_rg, c->d_npf};
-  for (int i = 0; i < 5; ++i) {
-    e = cudaMemcpy(dsts[i], srcs[i], mb, cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) {
-      free_ctx(c);
-      return cuda_fail(nullptr, e, "cudaMemcpy(maps)");
-    }
+  for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaMemcpy(dsts[i], srcs[i], mb, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    free_ctx(c);
+    return cuda_fail(nullptr, e, "cudaMemcpy(maps)");
   }
-  if (const char *s = std::getenv("PDP_CHUNK_FRAMES")) c->chunk_frames_override = std::atoi(s);
   *out_ctx = c;
   return PDP_OK;
 }
@@ -463,6 +453,30 @@ int pdp_destroy(pdp_ctx *ctx) {
 int pdp_last_launch_count(const pdp_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 const char *pdp_last_kernel_name(const pdp_ctx *ctx) { return ctx ? ctx->last_kernel : ""; }
+
+int pdp_debug_set(pdp_ctx *ctx, const char *key, int64_t value) {
+  if (!ctx || !key) return fail(ctx, PDP_E_NULL, "pdp_debug_set: null argument");
+  if (!std::strcmp(key, "kernel")) {
+    if (value < 0 || value > 2) return fail(ctx, PDP_E_VALUE, "pdp_debug_set: kernel must be 0, 1 or 2");
+    ctx->kernel_override = (int)value;
+    return PDP_OK;
+  }
+  if (!std::strcmp(key, "chunk_frames")) {
+    if (value < 0) return fail(ctx, PDP_E_VALUE, "pdp_debug_set: chunk_frames must be >= 0");
+    ctx->chunk_frames_override = (int)value;
+    return PDP_OK;
+  }
+  if (!std::strcmp(key, "sparse_warps")) {
+    if (value != 0 && value != 4 && value != 8) return fail(ctx, PDP_E_VALUE, "pdp_debug_set: sparse_warps must be 0, 4 or 8");
+    ctx->sparse_override = (int)value;
+    return PDP_OK;
+  }
+  if (!std::strcmp(key, "variant")) {   // V * 10000 + NV * 100 + LPS, 0 = automatic
+    ctx->forced = ChainVariant{(int)(value / 10000), (int)((value / 100) % 100), (int)(value % 100)};
+    return build_chain_plans(ctx);
+  }
+  return fail(ctx, PDP_E_VALUE, "pdp_debug_set: unknown key");
+}
 
 int pdp_keep_common_mode(pdp_ctx *ctx, int32_t enable) {
   if (!ctx) return fail(nullptr, PDP_E_NULL, "pdp_keep_common_mode: null ctx");
@@ -488,8 +502,118 @@ int pdp_get_common_mode(pdp_ctx *ctx, float *cm_device, int64_t n_floats, void *
 
 namespace {
 
+// The throughput path: pdp_chain_kernel (dense pass + sparse stage, one launch) followed by pdp_accum_kernel
+// (the accumulated image from the finished lists, no global atomics).
+int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o,
+                  bool keep_cm) {
+  CParams k{};
+  k.raw = raw;
+  k.n_frames = n;
+  k.ped = c->d_ped;
+  k.rg = c->d_rg;
+  k.rg64 = c->d_rg64;
+  k.P = c->geo.panels;
+  k.H = c->geo.rows;
+  k.W = c->geo.cols;
+  k.S = c->geo.seg_cols;
+  k.nseg = k.W / k.S;
+  k.WPR = pl.WPR;
+  k.R = pl.R;
+  k.bands_per_panel = pl.bands_per_panel;
+  k.n_bands = pl.n_bands;
+  k.NWD = pl.NWD;
+  k.NWS = pl.NWS;
+  k.T_seed = c->prm.seed_adu;
+  k.T_cm = c->prm.cm_adu;
+  k.E_ph = c->prm.photon_adu;
+  k.sqrtS = (float)std::sqrt((double)k.S);
+  // candidates: a superset of the seeds; the margin covers the fp32 rounding of v1 and of c
+  k.cand_thr = (float)((double)c->prm.seed_adu - std::max(1e-3, 4e-6 * std::fabs((double)c->prm.seed_adu)));
+  // BIG: the value of every pixel outside the mask; a power of two >= 4 * N * T_cm so that the sum of a lane's
+  // values splits exactly into (count outside the mask) * BIG + (sum inside)
+  {
+    const double need = std::max(1024.0, 4.0 * (double)(pl.v.V * pl.v.NV) * (double)c->prm.cm_adu + 1.0);
+    double big = 1024.0;
+    while (big < need) big *= 2.0;
+    k.big = (float)big;
+  }
+  k.dT_seed = (double)c->prm.seed_adu;
+  k.dE_ph = (double)c->prm.photon_adu;
+  k.cm_mode = c->prm.cm_mode;
+  k.cm_min_count = c->prm.cm_min_count > 0 ? c->prm.cm_min_count : (int)std::ceil(std::sqrt((double)k.S));
+  k.cap = o.hit_capacity;
+  k.hit_count = o.hit_count;
+  k.hit_pixel = o.hit_pixel;
+  k.hit_charge = o.hit_charge;
+  k.hit_nphot = o.hit_nphot;
+  k.hit_dx = o.hit_dx;
+  k.hit_dy = o.hit_dy;
+  k.frame_photons = o.frame_photons;
+  k.accum = o.accum;
+  k.status = o.status;
+  k.cm_keep = keep_cm ? c->d_cm : nullptr;
+  k.stats = c->d_stats;
+  k.off_cm = pl.off_cm;
+  k.off_flag = pl.off_flag;
+  k.off_bar = pl.off_bar;
+  k.off_done = pl.off_done;
+  k.off_pref = pl.off_pref;
+  k.off_phot = pl.off_phot;
+  k.off_sparse = pl.off_sparse;
+  k.sparse_stride = pl.sparse_stride;
+  k.off_ring = pl.off_ring;
+  k.off_maps = pl.off_maps;
+  k.ring_warp_bytes = pl.ring_warp_bytes;
+  k.maps_warp_bytes = pl.maps_warp_bytes;
+  const int grid = std::min(c->num_sms, n);
+  pdp::ChainFn fn = chain_kernel(pl.v, c->prm.cm_mode);
+  fn<<<grid, (pl.NWD + pl.NWS) * 32, pl.smem, st>>>(k);
+  PDP_CUDA(c, cudaGetLastError());
+  // accumulated image: owner-computes scatter of the finished lists
+  PostParams q{};
+  q.n_frames = n;
+  q.cap = o.hit_capacity;
+  q.npix = (uint32_t)c->npix;
+  const uint32_t span_max = (uint32_t)((c->smem_limit - 1024) / 4);
+  q.span = std::min(span_max, (uint32_t)((c->npix + c->num_sms - 1) / c->num_sms));
+  q.span = std::max(q.span, 1u);
+  q.hit_count = o.hit_count;
+  q.hit_pixel = o.hit_pixel;
+  q.hit_nphot = o.hit_nphot;
+  q.accum = o.accum;
+  const int grid_a = (int)((c->npix + q.span - 1) / q.span);
+  pdp::pdp_accum_kernel<<<grid_a, pdp::kPostThreads, (size_t)q.span * 4, st>>>(q);
+  PDP_CUDA(c, cudaGetLastError());
+  // density hint for the next call: running totals, copied back asynchronously and read without waiting
+  PDP_CUDA(c, cudaMemcpyAsync(c->h_stats, c->d_stats, (1 + (size_t)grid * pdp::kMaxSparseWarps) * sizeof(unsigned long long),
+                              cudaMemcpyDeviceToHost, st));
+  c->launches += 2;
+  std::snprintf(c->last_kernel_buf, sizeof(c->last_kernel_buf), "pdp_chain_kernel<%d,%d,%d,%d>", pl.v.V, pl.v.NV, pl.v.LPS,
+                c->prm.cm_mode);
+  c->last_kernel = c->last_kernel_buf;
+  return PDP_OK;
+}
+
 // Enqueue the chain for n frames at `raw` (device); outputs are already offset to this batch.
 int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o, bool keep_cm) {
+  // ---- large batches: the throughput kernel (frame-owner CTAs) ----
+  {
+    // seeds per pixel seen by earlier launches (stale by design: never waits for the device)
+    if (const unsigned long long pixels = c->h_stats[0]) {
+      unsigned long long seeds = 0;
+      for (int i = 0; i < std::min(c->num_sms, 256) * pdp::kMaxSparseWarps; ++i) seeds += c->h_stats[1 + i];
+      c->density = (double)seeds / (double)pixels;
+    }
+    int which = c->density > 0.01 ? 1 : 0;   // dense data: 8 sparse warps and 12 dense ones
+    if (c->sparse_override) which = c->sparse_override == 8 ? 1 : 0;
+    if (!c->cplan[which].ok) which ^= 1;
+    const bool can = c->cplan[which].ok;
+    const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
+    if (c->kernel_override == 2 && !can)
+      return fail(c, PDP_E_GEOMETRY, "pdp_debug_set(kernel=2): the throughput kernel does not support this geometry");
+    if (use_chain) return enqueue_chain(c, c->cplan[which], raw, n, st, o, keep_cm);
+  }
+  // ---- small batches: band x chunk items with decoupled look-back ----
   const LaunchPlan &pl = c->plan;
   KParams k{};
   k.raw = raw;
@@ -548,92 +672,6 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   k.off_cand = pl.off_cand;
   k.off_accum = pl.off_accum;
   k.off_misc = pl.off_misc;
-
-  // Large batches: the streaming kernel (frame-owner CTAs, no staging, no barriers).  It needs
-  // BIG = a power of two above twice the largest |v1| the maps allow, small enough to keep ~1e-2 ADU.
-  {
-    const double need = 2.0 * (c->amax + (double)c->prm.cm_adu) + 1.0;
-    double big = 1024.0;
-    while (big < need) big *= 2.0;
-    const bool big_ok = big <= 4194304.0 && (double)c->prm.cm_adu < 0.25 * big;
-    // median: maps in shared memory and 16 dense warps; mean / none: maps in registers, 12 dense warps
-    // variant: 0 mean/none; 1 median, maps in shared memory; 2 median, maps in registers (map tiles do not fit)
-    const int ms = c->prm.cm_mode != PDP_CM_MEDIAN ? 0 : ((c->splan[1].ok && c->splan[1].R >= c->splan[2].R) ? 1 : 2);
-    const bool use_stream = c->splan[ms].ok && big_ok &&
-                            (c->kernel_override == 3 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
-    if (c->kernel_override == 3 && !use_stream)
-      return fail(c, PDP_E_GEOMETRY, "PDP_KERNEL=stream: the streaming kernel does not support this geometry/maps");
-    if (use_stream) {
-      const StreamPlan &spl = c->splan[ms];
-      SParams s{};
-      s.k = k;
-      s.k.R = spl.R;
-      s.k.TR = spl.R;
-      s.k.bands_per_panel = spl.bands_per_panel;
-      s.k.n_bands = spl.n_bands;
-      s.rg64 = c->d_rg64;
-      s.big = (float)big;
-      s.magic = 0x4B000000u;
-      const double ulp_big = big / 8388608.0;
-      s.cand_thr = (float)((double)c->prm.seed_adu - (std::max(1e-3, 4e-6 * std::fabs((double)c->prm.seed_adu)) + 2.0 * ulp_big));
-      s.R = spl.R;
-      s.NW = spl.NW;
-      s.off_cm = spl.off_cm;
-      s.off_bits = spl.off_bits;
-      s.off_cnt = spl.off_cnt;
-      s.off_done = spl.off_done;
-      s.off_pref = spl.off_pref;
-      s.off_phot = spl.off_phot;
-      s.off_list = spl.off_list;
-      s.off_rowmask = spl.off_rowmask;
-      s.off_ring = spl.off_ring;
-      s.off_maps = spl.off_maps;
-      const int grid_s = std::min(c->num_sms, n);
-      StreamFn sf = stream_kernel(pl.V, pl.G, ms);
-      sf<<<grid_s, (spl.NW + pdp::kSparseWarps) * 32, spl.smem, st>>>(s);
-      PDP_CUDA(c, cudaGetLastError());
-      c->launches += 1;
-      c->last_kernel = "pdp_stream_kernel";
-      return PDP_OK;
-    }
-  }
-  // Otherwise: frame-owner kernel with the staged pipeline (every CTA owns a frame range).
-  // Small batches do not give every SM a frame range: band x chunk items with decoupled look-back.
-  const int pf = (c->prefilter && c->fplan[1].ok) ? 1 : 0;
-  const bool use_frames =
-      c->fplan[pf].ok && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
-  if (use_frames) {
-    const FramesPlan &fpl = c->fplan[pf];
-    FParams f{};
-    f.k = k;
-    f.k.R = fpl.R;
-    f.k.TR = fpl.TR;
-    f.k.bands_per_panel = fpl.bands_per_panel;
-    f.k.n_bands = fpl.n_bands;
-    f.k.stage_bytes = fpl.stage_bytes;
-    f.frames_per_cta_max = kFramesPerCtaMax;
-    f.off_v2h = fpl.off_v2h;
-    f.off_ctab = fpl.off_ctab;
-    f.off_cand = fpl.off_cand;
-    f.off_wcnt = fpl.off_wcnt;
-    f.off_rowcnt = fpl.off_rowcnt;
-    f.off_rowphot = fpl.off_rowphot;
-    f.off_rowbase = fpl.off_rowbase;
-    f.off_swh = fpl.off_swh;
-    f.off_stg = fpl.off_stg;
-    f.off_pref = fpl.off_pref;
-    f.off_phot = fpl.off_phot;
-    f.off_desc = fpl.off_desc;
-    f.off_bar = fpl.off_bar;
-    f.rg64 = c->d_rg64;
-    const int grid_f = std::max(std::min(c->num_sms, n), (n + kFramesPerCtaMax - 1) / kFramesPerCtaMax);
-    FramesFn ff = pf ? frames_kernel_for<true>(pl.V, pl.G) : frames_kernel_for<false>(pl.V, pl.G);
-    ff<<<grid_f, fpl.threads, fpl.smem, st>>>(f);
-    PDP_CUDA(c, cudaGetLastError());
-    c->launches += 1;
-    c->last_kernel = "pdp_frames_kernel";
-    return PDP_OK;
-  }
   PDP_CUDA(c, cudaMemsetAsync(c->d_lookback, 0, (size_t)n * pl.n_bands * sizeof(unsigned long long), st));
   PDP_CUDA(c, cudaMemsetAsync(c->d_ticket, 0, sizeof(unsigned), st));
   const int grid = std::min(k.n_items, c->num_sms);
@@ -669,15 +707,15 @@ int pdp_process(pdp_ctx *ctx, const pdp_batch *batch, void *stream, const pdp_ou
   return enqueue(ctx, batch->data, batch->n_frames, (cudaStream_t)stream, *out, ctx->keep_cm != 0);
 }
 
-int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, int32_t chunk_frames, void *stream,
-                     const pdp_output *out) {
-  if (!ctx || (!raw_host && n_frames > 0)) return fail(ctx, PDP_E_NULL, "pdp_process_host: null argument");
+int pdp_process_pinned(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, int32_t chunk_frames,
+                       void *compute_stream, void *copy_stream, const pdp_output *out) {
+  if (!ctx || (!raw_host && n_frames > 0)) return fail(ctx, PDP_E_NULL, "pdp_process_pinned: null argument");
   if (int rc = check_output(ctx, out)) return rc;
   if (n_frames < 0 || chunk_frames < 1 || chunk_frames > ctx->geo.max_frames_per_batch)
-    return fail(ctx, PDP_E_BATCH, "pdp_process_host: n_frames / chunk_frames out of range");
+    return fail(ctx, PDP_E_BATCH, "pdp_process_pinned: n_frames / chunk_frames out of range");
   ctx->launches = 0;
   if (n_frames == 0) return PDP_OK;
-  cudaStream_t st = (cudaStream_t)stream;
+  cudaStream_t st = (cudaStream_t)compute_stream;
   const size_t frame_bytes = ctx->npix * sizeof(uint16_t);
   if (ctx->feed_frames < chunk_frames) {
     for (int i = 0; i < 2; ++i) {
@@ -687,24 +725,26 @@ int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, i
     }
     ctx->feed_frames = chunk_frames;
   }
-  if (!ctx->copy_stream) {
-    PDP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+  if (!ctx->ev_ready[0]) {
     for (int i = 0; i < 2; ++i) {
       PDP_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_ready[i], cudaEventDisableTiming));
       PDP_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_free[i], cudaEventDisableTiming));
     }
   }
-  // the copy stream must not overwrite a feed buffer that earlier work on `st` still reads
-  for (int i = 0; i < 2; ++i) {
-    PDP_CUDA(ctx, cudaEventRecord(ctx->ev_free[i], st));
+  cudaStream_t cs = (cudaStream_t)copy_stream;
+  if (!cs) {   // no copy stream given: the context's own side stream
+    if (!ctx->copy_stream) PDP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    cs = ctx->copy_stream;
   }
+  // the copy stream must not overwrite a feed buffer that earlier work on `st` still reads
+  for (int i = 0; i < 2; ++i) PDP_CUDA(ctx, cudaEventRecord(ctx->ev_free[i], st));
   int launches = 0;
   for (int f0 = 0, i = 0; f0 < n_frames; f0 += chunk_frames, ++i) {
     const int b = i & 1, n = std::min(chunk_frames, n_frames - f0);
-    PDP_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_free[b], 0));
+    PDP_CUDA(ctx, cudaStreamWaitEvent(cs, ctx->ev_free[b], 0));
     PDP_CUDA(ctx, cudaMemcpyAsync(ctx->d_feed[b], raw_host + (size_t)f0 * ctx->npix, (size_t)n * frame_bytes,
-                                  cudaMemcpyHostToDevice, ctx->copy_stream));
-    PDP_CUDA(ctx, cudaEventRecord(ctx->ev_ready[b], ctx->copy_stream));
+                                  cudaMemcpyHostToDevice, cs));
+    PDP_CUDA(ctx, cudaEventRecord(ctx->ev_ready[b], cs));
     PDP_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_ready[b], 0));
     pdp_output o = *out;
     o.hit_count += f0;
@@ -715,13 +755,19 @@ int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, i
     o.hit_nphot += off;
     o.hit_dx += off;
     o.hit_dy += off;
+    ctx->launches = 0;
     if (int rc = enqueue(ctx, ctx->d_feed[b], n, st, o, false)) return rc;
-    launches += 1;
+    launches += ctx->launches;
     PDP_CUDA(ctx, cudaEventRecord(ctx->ev_free[b], st));
   }
   ctx->launches = launches;
   ctx->cm_frames = 0;
   return PDP_OK;
+}
+
+int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, int32_t chunk_frames, void *stream,
+                     const pdp_output *out) {
+  return pdp_process_pinned(ctx, raw_host, n_frames, chunk_frames, stream, nullptr, out);
 }
 
 }  // extern "C"

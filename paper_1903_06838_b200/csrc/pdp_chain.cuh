@@ -1,0 +1,907 @@
+// pdp_chain.cuh — the throughput kernel of the reduction chain (one launch per pdp_process call).
+//
+// Decomposition: frame-owner.  CTA b owns the frames [b*n/grid, (b+1)*n/grid) and walks them in chunks of
+// kFCH frame slots, band by band (band = R rows of one panel), so the per-frame hit-list offsets are a
+// CTA-local running prefix (ordered, deterministic output without any inter-CTA exchange).
+//
+// Warp roles (no CTA-wide barrier after the prologue):
+//   * dense warps, one per (row of the band, row segment).  A warp handles FPS = 32/LPS frames at once:
+//     LPS lanes share one row segment of one frame, every lane owns a contiguous run of N = V*NV pixels
+//     in registers.  The per-segment scalar work of the exact median (pivot policy, bracket, order-statistic
+//     read-out) is therefore amortised over N pixels per lane instead of S/32, the cross-lane reductions are
+//     log2(LPS) shuffles, and lanes of different frames run the same instruction stream.
+//       raw pixels : per-lane cp.async (LDGSTS) into a lane-major ring, kRingD steps deep (each lane copies
+//                    and later reads only its own vectors: cp.async.wait_group is the only synchronisation);
+//       maps       : pedestal and 1/gain of the segment, staged once per (band, chunk) into a lane-major
+//                    tile in shared memory (conflict-free LDS.128), shared by the FPS frames of a step;
+//       calibrate  : a = (float(raw) - ped) * (1/gain)            PAPER.md:L41, L51   (I2F.U16, FADD, FMUL)
+//       mask       : |a| < T_cm
+//       estimate   : exact median of the masked pixels (north_star (a)) by counting in value space, or the
+//                    paper's guarded mean sum/max(n, sqrt(S)), or none;
+//       candidates : ONE bit per lane: max(a) over the lane's run > T_seed - margin + c.
+//   * sparse warps: sleep on an mbarrier until every dense warp has published a band, then, for their frame
+//     slots: expand the flagged lane runs to pixel candidates (same fp32 formula), apply the exact fp64
+//     seed rule (strict 3x3 maximum, ties to the lower index, panel edges) to every candidate, compute E, n,
+//     dx, dy in the oracle's order of operations and emit the hits in pixel order.
+//
+// Nothing dense is written to HBM: common-mode estimates, candidate flags and the prefix state of the ordered
+// compaction live in shared memory.  The accumulated image is NOT touched here (pdp_post.cuh scatters the
+// finished lists by pixel-range ownership: no global atomics), except for hits beyond the list capacity.
+#pragma once
+#include "pdp_device.cuh"
+
+namespace pdp {
+
+constexpr int kFCH = 16;          // frame slots per chunk
+constexpr int kNB = 5;            // band slots of the shared-memory rings
+constexpr int kRingD = 2;         // raw-pixel ring depth in steps (kRingD - 1 steps of prefetch in flight; a step of a warp
+                                  // lasts microseconds because the sub-partition's other warps run in between)
+constexpr int kMaxIt = 7;         // counting passes before the search switches to walking / bisection
+constexpr int kListCap = 128;     // candidates evaluated per batch by a sparse warp
+constexpr int kItemCap = 64;      // flagged lane runs expanded per batch by a sparse warp
+constexpr int kChainMaxThreads = 640;
+constexpr int kMaxSparseWarps = 8;
+
+struct CParams {
+  // inputs
+  const uint16_t *raw;
+  int n_frames;
+  const float *ped;      // the caller's pedestal (float32)
+  const float *rg;       // 1/gain rounded to float32 (dense pass)
+  const double *rg64;    // 1/gain in double (exact evaluation of candidates)
+  // geometry
+  int P, H, W, S, nseg, WPR;                 // WPR: 32-bit words per bitmap row
+  int R, bands_per_panel, n_bands;           // band rows, bands
+  int NWD, NWS;                              // dense warps (R * nseg), sparse warps
+  // thresholds
+  float T_seed, T_cm, E_ph, sqrtS, cand_thr, big;
+  double dT_seed, dE_ph;
+  int cm_mode, cm_min_count;
+  // outputs
+  uint32_t cap;
+  uint32_t *hit_count, *hit_pixel;
+  float *hit_charge;
+  int32_t *hit_nphot;
+  float *hit_dx, *hit_dy;
+  uint32_t *frame_photons, *accum, *status;
+  float *cm_keep;                            // optional [n][P][H][nseg]
+  unsigned long long *stats;                 // density hint for the next launch, plain stores only: [0] pixels of this launch,
+                                             // [1 + block * kMaxSparseWarps + sw] seeds found by that sparse warp
+  // shared-memory carve-up (byte offsets)
+  uint32_t off_cm, off_flag, off_bar, off_done, off_pref, off_phot, off_sparse, sparse_stride, off_ring, off_maps;
+  uint32_t ring_warp_bytes, maps_warp_bytes;
+};
+
+// ---- small helpers ---------------------------------------------------------------------------------------
+template <int BYTES>
+__device__ __forceinline__ void cp_async_s(uint32_t dst_smem, const void *src) {   // SASS: LDGSTS
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst_smem), "l"(src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {   // release
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // acquire when it succeeds
+  uint32_t ok;   // try_wait suspends the warp in hardware until the phase completes or the hint (ns) expires
+  asm volatile(
+      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity), "r"(100000u)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void red_add_u32(uint32_t *p, uint32_t v) {
+  asm volatile("red.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ float rcp_approx(float x) {   // one MUFU.RCP
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+#ifndef PDP_CVT_PRMT
+__device__ __forceinline__ float u16lo_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H0
+  float f;
+  asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, l;}" : "=f"(f) : "r"(w));
+  return f;
+}
+__device__ __forceinline__ float u16hi_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H1
+  float f;
+  asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, h;}" : "=f"(f) : "r"(w));
+  return f;
+}
+#else   // PRMT builds the float 2^23 + raw, the subtraction of 2^23 is exact
+__device__ __forceinline__ float u16lo_to_f(uint32_t w) {
+  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - 8388608.f;
+}
+__device__ __forceinline__ float u16hi_to_f(uint32_t w) {
+  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8388608.f;
+}
+#endif
+__device__ __forceinline__ float set_lt_abs(float a, float t) {   // 1.0f if |a| < t else 0.0f
+  float d;
+  asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(fabsf(a)), "f"(t));
+  return d;
+}
+__device__ __forceinline__ float set_ge(float a, float b) {
+  float d;
+  asm("set.ge.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  return d;
+}
+__device__ __forceinline__ float max3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }   // FMNMX3
+__device__ __forceinline__ float min3(float a, float b, float c) { return fminf(fminf(a, b), c); }
+__device__ __forceinline__ float next_up(float a) {   // the next float above a (a finite)
+  const float z = a + 0.f;                              // -0 -> +0
+  const int b = __float_as_int(z);
+  return __int_as_float(z >= 0.f ? b + 1 : b - 1);
+}
+
+template <int V>
+struct VecLoadS;   // V uint16 pixels from a shared-memory byte address
+template <>
+struct VecLoadS<2> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[1]) {
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w[0]) : "r"(a));
+  }
+};
+template <>
+struct VecLoadS<4> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[2]) {
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(w[0]), "=r"(w[1]) : "r"(a));
+  }
+};
+template <>
+struct VecLoadS<8> {
+  __device__ static __forceinline__ void ld(uint32_t a, uint32_t (&w)[4]) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(a));
+  }
+};
+template <int CS>
+__device__ __forceinline__ void lds_f(uint32_t a, float *d) {   // CS (2 or 4) floats from shared memory
+  if constexpr (CS == 2) {
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(d[0]), "=f"(d[1]) : "r"(a));
+  } else {
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3]) : "r"(a));
+  }
+}
+
+// reductions over the LPS lanes that share a row segment (lanes [g*LPS, (g+1)*LPS) of the warp)
+template <int LPS>
+__device__ __forceinline__ float group_sum(float v) {
+#pragma unroll
+  for (int o = LPS / 2; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+  return v;
+}
+template <int LPS>
+__device__ __forceinline__ float group_count(float v) {   // sum of small exact integers held as floats
+  if constexpr (LPS == 32) return (float)__reduce_add_sync(FULL, __float2int_rn(v));   // REDUX
+  else return group_sum<LPS>(v);
+}
+template <int LPS>
+__device__ __forceinline__ float group_min(float v) {
+  if constexpr (LPS == 32) {
+    float r;
+    asm volatile("redux.sync.min.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+    return r;
+  } else {
+#pragma unroll
+    for (int o = LPS / 2; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+  }
+}
+template <int LPS>
+__device__ __forceinline__ float group_max(float v) {
+  if constexpr (LPS == 32) {
+    float r;
+    asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+    return r;
+  } else {
+#pragma unroll
+    for (int o = LPS / 2; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+  }
+}
+
+// ---- the three passes of the exact selection over the lane's N values (b: masked value, or BIG) --------------
+// count(p) = #{b < p};  up(p) = (#{b < p}, min{b >= p});  down(p) = (#{b < p}, max{b < p}).
+// Values on the wrong side of p are pushed out of range by +-big2 (the values that matter are untouched).
+template <int N, int LPS>
+__device__ __forceinline__ float pass_count(const float (&b)[N], float p) {
+  float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f;   // exact small integers; four chains for ILP
+#pragma unroll
+  for (int j = 0; j < N; ++j) {
+    const float d = set_lt(b[j], p);
+    if ((j & 3) == 0) c0 += d;
+    else if ((j & 3) == 1) c1 += d;
+    else if ((j & 3) == 2) c2 += d;
+    else c3 += d;
+  }
+  return group_count<LPS>((c0 + c1) + (c2 + c3));
+}
+template <int N, int LPS>
+__device__ __forceinline__ float pass_up(const float (&b)[N], float p, float big2, float &cnt) {
+  float c0 = 0.f, c1 = 0.f, m0 = __int_as_float(0x7f800000), m1 = m0;
+#pragma unroll
+  for (int j = 0; j + 1 < N; j += 2) {
+    const float d0 = set_lt(b[j], p), d1 = set_lt(b[j + 1], p);
+    c0 += d0;
+    c1 += d1;
+    const float t0 = fmaf(d0, big2, b[j]), t1 = fmaf(d1, big2, b[j + 1]);
+    if (j & 2) m1 = min3(m1, t0, t1);
+    else m0 = min3(m0, t0, t1);
+  }
+  if constexpr (N & 1) {
+    const float d0 = set_lt(b[N - 1], p);
+    c0 += d0;
+    m0 = fminf(m0, fmaf(d0, big2, b[N - 1]));
+  }
+  cnt = group_count<LPS>(c0 + c1);
+  return group_min<LPS>(fminf(m0, m1));
+}
+template <int N, int LPS>
+__device__ __forceinline__ float pass_down(const float (&b)[N], float p, float big2, float &cnt) {
+  float c0 = 0.f, c1 = 0.f, m0 = __int_as_float(0xff800000), m1 = m0;   // counts of b >= p here
+#pragma unroll
+  for (int j = 0; j + 1 < N; j += 2) {
+    const float d0 = set_ge(b[j], p), d1 = set_ge(b[j + 1], p);
+    c0 += d0;
+    c1 += d1;
+    const float t0 = fmaf(d0, -big2, b[j]), t1 = fmaf(d1, -big2, b[j + 1]);
+    if (j & 2) m1 = max3(m1, t0, t1);
+    else m0 = max3(m0, t0, t1);
+  }
+  if constexpr (N & 1) {
+    const float d0 = set_ge(b[N - 1], p);
+    c0 += d0;
+    m0 = fmaxf(m0, fmaf(d0, -big2, b[N - 1]));
+  }
+  cnt = (float)(LPS * N) - group_count<LPS>(c0 + c1);
+  return group_max<LPS>(fmaxf(m0, m1));
+}
+
+// Exact median of the masked values of a row segment held by a group of LPS lanes (N values per lane; values
+// outside the mask and padding are exactly `big`).  n = number of masked values (> 0), mean = their mean.
+// All lanes of the warp run this together; the lanes of a group hold identical scalar state.
+//   search : safeguarded secant on (pivot, rank) pairs inside the bracket (lo, hi), first step by a running
+//            estimate of the ADU-per-rank density; a pivot is accepted when its rank is within one of the
+//            wanted ones;
+//   read   : order statistics are read with up()/down() passes that walk from the accepted pivot, each
+//            returning one distinct value and how many ranks it covers (ties);
+//   rescue : when the search does not converge (exact ties), it walks up from the bracket's lower end.
+// The result is the fp32 value of the middle element (or the fp32 mean of the two middle ones).
+template <int N, int LPS>
+__device__ __forceinline__ float group_median(const float (&b)[N], int n, float mean, float T_cm, float big,
+                                              bool active, float &apr) {
+  const float big2 = 4.f * big;
+  const int kl = (n - 1) >> 1, kh = n >> 1;
+  const float tgt = 0.5f * (float)(kl + kh + 1);
+  // phase: 0 search, 1 walk up, 2 walk down, 3 split (up then down at the same pivot), 4 done
+  int phase = active ? 0 : 4;
+  float p = fminf(fmaxf(mean, -T_cm), T_cm), lo = -T_cm, hi = T_cm, p_prev = 0.f;
+  int c_prev = 0, it = 0;
+  float xl = 0.f, xh = 0.f, prev = 0.f;
+  bool got = false, has_prev = false;
+#pragma unroll 1
+  while (__any_sync(FULL, phase != 4)) {
+    if (__any_sync(FULL, phase == 0)) {
+      const int c = (int)pass_count<N, LPS>(b, p);
+      if (phase == 0) {
+        if ((unsigned)(c - kl + 1) <= (unsigned)(kh - kl + 3)) {   // rank in [kl-1, kh+2]
+          phase = c <= kl ? 1 : (c > kh ? 2 : 3);
+        } else {
+          const float dc = (float)(c - c_prev);
+          const float sec = (p - p_prev) * rcp_approx(dc);
+          const bool use_sec = it > 0 && c != c_prev;
+          const float slope = use_sec ? sec : apr;
+          if (it == 1 && fabsf(dc) >= 8.f) apr = fmaf(0.25f, sec - apr, apr);
+          if (c < kl) lo = p;
+          else hi = p;
+          p_prev = p;
+          c_prev = c;
+          float pn = fmaf(tgt - (float)c, slope, p);
+          if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
+          ++it;
+          if (!(pn > lo && pn < hi) || it >= kMaxIt) {   // ties or a hostile distribution: walk up from lo
+            phase = 1;
+            pn = lo;
+          }
+          p = pn;
+        }
+      }
+    }
+    if (__any_sync(FULL, phase == 1 || phase == 3)) {
+      float cf;
+      const float A = pass_up<N, LPS>(b, p, big2, cf);   // A = x[c], c = #{b < p}
+      const int c = (int)cf;
+      if (phase == 3) {
+        xh = A;          // kl < c <= kh: the pivot separates the two middle elements
+        phase = 2;
+        got = true;      // walking down now only needs x[kl] = max{b < p}
+        has_prev = false;
+      } else if (phase == 1) {
+        // ranks [c_before, c) hold `prev` (known from the second pass on); A = x[c]
+        if (!got && has_prev && kl < c) xl = prev, got = true;
+        if (got && has_prev && kh < c) {
+          xh = prev;
+          phase = 4;
+        } else {
+          if (!got && c == kl) xl = A, got = true;
+          if (got && c == kh) {
+            xh = A;
+            phase = 4;
+          } else if (c > kh) {   // only reachable when the rescue walk started above: cannot happen (c(lo) <= kl)
+            xh = got ? A : xh;
+            phase = 4;
+          } else {
+            prev = A;
+            has_prev = true;
+            p = next_up(A);
+          }
+        }
+      }
+    }
+    if (__any_sync(FULL, phase == 2)) {
+      float cf;
+      const float B = pass_down<N, LPS>(b, p, big2, cf);   // B = x[c-1], c = #{b < p}
+      const int c = (int)cf;
+      if (phase == 2) {
+        // walking down from above: ranks [c, r_before] hold `prev`; B = x[c-1].  `got` = x[kh] known.
+        if (!got && has_prev && kh >= c) xh = prev, got = true;
+        if (got && has_prev && kl >= c) {
+          xl = prev;
+          phase = 4;
+        } else {
+          if (!got && c - 1 == kh) xh = B, got = true;
+          if (got && c - 1 <= kl) {
+            xl = B;
+            phase = 4;
+          } else {
+            prev = B;
+            has_prev = true;
+            p = B;
+          }
+        }
+      }
+    }
+  }
+  return 0.5f * (xl + xh);
+}
+
+// fp64 evaluation of the 3x3 window of (row, col) of panel p: v2 = (raw - ped) * (1/gain) - c with the
+// common-mode estimates of the three rows passed as pointers (nullptr: the row does not exist).
+__device__ __forceinline__ Exact9 exact9_rows(const CParams &k, const uint16_t *frame_raw, const float *cm_m1,
+                                              const float *cm_0, const float *cm_p1, int p, int row, int col) {
+  const int sgc = col / k.S, cs = col - sgc * k.S;
+  const int sg3[3] = {cs == 0 ? sgc - 1 : sgc, sgc, cs == k.S - 1 ? sgc + 1 : sgc};
+  const float *cmr[3] = {cm_m1, cm_0, cm_p1};
+  double v[9];
+  bool ex[9];
+#pragma unroll
+  for (int dr = -1; dr <= 1; ++dr)
+#pragma unroll
+    for (int dc = -1; dc <= 1; ++dc) {
+      const int i = (dr + 1) * 3 + dc + 1;
+      const int r = row + dr, c = col + dc;
+      ex[i] = (r >= 0 && r < k.H && c >= 0 && c < k.W);
+      v[i] = 0.0;
+      if (ex[i]) {
+        const size_t gi = ((size_t)p * k.H + r) * k.W + c;
+        const unsigned rawv = __ldg(frame_raw + gi);
+        const double cm = (double)cmr[dr + 1][sg3[dc + 1]];
+        v[i] = ((double)rawv - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - cm;
+      }
+    }
+  Exact9 o;
+  const double x = v[4];
+  o.seed = x > k.dT_seed;
+  o.E = 0.0;
+  o.sx = 0.0;
+  o.sy = 0.0;
+#pragma unroll
+  for (int i = 0; i < 9; ++i) {
+    if (!ex[i]) continue;
+    const double y = v[i];
+    o.E += y;
+    o.sx += (double)(i % 3 - 1) * y;
+    o.sy += (double)(i / 3 - 1) * y;
+    if (i == 4) continue;
+    // strict maximum; a tie goes to the lower linear index (i < 4 <=> neighbour has lower index)
+    if (!(x > y || (x == y && i > 4))) o.seed = false;
+  }
+  return o;
+}
+
+struct HitRec {
+  float E, dx, dy;
+  int n;
+};
+__device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
+  HitRec h;
+  h.E = (float)e9.E;
+  h.n = photon_count(e9.E, E_ph);
+  h.dx = e9.E > 0.0 ? (float)(e9.sx / e9.E) : 0.f;
+  h.dy = e9.E > 0.0 ? (float)(e9.sy / e9.E) : 0.f;
+  return h;
+}
+
+// Hits beyond the caller's list capacity are not in the lists the post pass scatters: they reach the
+// accumulated image here (a frame that overflows is a sizing error of the caller, never the hot path).
+static __device__ __noinline__ void overflow_accum(uint32_t *accum_px, uint32_t n, uint32_t *status) {
+  red_add_u32(accum_px, n);
+  *status = 1u;   // PDP_STATUS_HIT_OVERFLOW (the only bit; every writer stores the same value)
+}
+
+struct BandDesc {      // one band of one panel, as the sparse warps see it
+  int gb, band, p, bi; // running band index (over chunks), band of the frame, panel, band of the panel
+};
+
+// ---- sparse stage of one band for the frame slots {sw, sw + NWS, ...} < nf of the chunk: ONE warp ---------
+//  1. flagged lane runs (one flag bit per dense lane and frame) -> item list;
+//  2. every item's pixels are tested with the dense pass's own fp32 formula; candidate bits go to a private
+//     bitmap [frames of this warp][rows][W/32] with a per-row summary of the non-zero words;
+//  3. the candidate bits are compacted in (frame, row, column) order into a list, and every lane evaluates one
+//     candidate at a time in fp64 (all loads of a batch in flight together); seeds take their slot by
+//     ballot/popc on top of the frame's running count.
+template <int N, int LPS>
+__device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *smem, int sw, int nf, const BandDesc &bd,
+                                             int f0, unsigned long long &seeds_total) {
+  const int lane = threadIdx.x & 31;
+  const int R = k.R, ring_rows = kNB * R, NWS = k.NWS;
+  const float *cmring = reinterpret_cast<const float *>(smem + k.off_cm);
+  const uint32_t *flags = reinterpret_cast<const uint32_t *>(smem + k.off_flag);
+  volatile int *done = reinterpret_cast<volatile int *>(smem + k.off_done);
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);
+  unsigned char *mine = smem + k.off_sparse + (size_t)sw * k.sparse_stride;
+  uint32_t *list = reinterpret_cast<uint32_t *>(mine);                       // [kListCap]
+  uint32_t *items = list + kListCap;                                          // [kItemCap]
+  unsigned long long *rowmask = reinterpret_cast<unsigned long long *>(items + kItemCap);   // [GFmax][R+1]
+  const int GFmax = (kFCH + NWS - 1) / NWS;
+  uint32_t *bits = reinterpret_cast<uint32_t *>(rowmask + GFmax * (R + 1));  // [GFmax][R+1][WPR]
+
+  const int p = bd.p, r0 = bd.bi * R;
+  const int ra = bd.bi == 0 ? 0 : r0 - 1;
+  const int rb = bd.bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
+  const int nrows = rb - ra + 1;
+  const int nfr = nf > sw ? (nf - sw + NWS - 1) / NWS : 0;    // my frame slots: sw, sw + NWS, ...
+  // ring slot of row r in [r0-2, r0+R): bands gb-1 and gb
+  const int s_prev = ((bd.gb + kNB - 1) % kNB) * R, s_cur = (bd.gb % kNB) * R;
+  auto slot_of = [&](int r) { return r < r0 ? s_prev + (r - r0 + R) : s_cur + (r - r0); };
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  const int n_tasks = nrows > 0 ? nfr * nrows : 0;
+
+  // ---- 1 + 2: flagged lane runs -> candidate bitmap ----
+  // task t = (q, rr, sg): frame slot sw + q*NWS, row ra + rr, segment sg
+  const int n_ft = n_tasks * k.nseg;
+  for (int t0 = 0; t0 < n_ft; t0 += 32) {
+    const int t = t0 + lane;
+    uint32_t fw = 0u;
+    int tq = 0, trr = 0, tsg = 0;
+    if (t < n_ft) {
+      tsg = t % k.nseg;
+      const int u = t / k.nseg;
+      tq = u / nrows;
+      trr = u - tq * nrows;
+      fw = flags[((size_t)(sw + tq * NWS) * ring_rows + slot_of(ra + trr)) * k.nseg + tsg];
+    }
+    if (!__any_sync(FULL, fw != 0u)) continue;
+    int mine_n = __popc(fw), incl = mine_n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += u;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    const int first = incl - mine_n;
+    for (int b0 = 0; b0 < total; b0 += kItemCap) {
+      if (first < b0 + kItemCap && first + mine_n > b0) {
+        int idx = first;
+        for (uint32_t m = fw; m; m &= m - 1, ++idx)
+          if (idx >= b0 && idx < b0 + kItemCap)
+            items[idx - b0] = ((uint32_t)tq << 24) | ((uint32_t)trr << 16) | ((uint32_t)tsg << 8) | (uint32_t)(__ffs(m) - 1);
+      }
+      __syncwarp();
+      const int nb = min(kItemCap, total - b0);
+      for (int i0 = 0; i0 < nb; i0 += 32) {
+        if (i0 + lane < nb) {
+          const uint32_t e = items[i0 + lane];
+          const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), l = (int)(e & 0xffu);
+          const int row = ra + rr, fl = sw + q * NWS;
+          const float c = cmring[((size_t)fl * ring_rows + slot_of(row)) * k.nseg + sg];
+          const float thr = k.cand_thr + c;
+          const int c0 = sg * k.S + l * N, c1 = min(c0 + N, (sg + 1) * k.S);
+          const size_t gi = ((size_t)p * k.H + row) * k.W;
+          const uint16_t *rw = k.raw + (size_t)(f0 + fl) * npix + gi;
+          uint32_t *brow = bits + ((size_t)q * (R + 1) + rr) * k.WPR;
+          unsigned long long rm = 0ull;
+          for (int col = c0; col < c1; col += 2) {     // runs start and end on even columns
+            const uint32_t w = __ldg(reinterpret_cast<const uint32_t *>(rw + col));
+            const float2 pd = __ldg(reinterpret_cast<const float2 *>(k.ped + gi + col));
+            const float2 rg = __ldg(reinterpret_cast<const float2 *>(k.rg + gi + col));
+            const float a0 = (u16lo_to_f(w) - pd.x) * rg.x, a1 = (u16hi_to_f(w) - pd.y) * rg.y;
+            const uint32_t bb = (a0 > thr ? 1u : 0u) | (a1 > thr ? 2u : 0u);
+            if (bb) {
+              atomicOr(brow + (col >> 5), bb << (col & 31));
+              rm |= 1ull << (col >> 5);
+            }
+          }
+          if (rm) atomicOr(rowmask + q * (R + 1) + rr, rm);
+        }
+      }
+      __syncwarp();
+    }
+  }
+  __syncwarp();
+
+  // ---- 3: candidates in (frame, row, column) order -> exact rule -> ordered emission ----
+  uint32_t base = lane < nfr ? pref[sw + lane * NWS] : 0u;   // lane q holds the running totals of my frame q
+  int ph = 0;
+  for (int t0 = 0; t0 < n_tasks; t0 += 32) {
+    const int t = t0 + lane;
+    const bool tv = t < n_tasks;
+    int tq = 0, trr = 0;
+    if (tv) {
+      tq = t / nrows;
+      trr = t - tq * nrows;
+    }
+    const int rowslot = tq * (R + 1) + trr;
+    const unsigned long long rmask = tv ? rowmask[rowslot] : 0ull;
+    if (!__any_sync(FULL, rmask != 0ull)) continue;
+    uint32_t *rowbits = bits + (size_t)rowslot * k.WPR;
+    int mine_n = 0;
+    for (unsigned long long m = rmask; m; m &= m - 1) mine_n += __popc(rowbits[__ffsll((long long)m) - 1]);
+    int incl = mine_n;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int u = __shfl_up_sync(FULL, incl, o);
+      if (lane >= o) incl += u;
+    }
+    const int total = __shfl_sync(FULL, incl, 31);
+    const int my_first = incl - mine_n;
+    for (int b0 = 0; b0 < total; b0 += kListCap) {
+      if (my_first < b0 + kListCap && my_first + mine_n > b0) {
+        int idx = my_first;
+        for (unsigned long long m = rmask; m; m &= m - 1) {
+          const int wi = __ffsll((long long)m) - 1;
+          for (uint32_t wv = rowbits[wi]; wv; wv &= wv - 1) {
+            if (idx >= b0 && idx < b0 + kListCap)
+              list[idx - b0] = ((uint32_t)tq << 28) | ((uint32_t)trr << 20) | (uint32_t)(wi * 32 + __ffs(wv) - 1);
+            ++idx;
+          }
+        }
+      }
+      __syncwarp();
+      const int nb = min(kListCap, total - b0);
+      for (int i0 = 0; i0 < nb; i0 += 32) {
+        const bool have = i0 + lane < nb;
+        const uint32_t e = have ? list[i0 + lane] : 0u;
+        const int q = (int)(e >> 28), row = ra + (int)((e >> 20) & 0xffu), col = (int)(e & 0xfffffu);
+        const int fl = sw + q * NWS;
+        bool seed = false;
+        HitRec h{0.f, 0.f, 0.f, 0};
+        if (have) {
+          const float *cmf = cmring + (size_t)fl * ring_rows * k.nseg;
+          const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
+          const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : nullptr;
+          const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : nullptr;
+          const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + fl) * npix, cm_m1, cm_0, cm_p1, p, row, col);
+          seed = e9.seed;
+          if (seed) h = make_rec(e9, k.dE_ph);
+        }
+        if (!__any_sync(FULL, seed)) continue;
+        const unsigned lt = (1u << lane) - 1u;
+        unsigned mymask = 0u;
+        int add = 0, addph = 0;
+        for (int qq = 0; qq < nfr; ++qq) {
+          const unsigned m = __ballot_sync(FULL, seed && q == qq);
+          if (!m) continue;
+          const int phq = __reduce_add_sync(FULL, seed && q == qq ? h.n : 0);
+          if (q == qq) mymask = m;
+          if (lane == qq) add = __popc(m), addph = phq;
+        }
+        const uint32_t b_q = __shfl_sync(FULL, base, q);
+        if (seed) {
+          const uint32_t pos = b_q + __popc(mymask & lt);
+          const uint32_t pix = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
+          if (pos < k.cap) {
+            const size_t o = (size_t)(f0 + fl) * k.cap + pos;
+            k.hit_pixel[o] = pix;
+            k.hit_charge[o] = h.E;
+            k.hit_nphot[o] = h.n;
+            k.hit_dx[o] = h.dx;
+            k.hit_dy[o] = h.dy;
+          } else {
+            overflow_accum(k.accum + pix, (uint32_t)h.n, k.status);
+          }
+        }
+        base += (uint32_t)add;
+        ph += addph;
+      }
+      __syncwarp();
+    }
+    if (rmask) {   // consumed: clear the words and the summary
+      for (unsigned long long m = rmask; m; m &= m - 1) rowbits[__ffsll((long long)m) - 1] = 0u;
+      rowmask[rowslot] = 0ull;
+    }
+  }
+  if (lane < nfr) {
+    const int fl = sw + lane * NWS;
+    const uint32_t pht = phot[fl] + (uint32_t)ph;
+    if (bd.band == k.n_bands - 1) {  // the frame is complete
+      k.hit_count[f0 + fl] = base;
+      k.frame_photons[f0 + fl] = pht;
+      pref[fl] = 0u;
+      phot[fl] = 0u;
+      seeds_total += base;
+    } else {
+      pref[fl] = base;
+      phot[fl] = pht;
+    }
+  }
+  __syncwarp();
+  if (lane == 0) {
+    __threadfence_block();
+    done[sw] = bd.gb + 1;
+  }
+  __syncwarp();
+}
+
+// ---- the kernel ------------------------------------------------------------------------------------------
+// V = pixels per vector (2/4/8), NV = vectors per lane (N = V*NV contiguous pixels), LPS = lanes per row
+// segment (LPS*N >= S), MODE = 0 exact median / 1 guarded mean / 2 no common mode.
+template <int V, int NV, int LPS, int MODE>
+__global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CParams k) {
+  constexpr int N = V * NV;
+  constexpr int FPS = 32 / LPS;              // frames per warp step
+  constexpr int CS = V >= 4 ? 4 : 2;         // floats per map chunk (LDS.128 / LDS.64)
+  constexpr int CH = V / CS;                 // chunks per vector
+  constexpr uint32_t VB = V * 2;             // bytes per raw vector
+  constexpr uint32_t kStepBytes = 32u * N * 2u;   // one step of one warp in the raw ring
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int nthreads = blockDim.x, NWD = k.NWD, NWS = k.NWS;
+  const int R = k.R, ring_rows = kNB * R;
+  float *cmring = reinterpret_cast<float *>(smem + k.off_cm);          // [kFCH][kNB*R][nseg]
+  uint32_t *flags = reinterpret_cast<uint32_t *>(smem + k.off_flag);   // [kFCH][kNB*R][nseg]
+  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + k.off_bar);      // [kNB][NWS] mbarriers: NWD arrivals
+  volatile int *done = reinterpret_cast<volatile int *>(smem + k.off_done);  // [NWS]
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);    // [kFCH]
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);    // [kFCH]
+
+  const int fs = (int)(((long long)blockIdx.x * k.n_frames) / gridDim.x);
+  const int fe = (int)(((long long)(blockIdx.x + 1) * k.n_frames) / gridDim.x);
+  const int FCn = fe - fs;
+  if (FCn <= 0) return;
+
+  {  // prologue: zero the sparse warps' private bitmaps, initialise barriers and per-slot state
+    uint32_t *z = reinterpret_cast<uint32_t *>(smem + k.off_sparse);
+    const uint32_t nz = (uint32_t)NWS * k.sparse_stride / 4u;
+    for (uint32_t i = tid; i < nz; i += nthreads) z[i] = 0u;
+    if (tid == 0) {
+      for (int i = 0; i < kNB * NWS; ++i) mbar_init(&bar[i], (uint32_t)NWD);
+      fence_mbar_init();
+    }
+    for (int i = tid; i < kFCH; i += nthreads) pref[i] = 0u, phot[i] = 0u;
+    for (int i = tid; i < NWS; i += nthreads) done[i] = 0;
+  }
+  __syncthreads();
+
+  if (warp >= NWD) {
+    // ===== sparse warps =====
+    const int sw = warp - NWD;
+    BandDesc bd{0, 0, 0, 0};
+    unsigned long long seeds_total = 0ull;   // per lane: seeds of the frames this lane finished
+    for (int c0 = 0; c0 < FCn; c0 += kFCH) {
+      const int nf = min(kFCH, FCn - c0);
+      bd.band = 0, bd.p = 0, bd.bi = 0;
+      for (; bd.band < k.n_bands; ++bd.band, ++bd.gb) {
+        // every dense warp has published the band: acquire on my barrier of the band's ring slot
+        while (!mbar_test(&bar[(bd.gb % kNB) * NWS + sw], (uint32_t)(bd.gb / kNB) & 1u))
+          __nanosleep(2000);   // a sleeping warp costs no issue slots; a band of dense work lasts tens of microseconds
+        chain_sparse<N, LPS>(k, smem, sw, nf, bd, fs + c0, seeds_total);
+        if (++bd.bi == k.bands_per_panel) bd.bi = 0, ++bd.p;
+      }
+    }
+    if (k.stats) {   // density hint for the host (plain stores, one slot per sparse warp)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) seeds_total += __shfl_xor_sync(FULL, seeds_total, o);
+      if (lane == 0) k.stats[1 + blockIdx.x * kMaxSparseWarps + sw] = seeds_total;
+      if (lane == 0 && sw == 0 && blockIdx.x == 0)
+        k.stats[0] = (unsigned long long)k.n_frames * (unsigned long long)k.P * (unsigned long long)k.H * (unsigned long long)k.W;
+    }
+    return;
+  }
+
+  // ===== dense warps: (row tr of the band, segment sg); lane = (frame g of the step, lane-in-group l) =====
+  const int tr = warp / k.nseg, sg = warp - tr * k.nseg;
+  const int g = lane / LPS, l = lane - g * LPS;
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  const float T_cm = k.T_cm, BIG = k.big;
+  float apr = 0.375f * T_cm / (float)k.S;   // ADU per rank near the median (running estimate)
+  uint32_t vmask = 0;                        // which of this lane's NV vectors lie inside the segment
+#pragma unroll
+  for (int v = 0; v < NV; ++v) vmask |= (l * N + v * V < k.S ? 1u : 0u) << v;
+  const uint32_t ring_lane = smem_u32(smem + k.off_ring) + (uint32_t)warp * k.ring_warp_bytes + (uint32_t)lane * VB;
+  const uint32_t maps_base = smem_u32(smem + k.off_maps) + (uint32_t)warp * k.maps_warp_bytes;
+  float *maps_ptr = reinterpret_cast<float *>(smem + k.off_maps + (size_t)warp * k.maps_warp_bytes);
+  constexpr uint32_t kMapFloats = (uint32_t)LPS * N;          // floats per map in the tile
+  const uint32_t maps_lane = maps_base + (uint32_t)l * (CS * 4);
+  const int pix_lane = sg * k.S + l * N;                      // first column of this lane's run
+
+  int gb = 0;
+  for (int c0 = 0; c0 < FCn; c0 += kFCH) {
+    const int nf = min(kFCH, FCn - c0);
+    const int nsteps = (nf + FPS - 1) / FPS;
+    // Raw-pixel prefetch cursor: runs kRingD-1 steps ahead of the step being processed and crosses band
+    // boundaries inside the chunk, so the DRAM latency is paid once per chunk, not once per band.
+    int i_step = 0, i_band = 0, i_bi = 0, i_p = 0;
+    bool i_active = tr < k.H;
+    const uint16_t *chunk_raw = k.raw + (size_t)(fs + c0 + g) * npix + pix_lane;
+    const uint16_t *src = chunk_raw + (size_t)tr * k.W;
+    uint32_t islot = 0, rslot = 0;
+    auto issue = [&]() {
+      if (i_active && i_step * FPS + g < nf) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+          if ((vmask >> v) & 1u) cp_async_s<VB>(ring_lane + islot + v * (32 * VB), src + v * V);
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      src += (size_t)FPS * npix;
+      islot = islot + kStepBytes == kRingD * kStepBytes ? 0u : islot + kStepBytes;
+      if (++i_step == nsteps) {   // on to the first step of the next band
+        i_step = 0;
+        if (i_band + 1 < k.n_bands) {
+          ++i_band;
+          if (++i_bi == k.bands_per_panel) i_bi = 0, ++i_p;
+          const int row_n = i_bi * R + tr;
+          i_active = row_n < k.H;
+          src = chunk_raw + ((size_t)i_p * k.H + row_n) * k.W;
+        } else {
+          i_active = false;
+        }
+      }
+    };
+#pragma unroll 1
+    for (int d = 0; d < kRingD - 1; ++d) issue();
+
+    for (int band = 0; band < k.n_bands; ++band, ++gb) {
+      const int p = band / k.bands_per_panel, r0 = (band - p * k.bands_per_panel) * R;
+      const int row = r0 + tr;
+      const bool active = row < k.H;
+      const int slot = (gb % kNB) * R + tr;
+      if (active) {   // maps of this warp's row segment: global (L2) -> lane-major tile, once per band and chunk
+        const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
+        __syncwarp();
+        for (int ci = lane; ci < (int)(kMapFloats / CS); ci += 32) {
+          // chunk ci of the tile holds pixels j .. j+CS-1 of lane-slot ll: tile index (ck * LPS + ll)
+          const int ck = ci / LPS, ll = ci - ck * LPS;
+          const int j = ll * N + ck * CS;
+          float pd[CS], rr[CS];
+          if (j < k.S) {
+            if constexpr (CS == 4) {
+              const float4 a = __ldg(reinterpret_cast<const float4 *>(k.ped + rowoff + j));
+              const float4 b = __ldg(reinterpret_cast<const float4 *>(k.rg + rowoff + j));
+              pd[0] = a.x, pd[1] = a.y, pd[2] = a.z, pd[3] = a.w;
+              rr[0] = b.x, rr[1] = b.y, rr[2] = b.z, rr[3] = b.w;
+            } else {
+              const float2 a = __ldg(reinterpret_cast<const float2 *>(k.ped + rowoff + j));
+              const float2 b = __ldg(reinterpret_cast<const float2 *>(k.rg + rowoff + j));
+              pd[0] = a.x, pd[1] = a.y;
+              rr[0] = b.x, rr[1] = b.y;
+            }
+          } else {   // padding: a = (raw - 3e38) * 1 = -3e38: outside the mask, never a candidate
+#pragma unroll
+            for (int e = 0; e < CS; ++e) pd[e] = 3.0e38f, rr[e] = 1.f;
+          }
+#pragma unroll
+          for (int e = 0; e < CS; ++e) {
+            maps_ptr[ci * CS + e] = pd[e];
+            maps_ptr[kMapFloats + ci * CS + e] = rr[e];
+          }
+        }
+        __syncwarp();
+      }
+      // the ring slot about to be written held band gb-kNB, last read by the sparse stage of band gb-kNB+1
+      for (int s = 0; s < NWS; ++s)
+        while (done[s] < gb - (kNB - 2)) {
+        }
+
+      float *cm_p = cmring + ((size_t)g * ring_rows + slot) * k.nseg + sg;
+      uint32_t *fl_p = flags + ((size_t)g * ring_rows + slot) * k.nseg + sg;
+      const int step_stride = FPS * ring_rows * k.nseg;
+      for (int s = 0; s < nsteps; ++s) {
+        issue();
+        asm volatile("cp.async.wait_group %0;" ::"n"(kRingD - 1) : "memory");
+        const int fl = s * FPS + g;
+        const bool act = active && fl < nf;
+        if (__any_sync(FULL, act)) {
+          float c = 0.f, amax = __int_as_float(0xff800000);
+          if constexpr (MODE == 0) {
+            // ================= exact median common mode (north_star (a)) =================
+            float b[N];
+            float sb0 = 0.f, sb1 = 0.f;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+              uint32_t w[V / 2];
+              VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
+#pragma unroll
+              for (int h = 0; h < CH; ++h) {
+                float pd[CS], rr[CS];
+                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), pd);
+                lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+#pragma unroll
+                for (int e = 0; e < CS; e += 2) {
+                  const uint32_t ww = w[(h * CS + e) / 2];
+                  const float a0 = (u16lo_to_f(ww) - pd[e]) * rr[e];
+                  const float a1 = (u16hi_to_f(ww) - pd[e + 1]) * rr[e + 1];
+                  const int j = v * V + h * CS + e;
+                  b[j] = fabsf(a0) < T_cm ? a0 : BIG;          // pixels WITHOUT signal keep their value
+                  b[j + 1] = fabsf(a1) < T_cm ? a1 : BIG;
+                  sb0 += b[j];
+                  sb1 += b[j + 1];
+                  amax = max3(amax, a0, a1);
+                }
+              }
+            }
+            // sum of the masked values and their count from ONE accumulation: sum(b) = s + n_out * BIG with
+            // |s| < BIG/2 (BIG >= 4*N*T_cm); decoded per lane, then reduced over the group
+            const float sb = sb0 + sb1;
+            const float n_out_l = rintf(sb * (1.f / BIG));
+            const float s_l = fmaf(-n_out_l, BIG, sb);
+            const int n = LPS * N - (int)group_count<LPS>(n_out_l);
+            const float tot = group_sum<LPS>(s_l);
+            const bool need = act && n >= k.cm_min_count && n > 0;
+            const float mean = tot * rcp_approx(fmaxf((float)n, 1.f));
+            c = group_median<N, LPS>(b, n, mean, T_cm, BIG, need, apr);
+            if (!need) c = 0.f;
+          } else {
+            // ================= guarded mean or no common mode =================
+            float n0 = 0.f, n1 = 0.f, s0 = 0.f, s1 = 0.f;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+              uint32_t w[V / 2];
+              VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
+#pragma unroll
+              for (int h = 0; h < CH; ++h) {
+                float pd[CS], rr[CS];
+                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), pd);
+                lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+#pragma unroll
+                for (int e = 0; e < CS; e += 2) {
+                  const uint32_t ww = w[(h * CS + e) / 2];
+                  const float a0 = (u16lo_to_f(ww) - pd[e]) * rr[e];
+                  const float a1 = (u16hi_to_f(ww) - pd[e + 1]) * rr[e + 1];
+                  if constexpr (MODE == 1) {
+                    const float m0 = set_lt_abs(a0, T_cm), m1 = set_lt_abs(a1, T_cm);
+                    n0 += m0, n1 += m1;
+                    s0 = fmaf(m0, a0, s0), s1 = fmaf(m1, a1, s1);
+                  }
+                  amax = max3(amax, a0, a1);
+                }
+              }
+            }
+            if constexpr (MODE == 1) {
+              const float n = group_count<LPS>(n0 + n1);
+              const float tot = group_sum<LPS>(s0 + s1);
+              c = __fdiv_rn(tot, fmaxf(n, k.sqrtS));
+            }
+          }
+          // ---- publish: common-mode estimate and one candidate flag per lane ----
+          const unsigned bal = __ballot_sync(FULL, act && amax > k.cand_thr + c);
+          if (act && l == 0) {
+            *cm_p = c;
+            *fl_p = LPS == 32 ? bal : (bal >> (g * LPS)) & ((1u << (LPS & 31)) - 1u);
+            if (k.cm_keep)   // debug only
+              k.cm_keep[(((size_t)(fs + c0 + fl) * k.P + p) * k.H + row) * k.nseg + sg] = c;
+          }
+        }
+        rslot = rslot + kStepBytes == kRingD * kStepBytes ? 0u : rslot + kStepBytes;
+        cm_p += step_stride;
+        fl_p += step_stride;
+      }
+      // ---- arrive (release) on every sparse warp's barrier of this band slot ----
+      __syncwarp();
+      if (lane < NWS) mbar_arrive(bar + (gb % kNB) * NWS + lane);
+    }
+  }
+}
+
+}  // namespace pdp

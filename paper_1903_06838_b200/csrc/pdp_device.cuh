@@ -103,6 +103,20 @@ __device__ __forceinline__ float set_lt(float a, float b) {  // 1.0f if a < b el
   return d;
 }
 
+// ----------------------------------------------------------------------------------------------
+// what the exact (fp64) evaluation of a seed candidate returns, and the photon count
+// ----------------------------------------------------------------------------------------------
+struct Exact9 {
+  bool seed;
+  double E, sx, sy;
+};
+
+__device__ __forceinline__ int photon_count(double E, double E_ph) {
+  // division by the single-photon gain, rounding to the nearest integer (half-to-even), >= 0
+  const double r = rint(E / E_ph);
+  return r > 0.0 ? (r > 2147483647.0 ? 2147483647 : (int)r) : 0;
+}
+
 template <int N>
 __device__ __forceinline__ int warp_count_below(const float (&b)[N], float p) {
   float c0 = 0.f, c1 = 0.f, c2 = 0.f;  // exact small integers in fp32; three chains for ILP

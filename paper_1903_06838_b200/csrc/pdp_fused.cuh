@@ -58,11 +58,6 @@ struct KParams {
   uint32_t stage_bytes, off_v1, off_ctab, off_cand, off_accum, off_misc;
 };
 
-struct Exact9 {
-  bool seed;
-  double E, sx, sy;
-};
-
 // Exact fp64 evaluation of the 3x3 window of pixel (row, col) of panel p: the seed rule, the
 // charge sum and the centroid sums, term by term in row-major window order.
 __device__ __forceinline__ Exact9 exact9(const KParams &k, const uint16_t *tile, const float *ctab, int p,
@@ -106,10 +101,6 @@ __device__ __forceinline__ Exact9 exact9(const KParams &k, const uint16_t *tile,
   return o;
 }
 
-__device__ __forceinline__ int photon_count(double E, double E_ph) {
-  const double rn = rint(E / E_ph);  // round-half-even
-  return rn > 0.0 ? (rn > 2147483647.0 ? 2147483647 : (int)rn) : 0;
-}
 
 template <int V>
 struct VecLoad;

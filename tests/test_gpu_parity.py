@@ -19,28 +19,32 @@ from paper_1903_06838_b200 import binding, build, synth  # noqa: E402
 
 build.build()
 DEV = "cuda"
-LAUNCHES_PER_CALL = 1      # kernels one pdp_process call enqueues
+LAUNCHES_PER_CALL = 2      # kernels one pdp_process call enqueues on the throughput path (chain + accumulated image)
 
 
 def small(cfg_id, **kw):
     return dataclasses.replace(synth.CONFIGS[cfg_id], **kw)
 
 
+KERNELS = {None: 0, "auto": 0, "lookback": 1, "chain": 2}
+LAUNCHES = {"lookback": 1, "chain": 2}       # chain kernel + accumulated-image pass
+
+
 def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=False, host_chunk=None,
-            n_calls=1, kernel=None):
-    # the library picks its kernel by batch size (frame-owner for large batches, band x chunk with
-    # look-back for small ones); PDP_KERNEL pins one so that both are tested on every case
-    os.environ.pop("PDP_KERNEL", None)
-    os.environ.pop("PDP_PREFILTER", None)
-    if kernel == "frames_pf":                      # frame-owner kernel with the fp16 pre-filter tile
-        os.environ["PDP_KERNEL"] = "frames"
-        os.environ["PDP_PREFILTER"] = "1"
-    elif kernel:
-        os.environ["PDP_KERNEL"] = kernel
+            n_calls=1, kernel=None, variant=0, sparse_warps=0, chunk_frames=0):
+    # the library picks its kernel by batch size (frame-owner throughput kernel for large batches, band x
+    # chunk items with look-back for small ones); pdp_debug_set pins one so that both are tested on every case
     ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols,
                           max_frames_per_batch=max(1, raw.shape[0]), pedestal=ped.cpu(), gain=gain.cpu(),
                           seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu,
                           cm_mode=cm_mode, cm_min_count=cm_min_count)
+    ctx.debug_set("kernel", KERNELS[kernel])
+    if variant:
+        ctx.debug_set("variant", variant)
+    if sparse_warps:
+        ctx.debug_set("sparse_warps", sparse_warps)
+    if chunk_frames:
+        ctx.debug_set("chunk_frames", chunk_frames)
     if keep_cm:
         ctx.keep_common_mode(True)
     out = binding.alloc_output(raw.shape[0], cfg.npix, cap or cfg.max_hits, DEV)
@@ -57,9 +61,8 @@ def gpu_run(cfg, raw, ped, gain, cm_mode, *, cap=None, cm_min_count=0, keep_cm=F
     if keep_cm:
         res["cm"] = ctx.common_mode(raw.shape[0]).cpu().numpy()
     res["launches"] = ctx.last_launch_count
+    res["kernel"] = ctx.last_kernel_name
     ctx.close()
-    os.environ.pop("PDP_KERNEL", None)
-    os.environ.pop("PDP_PREFILTER", None)
     return res
 
 
@@ -90,7 +93,7 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("kernel", ["stream", "frames", "frames_pf", "lookback"])
+@pytest.mark.parametrize("kernel", ["chain", "lookback"])
 @pytest.mark.parametrize("cm_mode", [0, 1, 2], ids=["median", "mean", "none"])
 @pytest.mark.parametrize("case", list(CASES), ids=list(CASES))
 def test_parity(oracle, case, cm_mode, kernel):
@@ -103,15 +106,51 @@ def test_parity(oracle, case, cm_mode, kernel):
     assert rep.ok, rep.failures[:10]
     assert rep.hits_oracle > 0
     assert rep.exempt_hits <= max(3, rep.hits_oracle // 200)       # exemptions stay rare
-    assert g["status"][0] == 0 and g["launches"] == 1
+    assert g["status"][0] == 0 and g["launches"] == LAUNCHES[kernel]
+    assert g["kernel"].startswith("pdp_chain_kernel" if kernel == "chain" else "pdp_fused_kernel")
+
+
+# layouts of the throughput kernel (V pixels per vector, NV vectors per lane, LPS lanes per row segment):
+# every layout that covers the geometry must give bit-identical results
+VARIANTS = {
+    "epix_704x768": (80608, 80316, 80232, 80332),
+    "lcls2_2x70x512": (80408, 80216, 80132, 80416),
+    "dense_96x1024": (80416, 80232, 80332),
+    "tiny_185x388": (21308, 20432, 20832),
+    "narrow_5x60_s30": (20132, 20232),
+    "single_segment_40x256": (80408, 80132, 80216),
+}
 
 
 @pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
-def test_common_mode_values(oracle, cm_mode):
-    """c of every segment against the oracle: the kernel's fp32 order statistic / mean."""
-    cfg, n = small(1, rows=64), 2
+@pytest.mark.parametrize("case", list(VARIANTS), ids=list(VARIANTS))
+def test_chain_layout_variants(oracle, case, cm_mode):
+    cfg, n = CASES[case]
+    n = 2 * n + 1
     raw, ped, gain = make(cfg, n)
-    g = gpu_run(cfg, raw, ped, gain, cm_mode, keep_cm=True)
+    o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+    ref = None
+    for variant in VARIANTS[case]:
+        for sw in (4, 8):
+            g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel="chain", variant=variant, sparse_warps=sw)
+            rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
+            print(case, cm_mode, variant, sw, g["kernel"], rep.summary())
+            assert rep.ok, (variant, sw, rep.failures[:10])
+            assert "%d,%d,%d" % (variant // 10000, variant // 100 % 100, variant % 100) in g["kernel"]
+            if ref is None:
+                ref = g
+            elif cm_mode == 0:    # the median is an order statistic: identical in every layout
+                for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
+                    assert np.array_equal(ref[k], g[k]), (variant, sw, k)
+
+
+@pytest.mark.parametrize("kernel,variant", [("chain", 0), ("chain", 80316), ("chain", 80232), ("lookback", 0)])
+@pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
+def test_common_mode_values(oracle, cm_mode, kernel, variant):
+    """c of every segment against the oracle: the kernel's fp32 order statistic / mean."""
+    cfg, n = small(1, rows=64), 5
+    raw, ped, gain = make(cfg, n)
+    g = gpu_run(cfg, raw, ped, gain, cm_mode, keep_cm=True, kernel=kernel, variant=variant)
     o = oracle.process(raw.cpu().numpy(), ped.cpu().numpy(), gain.cpu().numpy(), panels=1, rows=cfg.rows,
                        cols=cfg.cols, seg_cols=cfg.seg_cols, seed_adu=50, cm_adu=20, photon_adu=80,
                        cm_mode=cm_mode, want_cm=True, want_fragile=True)
@@ -135,9 +174,9 @@ def test_integer_exact_suite(oracle):
     sig = sig + ph2 * rng.choice([0, 20, 60], (n, P, H, W))                  # neighbours, ties
     raw = torch.tensor((ped.numpy() + gain.numpy() * sig).astype(np.uint16))
     cfg = small(0, panels=P, rows=H, cols=W, seg_cols=S, seed_adu=50.5, cm_adu=20.5, photon_adu=100.0)
-    for cm_mode, kernel in ((0, "stream"), (1, "stream"), (2, "stream"), (0, "frames"), (0, "frames_pf"), (0, "lookback"),
-                            (1, "frames"), (2, "frames_pf"), (2, "lookback")):
-        g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel)
+    for cm_mode, kernel, variant in ((0, "chain", 0), (1, "chain", 0), (2, "chain", 0), (0, "lookback", 0), (2, "lookback", 0),
+                                     (0, "chain", 80132), (0, "chain", 80216), (1, "chain", 80216)):
+        g = gpu_run(cfg, raw.to(DEV), ped, gain, cm_mode, kernel=kernel, variant=variant)
         o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
         rep = compare(o, g, panels=P, rows=H, cols=W, seg_cols=S, cm_adu=cfg.cm_adu)
         print(cm_mode, kernel, rep.summary())
@@ -149,7 +188,7 @@ def test_integer_exact_suite(oracle):
         assert rep.hits_oracle > 200
 
 
-@pytest.mark.parametrize("kernel", ["stream", "frames", "lookback"])
+@pytest.mark.parametrize("kernel", ["chain", "lookback"])
 def test_overflow_and_empty(oracle, kernel):
     cfg, n = small(0, rows=40, cols=128, seg_cols=64, occupancy=0.03), 3
     raw, ped, gain = make(cfg, n)
@@ -174,27 +213,29 @@ def test_overflow_and_empty(oracle, kernel):
     ctx.close()
 
 
-def test_chunking_determinism_accumulation_and_host_feed(oracle, monkeypatch):
+def test_chunking_determinism_accumulation_and_host_feed(oracle):
     cfg, n = small(0, rows=50, cols=128, seg_cols=64, occupancy=0.02), 21
     raw, ped, gain = make(cfg, n)
-    ref = gpu_run(cfg, raw, ped, gain, 0, kernel="stream")
-    again = gpu_run(cfg, raw, ped, gain, 0, kernel="stream")
-    staged = gpu_run(cfg, raw, ped, gain, 0, kernel="frames")
-    for k in ref:
-        assert np.array_equal(ref[k], staged[k]), k                          # both large-batch kernels agree bit for bit
-    for k in ref:
+    OUT = ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum", "status")
+    ref = gpu_run(cfg, raw, ped, gain, 0, kernel="chain")
+    again = gpu_run(cfg, raw, ped, gain, 0, kernel="chain")
+    for k in OUT:
         assert np.array_equal(ref[k], again[k]), k                           # bit-identical run to run
-    monkeypatch.setenv("PDP_CHUNK_FRAMES", "4")                              # 6 chunks, ragged last one
-    chunked = gpu_run(cfg, raw, ped, gain, 0, kernel="lookback")
-    for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
-        assert np.array_equal(ref[k], chunked[k]), k
-    monkeypatch.delenv("PDP_CHUNK_FRAMES")
-    twice = gpu_run(cfg, raw, ped, gain, 0, n_calls=2)                       # accum persists across calls
+    small_k = gpu_run(cfg, raw, ped, gain, 0, kernel="lookback")
+    chunked = gpu_run(cfg, raw, ped, gain, 0, kernel="lookback", chunk_frames=4)   # 6 chunks, ragged last one
+    for k in OUT:
+        assert np.array_equal(small_k[k], chunked[k]), k
+    # the two kernels calibrate with different (equally accurate) fp32 formulas: same hits, floats within tolerance
+    for k in ("hit_count", "hit_pixel", "hit_nphot", "frame_photons", "accum"):
+        assert np.array_equal(ref[k], small_k[k]), k
+    twice = gpu_run(cfg, raw, ped, gain, 0, n_calls=2, kernel="chain")        # accum persists across calls
     assert np.array_equal(twice["accum"], 2 * ref["accum"])
-    host = gpu_run(cfg, raw, ped, gain, 0, host_chunk=8)                     # 3 chunks through the side stream
-    for k in ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum"):
+    twice = gpu_run(cfg, raw, ped, gain, 0, n_calls=2, kernel="lookback")
+    assert np.array_equal(twice["accum"], 2 * ref["accum"])
+    host = gpu_run(cfg, raw, ped, gain, 0, host_chunk=8, kernel="chain")     # 3 chunks through the side stream
+    for k in OUT:
         assert np.array_equal(ref[k], host[k]), k
-    assert host["launches"] == 3
+    assert host["launches"] == 3 * LAUNCHES["chain"]
     o = oracle_run(oracle, cfg, raw, ped, gain, 0)
     assert compare(o, ref, panels=1, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu).ok
 
@@ -208,10 +249,10 @@ def test_occupancy_independence_of_lists(oracle):
 
 
 @pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
-def test_many_frames_prefilter(oracle, cm_mode):
+def test_many_frames_dense(oracle, cm_mode):
     cfg, n = small(3, rows=50, cols=256, seg_cols=128), 300     # dense, wide clouds: many non-maximum candidates
     raw, ped, gain = make(cfg, n)
-    g = gpu_run(cfg, raw, ped, gain, cm_mode, kernel="frames_pf")
+    g = gpu_run(cfg, raw, ped, gain, cm_mode, sparse_warps=8)
     o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
     rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(rep.summary())
@@ -363,7 +404,7 @@ def test_full_size_config0(oracle):
         assert rep.hits_oracle > 20000 and rep.exempt_hits <= rep.hits_oracle // 200
 
 
-@pytest.mark.parametrize("kernel", ["stream", "lookback"])
+@pytest.mark.parametrize("kernel", ["chain", "lookback"])
 def test_seed_threshold_below_mask_threshold(oracle, kernel):
     """T_seed < T_cm: pixels INSIDE the common-mode mask can seed (the kernels' rare 'low' candidate path)."""
     cfg, n = small(0, rows=40, cols=256, seg_cols=128, occupancy=0.01, photon_adu=30.0, seed_adu=12.0), 80
@@ -382,7 +423,7 @@ def test_wide_gain_range_and_min_count(oracle):
     cfg, n = small(4, panels=1, rows=48, gain_lo=0.25, gain_hi=4.0), 90
     raw, ped, gain = make(cfg, n)
     for cm_min_count in (0, 250):
-        g = gpu_run(cfg, raw, ped, gain, 0, cm_min_count=cm_min_count, kernel="stream")
+        g = gpu_run(cfg, raw, ped, gain, 0, cm_min_count=cm_min_count, kernel="chain")
         o = oracle_run(oracle, cfg, raw, ped, gain, 0, cm_min_count=cm_min_count)
         rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
         print(cm_min_count, rep.summary())
@@ -390,9 +431,8 @@ def test_wide_gain_range_and_min_count(oracle):
         assert rep.hits_oracle > 1000 and rep.exempt_hits <= max(3, rep.hits_oracle // 200)
 
 
-def test_wide_panel_falls_back_to_staged_kernel(oracle):
-    """W = 1280 (> 1024 columns: more than 32 bitmap words per row) is outside the streaming kernel's
-    geometry; a large batch must then run on the staged frame-owner kernel with identical results."""
+def test_wide_panel(oracle):
+    """W = 1280 (40 bitmap words per row, S = 640: padded lane runs) on the throughput kernel."""
     cfg, n = small(0, rows=24, cols=1280, seg_cols=640, occupancy=0.004), 90
     raw, ped, gain = make(cfg, n)
     g = gpu_run(cfg, raw, ped, gain, 0)                 # auto choice
@@ -400,6 +440,6 @@ def test_wide_panel_falls_back_to_staged_kernel(oracle):
     rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
     print(rep.summary())
     assert rep.ok, rep.failures[:10]
-    assert rep.hits_oracle > 3000 and g["launches"] == 1
+    assert rep.hits_oracle > 3000 and g["kernel"].startswith("pdp_chain_kernel")
     with pytest.raises(binding.PdpError):
-        gpu_run(cfg, raw, ped, gain, 0, kernel="stream")   # pinning the streaming kernel must fail loudly
+        gpu_run(cfg, raw, ped, gain, 0, kernel="chain", variant=80608)   # a layout that cannot cover S = 640 must fail loudly
