@@ -164,6 +164,45 @@ int pdp_process_pinned(pdp_ctx *ctx, const uint16_t *pinned_host, int32_t n_fram
 int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
                      int32_t chunk_frames, void *cuda_stream, const pdp_output *out);
 
+/*
+ * pdp_process_dense — dense photon counting for areas of high flux ("areas with high photon fluxes can
+ * be converted easily to photon counting images by division with the expected single photon gain followed by
+ * rounding to the nearest integer"): for every pixel of every frame of the batch (DEVICE pointer, as pdp_process)
+ *     v2 = (raw - pedestal) / gain - c          (c: the context's common-mode estimator on row segments)
+ *     n  = v2 < zero_below_adu ? 0 : max(0, rint(v2 / photon_adu))        (round-half-even)
+ * image[idx] += n (DEVICE uint32 [P*H*W], the photon-counting image of PAPER.md:L99, persists across calls, caller
+ * zeroes) and, when frame_totals is not NULL, frame_totals[f] = sum of n over frame f (DEVICE uint32 [n_frames]).
+ * zero_below_adu is the "zeroing the signal of pixels within noise" of PAPER.md:L91; pass -INFINITY for none.
+ * Asynchronous on `cuda_stream`.  No atomics on global memory: a warp owns a row segment for all frames.
+ * Errors: PDP_E_NULL, PDP_E_BATCH, PDP_E_ALIGN, PDP_E_VALUE (NaN), PDP_E_GEOMETRY, PDP_E_CUDA.
+ */
+int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *raw_u16_batch, void *cuda_stream, float zero_below_adu,
+                      uint32_t *image, uint32_t *frame_totals);
+
+/*
+ * Histogram summarization of finished hit lists ("functions for histogramming"; L109 Fig. 7: the
+ * spectrum of the summed charge; L113 Fig. 8: the histogram of the centroids).  Uniform bins
+ * [lo + b*width, lo + (b+1)*width), b = 0 .. nbins-1; the bin of a value x is floor((x - lo) / width) evaluated in
+ * double on the float32 value stored in the list; values outside [lo, lo + nbins*width) are dropped.
+ */
+typedef struct pdp_hist_spec {
+  float lo, width; /* width > 0 */
+  int32_t nbins;   /* 1 .. 16384 */
+} pdp_hist_spec;
+
+/*
+ * pdp_histograms — enqueue on `cuda_stream`: hist_energy[b] += number of listed hits of the n_frames frames of
+ * `lists` (a pdp_output filled by pdp_process; only hit_capacity, hit_count, hit_charge, hit_dx, hit_dy are read)
+ * whose summed charge E falls into bin b of `energy`; hist_dx / hist_dy likewise for the centroid offsets with the
+ * bins of `dxy`.  Histograms are DEVICE uint32 arrays of nbins words, caller-owned, += (the caller zeroes them
+ * when a run starts).  Either spec may be NULL (that histogram is skipped).  Only hits stored in the lists count
+ * (the first hit_capacity of a frame).  No global atomics: privatised shared-memory histograms, merged by bin
+ * ownership.  Errors: PDP_E_NULL, PDP_E_VALUE (width <= 0, nbins out of range), PDP_E_BATCH, PDP_E_CUDA.
+ */
+int pdp_histograms(pdp_ctx *ctx, const pdp_output *lists, int32_t n_frames, const pdp_hist_spec *energy,
+                   uint32_t *hist_energy, const pdp_hist_spec *dxy, uint32_t *hist_dx, uint32_t *hist_dy,
+                   void *cuda_stream);
+
 /* pdp_set_params — replace thresholds / estimator of an existing context
  * (host struct, validated as in pdp_create).  Must not race with pdp_process. */
 int pdp_set_params(pdp_ctx *ctx, const pdp_params *params);
@@ -187,8 +226,8 @@ const char *pdp_last_kernel_name(const pdp_ctx *ctx);
  *                   2 the throughput kernel (frame-owner CTAs); PDP_E_GEOMETRY at the next pdp_process if the
  *                   geometry does not fit it;
  *   "chunk_frames"  frames per work item of the small-batch kernel (0 = automatic);
- *   "sparse_warps"  0 automatic (from the hit density of earlier calls), 4 or 8: warps of the throughput
- *                   kernel that evaluate seed candidates;
+ *   "sparse_warps"  0 default, 4 or 8: warps of the throughput kernel that evaluate seed candidates (8 for data
+ *                   with percents of the pixels above the seed threshold);
  *   "variant"       V*10000 + NV*100 + LPS: pin the throughput kernel's layout (pixels per vector, vectors per
  *                   lane, lanes per row segment), 0 = automatic; PDP_E_GEOMETRY if it does not cover seg_cols.
  * None of them changes any output.  Errors: PDP_E_NULL, PDP_E_VALUE (unknown key / value).

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpdp.so")
 CM_MEDIAN, CM_MEAN_GUARDED, CM_NONE = 0, 1, 2
 STATUS_HIT_OVERFLOW = 1
 
-EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_set_params", "pdp_destroy",
+EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_histograms", "pdp_process_dense", "pdp_set_params", "pdp_destroy",
            "pdp_last_launch_count", "pdp_last_kernel_name", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
            "pdp_last_error", "pdp_version")
 
@@ -42,6 +42,10 @@ class pdp_output(ctypes.Structure):
                 ("hit_pixel", ctypes.c_void_p), ("hit_charge", ctypes.c_void_p),
                 ("hit_nphot", ctypes.c_void_p), ("hit_dx", ctypes.c_void_p), ("hit_dy", ctypes.c_void_p),
                 ("frame_photons", ctypes.c_void_p), ("accum", ctypes.c_void_p), ("status", ctypes.c_void_p)]
+
+
+class pdp_hist_spec(ctypes.Structure):
+    _fields_ = [("lo", ctypes.c_float), ("width", ctypes.c_float), ("nbins", ctypes.c_int32)]
 
 
 class PdpError(RuntimeError):
@@ -72,6 +76,11 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.pdp_process_pinned.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
                                        ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(pdp_output)]
     lib.pdp_debug_set.argtypes = [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]
+    lib.pdp_histograms.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_output), ctypes.c_int32, ctypes.POINTER(pdp_hist_spec),
+                                   ctypes.c_void_p, ctypes.POINTER(pdp_hist_spec), ctypes.c_void_p, ctypes.c_void_p,
+                                   ctypes.c_void_p]
+    lib.pdp_process_dense.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_batch), ctypes.c_void_p, ctypes.c_float,
+                                      ctypes.c_void_p, ctypes.c_void_p]
     lib.pdp_set_params.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_params)]
     lib.pdp_destroy.argtypes = [ctypes.c_void_p]
     lib.pdp_last_launch_count.argtypes = [ctypes.c_void_p]
@@ -186,6 +195,29 @@ class Context:
         cs = ctypes.c_void_p(copy_stream.cuda_stream) if copy_stream is not None else None
         self._check(self._lib.pdp_process_pinned(self._h, raw_host.data_ptr(), n, chunk_frames,
                                                  ctypes.c_void_p(s.cuda_stream), cs, ctypes.byref(o)), "pdp_process_pinned")
+
+    def histograms(self, out: Output, n_frames: int, *, energy=None, dxy=None, hist_energy=None, hist_dx=None,
+                   hist_dy=None, stream: torch.cuda.Stream | None = None):
+        """energy / dxy: (lo, width, nbins) or None; histograms: CUDA int32 tensors of nbins words, += (pdp_histograms)."""
+        s = stream if stream is not None else torch.cuda.current_stream()
+        o = out.c_struct()
+        es = pdp_hist_spec(*energy) if energy is not None else None
+        ds = pdp_hist_spec(*dxy) if dxy is not None else None
+        ptr = lambda t: t.data_ptr() if t is not None else None
+        self._check(self._lib.pdp_histograms(self._h, ctypes.byref(o), n_frames, ctypes.byref(es) if es else None,
+                                             ptr(hist_energy), ctypes.byref(ds) if ds else None, ptr(hist_dx),
+                                             ptr(hist_dy), ctypes.c_void_p(s.cuda_stream)), "pdp_histograms")
+
+    def process_dense(self, raw: torch.Tensor, image: torch.Tensor, frame_totals: torch.Tensor | None = None,
+                      zero_below_adu: float = float("-inf"), stream: torch.cuda.Stream | None = None):
+        """Dense photon counting (pdp_process_dense): image int32[npix] +=, frame_totals int32[n] or None."""
+        if not raw.is_cuda or not raw.is_contiguous() or raw.element_size() != 2:
+            raise ValueError("raw must be a contiguous CUDA tensor of 16-bit elements")
+        s = stream if stream is not None else torch.cuda.current_stream(raw.device)
+        b = pdp_batch(raw.data_ptr(), raw.numel() // self.npix)
+        self._check(self._lib.pdp_process_dense(self._h, ctypes.byref(b), ctypes.c_void_p(s.cuda_stream), zero_below_adu,
+                                                image.data_ptr(), frame_totals.data_ptr() if frame_totals is not None else None),
+                    "pdp_process_dense")
 
     def debug_set(self, key: str, value: int):
         """Diagnostic switches of include/pdp.h (kernel, chunk_frames, sparse_warps, variant)."""

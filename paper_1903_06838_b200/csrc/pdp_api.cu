@@ -11,6 +11,7 @@
 
 #include "../../include/pdp.h"
 #include "pdp_chain.cuh"
+#include "pdp_dense.cuh"
 #include "pdp_fused.cuh"
 #include "pdp_post.cuh"
 
@@ -23,14 +24,16 @@ using ChainFn = void (*)(const CParams);
 ChainFn chain_lookup_v8(int nv, int lps, int mode);   // pdp_chain_v8.cu
 ChainFn chain_lookup_v4(int nv, int lps, int mode);   // pdp_chain_v4.cu
 ChainFn chain_lookup_v2(int nv, int lps, int mode);   // pdp_chain_v2.cu
+using DenseFn = void (*)(const DParams);
+DenseFn dense_lookup_v8(int nv, int mode);
+DenseFn dense_lookup_v4(int nv, int mode);
+DenseFn dense_lookup_v2(int nv, int mode);
 }  // namespace pdp
 
 namespace {
 
 thread_local std::string g_last_error;  // errors raised before a context exists
 
-constexpr int kStatsSlots = 1 + 256 * pdp::kMaxSparseWarps;   // pixels, then seeds per (CTA, sparse warp)
-constexpr size_t kStatsBytes = kStatsSlots * sizeof(unsigned long long);
 
 // small-batch kernel (pdp_fused.cuh): band x chunk items with decoupled look-back
 struct LaunchPlan {
@@ -48,8 +51,8 @@ struct ChainVariant {
 struct ChainPlan {
   bool ok = false;
   ChainVariant v{0, 0, 0};
-  int R = 0, NWD = 0, NWS = 0, WPR = 0, bands_per_panel = 0, n_bands = 0;
-  uint32_t off_cm = 0, off_flag = 0, off_bar = 0, off_done = 0, off_pref = 0, off_phot = 0, off_sparse = 0,
+  int R = 0, NWD = 0, NWS = 0, NB = 0, bands_per_panel = 0, n_bands = 0;
+  uint32_t off_cm = 0, off_flag = 0, off_done = 0, off_pref = 0, off_phot = 0, off_sparse = 0,
            sparse_stride = 0, off_ring = 0, off_maps = 0, ring_warp_bytes = 0, maps_warp_bytes = 0, smem = 0;
 };
 
@@ -79,22 +82,23 @@ struct pdp_ctx {
   size_t smem_limit = 0;
   size_t npix = 0;
   float *d_ped = nullptr, *d_gain = nullptr, *d_rg = nullptr;
-  float *d_K = nullptr, *d_npf = nullptr;   // small-batch kernel: 2^23 + rint(ped), -(ped - rint(ped))/gain
+  float *d_K = nullptr, *d_npf = nullptr;   // dense passes: 2^23 + rint(ped), -(ped - rint(ped))/gain
   double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
-  unsigned long long *d_stats = nullptr;    // written by the throughput kernel: [0] pixels, [1..] seeds per sparse warp
-  unsigned long long *h_stats = nullptr;    // pinned copy, refreshed asynchronously after every launch
-  double density = 0.0;                     // seeds per pixel of the last launch whose statistics have arrived
+  uint32_t *d_dense_ws = nullptr;           // per-CTA partial frame totals (pdp_process_dense), grown on demand
+  size_t dense_ws_words = 0;
+  uint32_t *d_hist_ws = nullptr;            // per-CTA partial histograms (pdp_histograms), grown on demand
+  size_t hist_ws_words = 0;
   float *d_cm = nullptr;                    // optional kept common-mode estimates
   int keep_cm = 0;
   int64_t cm_frames = 0;                    // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
   ChainPlan cplan[2];                       // [0] 4 sparse warps (sparse data), [1] 8 sparse warps (dense data)
+  int sparse_override = 0;                  // pdp_debug_set("sparse_warps"): 0 default (4), 4, 8
   ChainVariant forced{0, 0, 0};             // pdp_debug_set("variant")
   int kernel_override = 0;                  // pdp_debug_set("kernel"): 0 auto, 1 look-back kernel, 2 throughput kernel
   int chunk_frames_override = 0;            // pdp_debug_set("chunk_frames")
-  int sparse_override = 0;                  // pdp_debug_set("sparse_warps"): 0 auto, 4, 8
   // host-feed state
   uint16_t *d_feed[2] = {nullptr, nullptr};
   int64_t feed_frames = 0;
@@ -217,34 +221,32 @@ bool make_plan_chain(const pdp_geometry &g, const ChainVariant &v, int dense_war
   const int nseg = g.cols / g.seg_cols;
   const int N = v.V * v.NV;
   if (v.V * v.NV * v.LPS < g.seg_cols || nseg > dense_warps_max) return false;
-  const int WPR = (g.cols + 31) / 32;
-  if (WPR > 64) return false;   // the per-row summary of non-zero bitmap words is one 64-bit word
+  if (nseg > 255 || g.cols >= (1 << 20)) return false;   // packed item / candidate descriptors
+  const int NB = nws + 3;       // band slots of the rings: every sparse warp can own a band in flight, plus slack
   auto al = [](uint32_t x) { return (x + 127u) & ~127u; };
   for (int R = std::min(std::min(dense_warps_max / nseg, (int)g.rows), 254); R >= 1; --R) {
     if (R < 2 && g.rows > 1) return false;   // the sparse stage needs the previous band's last two rows in the ring
-    const uint32_t ring = (uint32_t)pdp::kNB * (uint32_t)R;
+    const uint32_t ring = (uint32_t)NB * (uint32_t)R;
     const int NWD = R * nseg;
-    const uint32_t gfmax = (uint32_t)((pdp::kFCH + nws - 1) / nws);
     uint32_t off = 0;
     pl.off_cm = off;      off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
-    pl.off_flag = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
-    pl.off_bar = off;     off = al(off + (uint32_t)pdp::kNB * (uint32_t)nws * 8u);
-    pl.off_done = off;    off = al(off + (uint32_t)nws * 4u);
+    pl.off_flag = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 8u);
+    pl.off_done = off;    off = al(off + 16u);
     pl.off_pref = off;    off = al(off + pdp::kFCH * 4u);
     pl.off_phot = off;    off = al(off + pdp::kFCH * 4u);
-    pl.sparse_stride = al((uint32_t)(pdp::kListCap + pdp::kItemCap) * 4u + gfmax * (uint32_t)(R + 1) * 8u +
-                          gfmax * (uint32_t)(R + 1) * (uint32_t)WPR * 4u);
+    // per sparse warp: item list + masks, candidate list, seed buffer (6 words per seed), per-frame working totals
+    pl.sparse_stride = al((uint32_t)(2 * pdp::kItemCap + pdp::kListCap + 6 * pdp::kSeedCap + 2 * pdp::kFCH) * 4u);
     pl.off_sparse = off;  off = al(off + (uint32_t)nws * pl.sparse_stride);
     pl.ring_warp_bytes = (uint32_t)pdp::kRingD * 32u * (uint32_t)N * 2u;
     pl.off_ring = off;    off = al(off + (uint32_t)NWD * pl.ring_warp_bytes);
-    pl.maps_warp_bytes = 2u * (uint32_t)v.LPS * (uint32_t)N * 4u;
+    pl.maps_warp_bytes = 3u * (uint32_t)v.LPS * (uint32_t)N * 4u;
     pl.off_maps = off;    off = al(off + (uint32_t)NWD * pl.maps_warp_bytes);
     if (off > smem_limit) continue;
     pl.v = v;
     pl.R = R;
     pl.NWD = NWD;
     pl.NWS = nws;
-    pl.WPR = WPR;
+    pl.NB = NB;
     pl.bands_per_panel = (g.rows + R - 1) / R;
     pl.n_bands = pl.bands_per_panel * g.panels;
     pl.smem = off;
@@ -284,9 +286,9 @@ void free_ctx(pdp_ctx *c) {
   cudaFree(c->d_rg64);
   cudaFree(c->d_lookback);
   cudaFree(c->d_ticket);
-  cudaFree(c->d_stats);
   cudaFree(c->d_cm);
-  if (c->h_stats) cudaFreeHost(c->h_stats);
+  cudaFree(c->d_hist_ws);
+  cudaFree(c->d_dense_ws);
   for (int i = 0; i < 2; ++i) {
     cudaFree(c->d_feed[i]);
     if (c->ev_ready[i]) cudaEventDestroy(c->ev_ready[i]);
@@ -403,6 +405,8 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->plan.smem);
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(pdp::pdp_accum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_limit);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(pdp::pdp_hist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 16384 * 4);
   if (e != cudaSuccess) {
     free_ctx(c);
     return cuda_fail(nullptr, e, "cudaFuncSetAttribute");
@@ -416,17 +420,13 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
   cudaError_t errs[] = {cudaMalloc(&c->d_ped, mb),      cudaMalloc(&c->d_gain, mb),
                         cudaMalloc(&c->d_K, mb),        cudaMalloc(&c->d_rg, mb),
                         cudaMalloc(&c->d_npf, mb),      cudaMalloc(&c->d_lookback, lb),
-                        cudaMalloc(&c->d_ticket, 256),  cudaMalloc(&c->d_stats, kStatsBytes),
-                        cudaMalloc(&c->d_rg64, npix * sizeof(double)),
-                        cudaHostAlloc(&c->h_stats, kStatsBytes, cudaHostAllocDefault)};
+                        cudaMalloc(&c->d_ticket, 256),  cudaMalloc(&c->d_rg64, npix * sizeof(double))};
   for (cudaError_t x : errs)
     if (x != cudaSuccess) {
       free_ctx(c);
       return cuda_fail(nullptr, x, "cudaMalloc");
     }
-  std::memset(c->h_stats, 0, kStatsBytes);
-  e = cudaMemset(c->d_stats, 0, kStatsBytes);
-  if (e == cudaSuccess) e = cudaMemcpy(c->d_rg64, rg64.data(), npix * sizeof(double), cudaMemcpyHostToDevice);
+  e = cudaMemcpy(c->d_rg64, rg64.data(), npix * sizeof(double), cudaMemcpyHostToDevice);
   const void *srcs[] = {ped, gain, K.data(), rg.data(), npf.data()};
   float *dsts[] = {c->d_ped, c->d_gain, c->d_K, c->d_rg, c->d_npf};
   for (int i = 0; i < 5 && e == cudaSuccess; ++i) e = cudaMemcpy(dsts[i], srcs[i], mb, cudaMemcpyHostToDevice);
@@ -511,18 +511,21 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   k.n_frames = n;
   k.ped = c->d_ped;
   k.rg = c->d_rg;
+  k.mapK = c->d_K;
+  k.mapNpf = c->d_npf;
   k.rg64 = c->d_rg64;
   k.P = c->geo.panels;
   k.H = c->geo.rows;
   k.W = c->geo.cols;
   k.S = c->geo.seg_cols;
   k.nseg = k.W / k.S;
-  k.WPR = pl.WPR;
   k.R = pl.R;
   k.bands_per_panel = pl.bands_per_panel;
   k.n_bands = pl.n_bands;
   k.NWD = pl.NWD;
   k.NWS = pl.NWS;
+  k.NB = pl.NB;
+  k.off_done = pl.off_done;
   k.T_seed = c->prm.seed_adu;
   k.T_cm = c->prm.cm_adu;
   k.E_ph = c->prm.photon_adu;
@@ -552,11 +555,8 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   k.accum = o.accum;
   k.status = o.status;
   k.cm_keep = keep_cm ? c->d_cm : nullptr;
-  k.stats = c->d_stats;
   k.off_cm = pl.off_cm;
   k.off_flag = pl.off_flag;
-  k.off_bar = pl.off_bar;
-  k.off_done = pl.off_done;
   k.off_pref = pl.off_pref;
   k.off_phot = pl.off_phot;
   k.off_sparse = pl.off_sparse;
@@ -584,9 +584,6 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   const int grid_a = (int)((c->npix + q.span - 1) / q.span);
   pdp::pdp_accum_kernel<<<grid_a, pdp::kPostThreads, (size_t)q.span * 4, st>>>(q);
   PDP_CUDA(c, cudaGetLastError());
-  // density hint for the next call: running totals, copied back asynchronously and read without waiting
-  PDP_CUDA(c, cudaMemcpyAsync(c->h_stats, c->d_stats, (1 + (size_t)grid * pdp::kMaxSparseWarps) * sizeof(unsigned long long),
-                              cudaMemcpyDeviceToHost, st));
   c->launches += 2;
   std::snprintf(c->last_kernel_buf, sizeof(c->last_kernel_buf), "pdp_chain_kernel<%d,%d,%d,%d>", pl.v.V, pl.v.NV, pl.v.LPS,
                 c->prm.cm_mode);
@@ -598,14 +595,7 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
 int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o, bool keep_cm) {
   // ---- large batches: the throughput kernel (frame-owner CTAs) ----
   {
-    // seeds per pixel seen by earlier launches (stale by design: never waits for the device)
-    if (const unsigned long long pixels = c->h_stats[0]) {
-      unsigned long long seeds = 0;
-      for (int i = 0; i < std::min(c->num_sms, 256) * pdp::kMaxSparseWarps; ++i) seeds += c->h_stats[1 + i];
-      c->density = (double)seeds / (double)pixels;
-    }
-    int which = c->density > 0.01 ? 1 : 0;   // dense data: 8 sparse warps and 12 dense ones
-    if (c->sparse_override) which = c->sparse_override == 8 ? 1 : 0;
+    int which = c->sparse_override == 8 ? 1 : 0;
     if (!c->cplan[which].ok) which ^= 1;
     const bool can = c->cplan[which].ok;
     const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
@@ -630,7 +620,6 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   k.nseg = k.W / k.S;
   k.R = pl.R;
   k.TR = pl.TR;
-  k.WPR = pl.WPR;
   k.bands_per_panel = pl.bands_per_panel;
   k.n_bands = pl.n_bands;
   // frames per work item: enough items for ~16 waves of CTAs, at least 8 frames each so that the
@@ -768,6 +757,134 @@ int pdp_process_pinned(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
 int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames, int32_t chunk_frames, void *stream,
                      const pdp_output *out) {
   return pdp_process_pinned(ctx, raw_host, n_frames, chunk_frames, stream, nullptr, out);
+}
+
+int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *batch, void *stream, float zero_below_adu, uint32_t *image,
+                      uint32_t *frame_totals) {
+  if (!ctx || !batch || !image) return fail(ctx, PDP_E_NULL, "pdp_process_dense: null argument");
+  if (batch->n_frames < 0 || batch->n_frames > ctx->geo.max_frames_per_batch)
+    return fail(ctx, PDP_E_BATCH, "pdp_process_dense: n_frames out of range");
+  if (std::isnan(zero_below_adu)) return fail(ctx, PDP_E_VALUE, "pdp_process_dense: zero_below_adu is NaN");
+  ctx->launches = 0;
+  if (batch->n_frames == 0) return PDP_OK;
+  if (!batch->data) return fail(ctx, PDP_E_NULL, "pdp_process_dense: null batch data");
+  if (reinterpret_cast<uintptr_t>(batch->data) & 15) return fail(ctx, PDP_E_ALIGN, "pdp_process_dense: batch not 16-byte aligned");
+  const int S = ctx->geo.seg_cols, W = ctx->geo.cols, n = batch->n_frames;
+  int V = 0;
+  for (int v : {8, 4, 2})
+    if (S % v == 0 && W % v == 0) {
+      V = v;
+      break;
+    }
+  int NV = (S + 32 * V - 1) / (32 * V);
+  pdp::DenseFn fn = nullptr;
+  for (; NV <= 16 && !fn; ++NV)   // the next instantiated vector count that covers S
+    fn = V == 8 ? pdp::dense_lookup_v8(NV, ctx->prm.cm_mode) : (V == 4 ? pdp::dense_lookup_v4(NV, ctx->prm.cm_mode) : pdp::dense_lookup_v2(NV, ctx->prm.cm_mode));
+  --NV;
+  if (!fn) return fail(ctx, PDP_E_GEOMETRY, "pdp_process_dense: no kernel variant covers seg_cols");
+  pdp::DParams k{};
+  k.raw = batch->data;
+  k.n_frames = n;
+  k.ped = ctx->d_ped;
+  k.rg = ctx->d_rg;
+  k.rg64 = ctx->d_rg64;
+  k.P = ctx->geo.panels;
+  k.H = ctx->geo.rows;
+  k.W = W;
+  k.S = S;
+  k.nseg = W / S;
+  k.n_tasks = k.P * k.H * k.nseg;
+  k.T_cm = ctx->prm.cm_adu;
+  k.sqrtS = (float)std::sqrt((double)S);
+  {
+    const double need = std::max(1024.0, 4.0 * (double)(V * NV) * (double)ctx->prm.cm_adu + 1.0);
+    double big = 1024.0;
+    while (big < need) big *= 2.0;
+    k.big = (float)big;
+  }
+  k.zero_below = zero_below_adu;
+  k.dzero_below = (double)zero_below_adu;
+  k.inv_Eph = (float)(1.0 / (double)ctx->prm.photon_adu);
+  k.dE_ph = (double)ctx->prm.photon_adu;
+  k.cm_mode = ctx->prm.cm_mode;
+  k.cm_min_count = ctx->prm.cm_min_count > 0 ? ctx->prm.cm_min_count : (int)std::ceil(std::sqrt((double)S));
+  k.image = image;
+  const int nwarps = pdp::kDenseThreads / 32;
+  const int grid = std::max(1, std::min(ctx->num_sms, (k.n_tasks + nwarps - 1) / nwarps));
+  const size_t tot_bytes = frame_totals ? (((size_t)n * 4 + 127) & ~(size_t)127) : 0;
+  const size_t smem = tot_bytes + (size_t)nwarps * pdp::kDenseRing * 32 * (size_t)(V * NV) * 2;
+  if (smem > ctx->smem_limit) return fail(ctx, PDP_E_BATCH, "pdp_process_dense: too many frames per call for the per-frame totals");
+  if (frame_totals) {
+    const size_t need = (size_t)grid * n;
+    if (ctx->dense_ws_words < need) {
+      cudaFree(ctx->d_dense_ws);
+      ctx->d_dense_ws = nullptr;
+      ctx->dense_ws_words = 0;
+      PDP_CUDA(ctx, cudaMalloc(&ctx->d_dense_ws, need * sizeof(uint32_t)));
+      ctx->dense_ws_words = need;
+    }
+    k.partial_totals = ctx->d_dense_ws;
+    k.frame_totals = frame_totals;
+    k.n_partials = grid;
+  }
+  PDP_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ctx->smem_limit));
+  cudaStream_t st = (cudaStream_t)stream;
+  fn<<<grid, pdp::kDenseThreads, smem, st>>>(k);
+  PDP_CUDA(ctx, cudaGetLastError());
+  ctx->launches = 1;
+  if (frame_totals) {
+    pdp::pdp_dense_totals_kernel<<<(n + 255) / 256, 256, 0, st>>>(k);
+    PDP_CUDA(ctx, cudaGetLastError());
+    ctx->launches = 2;
+  }
+  std::snprintf(ctx->last_kernel_buf, sizeof(ctx->last_kernel_buf), "pdp_dense_kernel<%d,%d,%d>", V, NV, ctx->prm.cm_mode);
+  ctx->last_kernel = ctx->last_kernel_buf;
+  return PDP_OK;
+}
+
+int pdp_histograms(pdp_ctx *ctx, const pdp_output *lists, int32_t n_frames, const pdp_hist_spec *energy,
+                   uint32_t *hist_energy, const pdp_hist_spec *dxy, uint32_t *hist_dx, uint32_t *hist_dy, void *stream) {
+  if (!ctx || !lists || !lists->hit_count || !lists->hit_charge || !lists->hit_dx || !lists->hit_dy)
+    return fail(ctx, PDP_E_NULL, "pdp_histograms: null argument");
+  if ((energy && !hist_energy) || (dxy && (!hist_dx || !hist_dy))) return fail(ctx, PDP_E_NULL, "pdp_histograms: null histogram");
+  if (n_frames < 0) return fail(ctx, PDP_E_BATCH, "pdp_histograms: n_frames < 0");
+  for (const pdp_hist_spec *s : {energy, dxy})
+    if (s && (!std::isfinite(s->lo) || !std::isfinite(s->width) || !(s->width > 0.f) || s->nbins < 1 || s->nbins > 16384))
+      return fail(ctx, PDP_E_VALUE, "pdp_histograms: invalid histogram specification");
+  ctx->launches = 0;
+  if (n_frames == 0 || (!energy && !dxy)) return PDP_OK;
+  pdp::HistParams q{};
+  q.n_frames = n_frames;
+  q.cap = lists->hit_capacity;
+  q.hit_count = lists->hit_count;
+  q.hit_charge = lists->hit_charge;
+  q.hit_dx = lists->hit_dx;
+  q.hit_dy = lists->hit_dy;
+  if (energy) q.e_lo = energy->lo, q.e_w = energy->width, q.e_bins = energy->nbins;
+  if (dxy) q.d_lo = dxy->lo, q.d_w = dxy->width, q.d_bins = dxy->nbins;
+  const int total = q.e_bins + 2 * q.d_bins;
+  const int grid = std::min(ctx->num_sms, n_frames);
+  const size_t need = (size_t)grid * total;
+  if (ctx->hist_ws_words < need) {
+    cudaFree(ctx->d_hist_ws);
+    ctx->d_hist_ws = nullptr;
+    ctx->hist_ws_words = 0;
+    PDP_CUDA(ctx, cudaMalloc(&ctx->d_hist_ws, need * sizeof(uint32_t)));
+    ctx->hist_ws_words = need;
+  }
+  q.partial = ctx->d_hist_ws;
+  q.n_partials = grid;
+  q.hist_e = hist_energy;
+  q.hist_dx = hist_dx;
+  q.hist_dy = hist_dy;
+  cudaStream_t st = (cudaStream_t)stream;
+  pdp::pdp_hist_kernel<<<grid, pdp::kPostThreads, (size_t)total * 4, st>>>(q);
+  PDP_CUDA(ctx, cudaGetLastError());
+  pdp::pdp_hist_merge_kernel<<<(total + 255) / 256, 256, 0, st>>>(q);
+  PDP_CUDA(ctx, cudaGetLastError());
+  ctx->launches = 2;
+  ctx->last_kernel = "pdp_hist_kernel";
+  return PDP_OK;
 }
 
 }  // extern "C"

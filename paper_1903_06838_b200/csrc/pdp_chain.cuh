@@ -4,23 +4,24 @@
 // kFCH frame slots, band by band (band = R rows of one panel), so the per-frame hit-list offsets are a
 // CTA-local running prefix (ordered, deterministic output without any inter-CTA exchange).
 //
-// Warp roles (no CTA-wide barrier after the prologue):
-//   * dense warps, one per (row of the band, row segment).  A warp handles FPS = 32/LPS frames at once:
+// Every warp has two jobs per band (one CTA barrier per band):
+//   * the dense pass of its (row of the band, row segment).  A warp handles FPS = 32/LPS frames at once:
 //     LPS lanes share one row segment of one frame, every lane owns a contiguous run of N = V*NV pixels
 //     in registers.  The per-segment scalar work of the exact median (pivot policy, bracket, order-statistic
 //     read-out) is therefore amortised over N pixels per lane instead of S/32, the cross-lane reductions are
 //     log2(LPS) shuffles, and lanes of different frames run the same instruction stream.
 //       raw pixels : per-lane cp.async (LDGSTS) into a lane-major ring, kRingD steps deep (each lane copies
 //                    and later reads only its own vectors: cp.async.wait_group is the only synchronisation);
-//       maps       : pedestal and 1/gain of the segment, staged once per (band, chunk) into a lane-major
+//       maps       : K, 1/gain and npf of the segment, staged once per (band, chunk) into a lane-major
 //                    tile in shared memory (conflict-free LDS.128), shared by the FPS frames of a step;
-//       calibrate  : a = (float(raw) - ped) * (1/gain)            PAPER.md:L41, L51   (I2F.U16, FADD, FMUL)
+//       calibrate  : a = fma((2^23 + raw) - K, 1/gain, npf)        PAPER.md:L41, L51   (PRMT, FADD, FFMA; K = 2^23 +
+//                    rint(ped), npf = -(ped - rint(ped))/gain: the subtraction is exact, one rounding)
 //       mask       : |a| < T_cm
 //       estimate   : exact median of the masked pixels (north_star (a)) by counting in value space, or the
 //                    paper's guarded mean sum/max(n, sqrt(S)), or none;
-//       candidates : ONE bit per lane: max(a) over the lane's run > T_seed - margin + c.
-//   * sparse warps: sleep on an mbarrier until every dense warp has published a band, then, for their frame
-//     slots: expand the flagged lane runs to pixel candidates (same fp32 formula), apply the exact fp64
+//       candidates : one flag bit per unit (about 8 pixels) of the lane's run: max(a) > T_seed - margin + c.
+//   * the sparse stage of its frame slot for the band before (published by all warps before the last barrier):
+//     expand the flagged units to pixel candidates (same fp32 formula), apply the exact fp64
 //     seed rule (strict 3x3 maximum, ties to the lower index, panel edges) to every candidate, compute E, n,
 //     dx, dy in the oracle's order of operations and emit the hits in pixel order.
 //
@@ -33,26 +34,32 @@
 namespace pdp {
 
 constexpr int kFCH = 16;          // frame slots per chunk
-constexpr int kNB = 5;            // band slots of the shared-memory rings
 constexpr int kRingD = 2;         // raw-pixel ring depth in steps (kRingD - 1 steps of prefetch in flight; a step of a warp
                                   // lasts microseconds because the sub-partition's other warps run in between)
 constexpr int kMaxIt = 7;         // counting passes before the search switches to walking / bisection
-constexpr int kListCap = 128;     // candidates evaluated per batch by a sparse warp
-constexpr int kItemCap = 64;      // flagged lane runs expanded per batch by a sparse warp
+constexpr int kListCap = 32 * 16; // candidates of 32 items (at most 16 pixels each)
+constexpr int kItemCap = 128;     // flagged units expanded per batch by a sparse warp
 constexpr int kChainMaxThreads = 640;
 constexpr int kMaxSparseWarps = 8;
+
+// Candidate flags are kept per UNIT of a lane's run: NU units of U pixels (the last one may be shorter), chosen so
+// that the LPS * NU flag bits of a row segment fit one 64-bit word and a unit is about 8 pixels.
+__host__ __device__ constexpr int flag_units(int N, int LPS) { return LPS * ((N + 7) / 8) <= 64 ? (N + 7) / 8 : 64 / LPS; }
+__host__ __device__ constexpr int flag_unit_px(int N, int LPS) { return ((N + flag_units(N, LPS) - 1) / flag_units(N, LPS) + 1) & ~1; }
 
 struct CParams {
   // inputs
   const uint16_t *raw;
   int n_frames;
   const float *ped;      // the caller's pedestal (float32)
-  const float *rg;       // 1/gain rounded to float32 (dense pass)
+  const float *rg;       // 1/gain rounded to float32
+  const float *mapK;     // dense pass: 2^23 + rint(ped)            v1 = fma((2^23 + raw) - K, rg, npf): the subtraction
+  const float *mapNpf;   // dense pass: -(ped - rint(ped)) / gain    is exact, one rounding in the fma
   const double *rg64;    // 1/gain in double (exact evaluation of candidates)
   // geometry
-  int P, H, W, S, nseg, WPR;                 // WPR: 32-bit words per bitmap row
+  int P, H, W, S, nseg;
   int R, bands_per_panel, n_bands;           // band rows, bands
-  int NWD, NWS;                              // dense warps (R * nseg), sparse warps
+  int NWD, NWS, NB;                          // dense warps (R * nseg), sparse warps, band slots of the rings
   // thresholds
   float T_seed, T_cm, E_ph, sqrtS, cand_thr, big;
   double dT_seed, dE_ph;
@@ -65,10 +72,8 @@ struct CParams {
   float *hit_dx, *hit_dy;
   uint32_t *frame_photons, *accum, *status;
   float *cm_keep;                            // optional [n][P][H][nseg]
-  unsigned long long *stats;                 // density hint for the next launch, plain stores only: [0] pixels of this launch,
-                                             // [1 + block * kMaxSparseWarps + sw] seeds found by that sparse warp
   // shared-memory carve-up (byte offsets)
-  uint32_t off_cm, off_flag, off_bar, off_done, off_pref, off_phot, off_sparse, sparse_stride, off_ring, off_maps;
+  uint32_t off_cm, off_flag, off_done, off_pref, off_phot, off_sparse, sparse_stride, off_ring, off_maps;
   uint32_t ring_warp_bytes, maps_warp_bytes;
 };
 
@@ -76,18 +81,6 @@ struct CParams {
 template <int BYTES>
 __device__ __forceinline__ void cp_async_s(uint32_t dst_smem, const void *src) {   // SASS: LDGSTS
   asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst_smem), "l"(src), "n"(BYTES) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {   // release
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity) {  // acquire when it succeeds
-  uint32_t ok;   // try_wait suspends the warp in hardware until the phase completes or the hint (ns) expires
-  asm volatile(
-      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity), "r"(100000u)
-      : "memory");
-  return ok != 0;
 }
 __device__ __forceinline__ void red_add_u32(uint32_t *p, uint32_t v) {
   asm volatile("red.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -97,7 +90,9 @@ __device__ __forceinline__ float rcp_approx(float x) {   // one MUFU.RCP
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
-#ifndef PDP_CVT_PRMT
+// uint16 -> float.  I2F.U16 is a quarter-rate conversion on sm_100a (8 cycles per warp instruction measured):
+// PRMT builds the float 2^23 + raw from the 16-bit half and the constant 0x4B00, then an exact subtraction.
+#ifdef PDP_CVT_I2F
 __device__ __forceinline__ float u16lo_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H0
   float f;
   asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, l;}" : "=f"(f) : "r"(w));
@@ -108,7 +103,7 @@ __device__ __forceinline__ float u16hi_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H1
   asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, h;}" : "=f"(f) : "r"(w));
   return f;
 }
-#else   // PRMT builds the float 2^23 + raw, the subtraction of 2^23 is exact
+#else
 __device__ __forceinline__ float u16lo_to_f(uint32_t w) {
   return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - 8388608.f;
 }
@@ -116,6 +111,12 @@ __device__ __forceinline__ float u16hi_to_f(uint32_t w) {
   return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8388608.f;
 }
 #endif
+__device__ __forceinline__ float magic_lo(uint32_t w) {   // 2^23 + low 16 bits, as a float (one PRMT)
+  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));
+}
+__device__ __forceinline__ float magic_hi(uint32_t w) {   // 2^23 + high 16 bits
+  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632));
+}
 __device__ __forceinline__ float set_lt_abs(float a, float t) {   // 1.0f if |a| < t else 0.0f
   float d;
   asm("set.lt.f32.f32 %0, %1, %2;" : "=f"(d) : "f"(fabsf(a)), "f"(t));
@@ -172,8 +173,13 @@ __device__ __forceinline__ float group_sum(float v) {
 }
 template <int LPS>
 __device__ __forceinline__ float group_count(float v) {   // sum of small exact integers held as floats
-  if constexpr (LPS == 32) return (float)__reduce_add_sync(FULL, __float2int_rn(v));   // REDUX
-  else return group_sum<LPS>(v);
+  if constexpr (LPS == 32) {
+    // REDUX.ADD on the bits of v + 2^23 (the low mantissa bits hold the integer): F2I is a quarter-rate conversion
+    const int r = __reduce_add_sync(FULL, __float_as_int(v + 8388608.f) & 0x7fffff);
+    return (float)r;
+  } else {
+    return group_sum<LPS>(v);
+  }
 }
 template <int LPS>
 __device__ __forceinline__ float group_min(float v) {
@@ -280,8 +286,13 @@ __device__ __forceinline__ float group_median(const float (&b)[N], int n, float 
   float xl = 0.f, xh = 0.f, prev = 0.f;
   bool got = false, has_prev = false;
 #pragma unroll 1
-  while (__any_sync(FULL, phase != 4)) {
-    if (__any_sync(FULL, phase == 0)) {
+  for (;;) {
+    // which phases are present in the warp: one REDUX.OR (LPS < 32), or the warp-uniform state itself
+    unsigned present;
+    if constexpr (LPS == 32) present = 1u << phase;
+    else present = __reduce_or_sync(FULL, 1u << phase);
+    if ((present & 15u) == 0u) break;
+    if (present & 1u) {
       const int c = (int)pass_count<N, LPS>(b, p);
       if (phase == 0) {
         if ((unsigned)(c - kl + 1) <= (unsigned)(kh - kl + 3)) {   // rank in [kl-1, kh+2]
@@ -307,7 +318,8 @@ __device__ __forceinline__ float group_median(const float (&b)[N], int n, float 
         }
       }
     }
-    if (__any_sync(FULL, phase == 1 || phase == 3)) {
+    if constexpr (LPS == 32) present = 1u << phase;   // uniform state: take the transition at once
+    if (present & 10u) {
       float cf;
       const float A = pass_up<N, LPS>(b, p, big2, cf);   // A = x[c], c = #{b < p}
       const int c = (int)cf;
@@ -338,7 +350,8 @@ __device__ __forceinline__ float group_median(const float (&b)[N], int n, float 
         }
       }
     }
-    if (__any_sync(FULL, phase == 2)) {
+    if constexpr (LPS == 32) present = 1u << phase;
+    if (present & 4u) {
       float cf;
       const float B = pass_down<N, LPS>(b, p, big2, cf);   // B = x[c-1], c = #{b < p}
       const int c = (int)cf;
@@ -429,61 +442,118 @@ static __device__ __noinline__ void overflow_accum(uint32_t *accum_px, uint32_t 
   *status = 1u;   // PDP_STATUS_HIT_OVERFLOW (the only bit; every writer stores the same value)
 }
 
-struct BandDesc {      // one band of one panel, as the sparse warps see it
-  int gb, band, p, bi; // running band index (over chunks), band of the frame, panel, band of the panel
-};
+// Named barriers (ids 1..kNB, one per band slot in flight): the dense warps ARRIVE after publishing a band, the one
+// sparse warp that owns the band SYNCs before it reads it.  A waiting warp is parked by the hardware: no polling.
+__device__ __forceinline__ void named_arrive(int id, int threads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ void named_sync(int id, int threads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
 
-// ---- sparse stage of one band for the frame slots {sw, sw + NWS, ...} < nf of the chunk: ONE warp ---------
-//  1. flagged lane runs (one flag bit per dense lane and frame) -> item list;
-//  2. every item's pixels are tested with the dense pass's own fp32 formula; candidate bits go to a private
-//     bitmap [frames of this warp][rows][W/32] with a per-row summary of the non-zero words;
-//  3. the candidate bits are compacted in (frame, row, column) order into a list, and every lane evaluates one
-//     candidate at a time in fp64 (all loads of a batch in flight together); seeds take their slot by
-//     ballot/popc on top of the frame's running count.
+constexpr int kSeedCap = 256;     // seeds buffered per sparse warp between evaluation and ordered emission
+
+// ---- sparse stage of ONE band for ALL frame slots of the chunk: one warp ------------------------------------------
+// Sparse warp s owns the bands gb = s, s + NWS, ...: several bands are evaluated at the same time by different
+// warps, each call covers up to 16 band-frames (full batches, the per-call overhead shared), and only the ordered
+// emission is chained from band to band (band_done).
+//  1. flagged units (about 8 pixels of a dense lane's run, one flag bit each, in column order) -> item list;
+//  2. every item's pixels are tested with the dense pass's own fp32 formula (all loads of up to 8 pixel pairs per
+//     lane in flight); the candidates go to a list in (frame, row, column) order;
+//  3. every lane evaluates one candidate at a time in fp64 (the exact seed rule, E, n, dx, dy in the oracle's order
+//     of operations); seeds are appended, in order, to a buffer;
+//  4. once the band before has been emitted (its running per-frame counts are final), the buffer is written to the
+//     frames' lists at base[frame] + rank.
 template <int N, int LPS>
-__device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *smem, int sw, int nf, const BandDesc &bd,
-                                             int f0, unsigned long long &seeds_total) {
+__device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *smem, int sw, int nf, int gb, int band,
+                                             int f0) {
+  constexpr int NU = flag_units(N, LPS), U = flag_unit_px(N, LPS);
   const int lane = threadIdx.x & 31;
-  const int R = k.R, ring_rows = kNB * R, NWS = k.NWS;
+  const int R = k.R, kNBr = k.NB, ring_rows = kNBr * R;
   const float *cmring = reinterpret_cast<const float *>(smem + k.off_cm);
-  const uint32_t *flags = reinterpret_cast<const uint32_t *>(smem + k.off_flag);
-  volatile int *done = reinterpret_cast<volatile int *>(smem + k.off_done);
-  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);
-  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);
+  const unsigned long long *flags = reinterpret_cast<const unsigned long long *>(smem + k.off_flag);
+  volatile int *band_done = reinterpret_cast<volatile int *>(smem + k.off_done);
+  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);      // [kFCH] hits of the frame so far
+  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);      // [kFCH] photons of the frame so far
   unsigned char *mine = smem + k.off_sparse + (size_t)sw * k.sparse_stride;
-  uint32_t *list = reinterpret_cast<uint32_t *>(mine);                       // [kListCap]
-  uint32_t *items = list + kListCap;                                          // [kItemCap]
-  unsigned long long *rowmask = reinterpret_cast<unsigned long long *>(items + kItemCap);   // [GFmax][R+1]
-  const int GFmax = (kFCH + NWS - 1) / NWS;
-  uint32_t *bits = reinterpret_cast<uint32_t *>(rowmask + GFmax * (R + 1));  // [GFmax][R+1][WPR]
+  uint32_t *items = reinterpret_cast<uint32_t *>(mine);                  // [kItemCap] flagged units
+  uint32_t *imask = items + kItemCap;                                    // [kItemCap] candidate pixels of the unit
+  uint32_t *cand = imask + kItemCap;                                     // [kListCap] candidates (q, row, col)
+  uint32_t *s_pix = cand + kListCap;                                     // [kSeedCap] seed buffer
+  float *s_E = reinterpret_cast<float *>(s_pix + kSeedCap);
+  int32_t *s_n = reinterpret_cast<int32_t *>(s_E + kSeedCap);
+  float *s_dx = reinterpret_cast<float *>(s_n + kSeedCap);
+  float *s_dy = s_dx + kSeedCap;
+  uint32_t *s_q = reinterpret_cast<uint32_t *>(s_dy + kSeedCap);
+  uint32_t *base_s = s_q + kSeedCap;                                     // [kFCH] working copy of pref
+  uint32_t *pht_s = base_s + kFCH;                                       // [kFCH] photons added by this band
 
-  const int p = bd.p, r0 = bd.bi * R;
-  const int ra = bd.bi == 0 ? 0 : r0 - 1;
-  const int rb = bd.bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
+  const int p = band / k.bands_per_panel, bi = band - p * k.bands_per_panel, r0 = bi * R;
+  const int ra = bi == 0 ? 0 : r0 - 1;
+  const int rb = bi == k.bands_per_panel - 1 ? k.H - 1 : r0 + R - 2;
   const int nrows = rb - ra + 1;
-  const int nfr = nf > sw ? (nf - sw + NWS - 1) / NWS : 0;    // my frame slots: sw, sw + NWS, ...
   // ring slot of row r in [r0-2, r0+R): bands gb-1 and gb
-  const int s_prev = ((bd.gb + kNB - 1) % kNB) * R, s_cur = (bd.gb % kNB) * R;
+  const int s_prev = ((gb + kNBr - 1) % kNBr) * R, s_cur = (gb % kNBr) * R;
   auto slot_of = [&](int r) { return r < r0 ? s_prev + (r - r0 + R) : s_cur + (r - r0); };
   const size_t npix = (size_t)k.P * k.H * k.W;
-  const int n_tasks = nrows > 0 ? nfr * nrows : 0;
+  bool waited = false;      // the band before has been emitted and base_s / pht_s are loaded
+  int ns = 0;               // seeds in the buffer (warp-uniform)
+  if (lane < kFCH) pht_s[lane] = 0u;
 
-  // ---- 1 + 2: flagged lane runs -> candidate bitmap ----
-  // task t = (q, rr, sg): frame slot sw + q*NWS, row ra + rr, segment sg
-  const int n_ft = n_tasks * k.nseg;
+  auto flush = [&]() {      // ordered emission of the buffered seeds
+    if (!waited) {
+      if (lane == 0)
+        while (*band_done < gb) {
+        }
+      __syncwarp();
+      __threadfence_block();
+      if (lane < kFCH) base_s[lane] = pref[lane];
+      __syncwarp();
+      waited = true;
+    }
+    for (int i0 = 0; i0 < ns; i0 += 32) {
+      const int i = i0 + lane;
+      const bool have = i < ns;
+      const uint32_t q = have ? s_q[i] : 0xffffffffu;
+      const unsigned same = __match_any_sync(FULL, q);
+      if (have) {
+        const uint32_t pos = base_s[q] + __popc(same & ((1u << lane) - 1u));
+        const uint32_t pix = s_pix[i];
+        const int n = s_n[i];
+        if (pos < k.cap) {
+          const size_t o = (size_t)(f0 + q) * k.cap + pos;
+          k.hit_pixel[o] = pix;
+          k.hit_charge[o] = s_E[i];
+          k.hit_nphot[o] = n;
+          k.hit_dx[o] = s_dx[i];
+          k.hit_dy[o] = s_dy[i];
+        } else {
+          overflow_accum(k.accum + pix, (uint32_t)n, k.status);
+        }
+        if (n) atomicAdd(&pht_s[q], (uint32_t)n);   // shared memory; integer sum: order-independent
+      }
+      __syncwarp();
+      if (have && (same >> lane) <= 1u) base_s[q] += __popc(same);   // the last lane of each frame's run
+      __syncwarp();
+    }
+    ns = 0;
+  };
+
+  // ---- 1-3 over the (frame, row, segment) tasks in output order ----
+  const int n_ft = nrows > 0 ? nf * nrows * k.nseg : 0;
   for (int t0 = 0; t0 < n_ft; t0 += 32) {
     const int t = t0 + lane;
-    uint32_t fw = 0u;
+    unsigned long long fw = 0ull;
     int tq = 0, trr = 0, tsg = 0;
     if (t < n_ft) {
       tsg = t % k.nseg;
       const int u = t / k.nseg;
       tq = u / nrows;
       trr = u - tq * nrows;
-      fw = flags[((size_t)(sw + tq * NWS) * ring_rows + slot_of(ra + trr)) * k.nseg + tsg];
+      fw = flags[((size_t)tq * ring_rows + slot_of(ra + trr)) * k.nseg + tsg];
     }
-    if (!__any_sync(FULL, fw != 0u)) continue;
-    int mine_n = __popc(fw), incl = mine_n;
+    if (!__any_sync(FULL, fw != 0ull)) continue;
+    int mine_n = __popcll(fw), incl = mine_n;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
       const int u = __shfl_up_sync(FULL, incl, o);
@@ -492,154 +562,133 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
     const int total = __shfl_sync(FULL, incl, 31);
     const int first = incl - mine_n;
     for (int b0 = 0; b0 < total; b0 += kItemCap) {
+      // ---- 1: items [b0, b0 + kItemCap) of this group of tasks ----
       if (first < b0 + kItemCap && first + mine_n > b0) {
         int idx = first;
-        for (uint32_t m = fw; m; m &= m - 1, ++idx)
-          if (idx >= b0 && idx < b0 + kItemCap)
-            items[idx - b0] = ((uint32_t)tq << 24) | ((uint32_t)trr << 16) | ((uint32_t)tsg << 8) | (uint32_t)(__ffs(m) - 1);
+        for (unsigned long long m = fw; m; m &= m - 1, ++idx)
+          if (idx >= b0 && idx < b0 + kItemCap)   // flag bit = lane-in-group * NU + unit: ascending bits = ascending columns
+            items[idx - b0] = ((uint32_t)tq << 24) | ((uint32_t)trr << 16) | ((uint32_t)tsg << 8) | (uint32_t)(__ffsll((long long)m) - 1);
       }
-      __syncwarp();
       const int nb = min(kItemCap, total - b0);
-      for (int i0 = 0; i0 < nb; i0 += 32) {
-        if (i0 + lane < nb) {
-          const uint32_t e = items[i0 + lane];
-          const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), l = (int)(e & 0xffu);
-          const int row = ra + rr, fl = sw + q * NWS;
-          const float c = cmring[((size_t)fl * ring_rows + slot_of(row)) * k.nseg + sg];
-          const float thr = k.cand_thr + c;
-          const int c0 = sg * k.S + l * N, c1 = min(c0 + N, (sg + 1) * k.S);
-          const size_t gi = ((size_t)p * k.H + row) * k.W;
-          const uint16_t *rw = k.raw + (size_t)(f0 + fl) * npix + gi;
-          uint32_t *brow = bits + ((size_t)q * (R + 1) + rr) * k.WPR;
-          unsigned long long rm = 0ull;
-          for (int col = c0; col < c1; col += 2) {     // runs start and end on even columns
-            const uint32_t w = __ldg(reinterpret_cast<const uint32_t *>(rw + col));
-            const float2 pd = __ldg(reinterpret_cast<const float2 *>(k.ped + gi + col));
-            const float2 rg = __ldg(reinterpret_cast<const float2 *>(k.rg + gi + col));
-            const float a0 = (u16lo_to_f(w) - pd.x) * rg.x, a1 = (u16hi_to_f(w) - pd.y) * rg.y;
-            const uint32_t bb = (a0 > thr ? 1u : 0u) | (a1 > thr ? 2u : 0u);
-            if (bb) {
-              atomicOr(brow + (col >> 5), bb << (col & 31));
-              rm |= 1ull << (col >> 5);
+      for (int i = lane; i < nb; i += 32) imask[i] = 0u;
+      __syncwarp();
+      // ---- 2: pixel test; a lane takes kPxU (item, pixel pair) tasks at a time, all loads first ----
+      constexpr int PP = U / 2, kPxU = 8;
+      const int n_px_tasks = nb * PP;
+      for (int u0 = 0; u0 < n_px_tasks; u0 += 32 * kPxU) {
+        uint32_t w[kPxU];
+        float2 mk[kPxU], rg[kPxU], nf2[kPxU];
+        float thr[kPxU];
+        int itu[kPxU], pju[kPxU];
+#pragma unroll
+        for (int u = 0; u < kPxU; ++u) {
+          const int tt = u0 + u * 32 + lane;
+          itu[u] = -1;
+          if (tt < n_px_tasks) {
+            const int it = tt / PP, pj = tt - it * PP;
+            const uint32_t e = items[it];
+            const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
+            const int l = fb / NU, un = fb - l * NU;
+            const int j = un * U + 2 * pj;                 // pixel of the lane's run
+            const int col = sg * k.S + l * N + j;
+            if (j < N && col < (sg + 1) * k.S) {
+              const int row = ra + rr;
+              const size_t gi = ((size_t)p * k.H + row) * k.W + col;
+              w[u] = __ldg(reinterpret_cast<const uint32_t *>(k.raw + (size_t)(f0 + q) * npix + gi));
+              mk[u] = __ldg(reinterpret_cast<const float2 *>(k.mapK + gi));
+              rg[u] = __ldg(reinterpret_cast<const float2 *>(k.rg + gi));
+              nf2[u] = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + gi));
+              thr[u] = k.cand_thr + cmring[((size_t)q * ring_rows + slot_of(row)) * k.nseg + sg];
+              itu[u] = it;
+              pju[u] = pj;
             }
           }
-          if (rm) atomicOr(rowmask + q * (R + 1) + rr, rm);
         }
-      }
-      __syncwarp();
-    }
-  }
-  __syncwarp();
-
-  // ---- 3: candidates in (frame, row, column) order -> exact rule -> ordered emission ----
-  uint32_t base = lane < nfr ? pref[sw + lane * NWS] : 0u;   // lane q holds the running totals of my frame q
-  int ph = 0;
-  for (int t0 = 0; t0 < n_tasks; t0 += 32) {
-    const int t = t0 + lane;
-    const bool tv = t < n_tasks;
-    int tq = 0, trr = 0;
-    if (tv) {
-      tq = t / nrows;
-      trr = t - tq * nrows;
-    }
-    const int rowslot = tq * (R + 1) + trr;
-    const unsigned long long rmask = tv ? rowmask[rowslot] : 0ull;
-    if (!__any_sync(FULL, rmask != 0ull)) continue;
-    uint32_t *rowbits = bits + (size_t)rowslot * k.WPR;
-    int mine_n = 0;
-    for (unsigned long long m = rmask; m; m &= m - 1) mine_n += __popc(rowbits[__ffsll((long long)m) - 1]);
-    int incl = mine_n;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int u = __shfl_up_sync(FULL, incl, o);
-      if (lane >= o) incl += u;
-    }
-    const int total = __shfl_sync(FULL, incl, 31);
-    const int my_first = incl - mine_n;
-    for (int b0 = 0; b0 < total; b0 += kListCap) {
-      if (my_first < b0 + kListCap && my_first + mine_n > b0) {
-        int idx = my_first;
-        for (unsigned long long m = rmask; m; m &= m - 1) {
-          const int wi = __ffsll((long long)m) - 1;
-          for (uint32_t wv = rowbits[wi]; wv; wv &= wv - 1) {
-            if (idx >= b0 && idx < b0 + kListCap)
-              list[idx - b0] = ((uint32_t)tq << 28) | ((uint32_t)trr << 20) | (uint32_t)(wi * 32 + __ffs(wv) - 1);
-            ++idx;
+        for (int u = 0; u < kPxU; ++u) {
+          if (itu[u] >= 0) {
+            const float a0 = fmaf(magic_lo(w[u]) - mk[u].x, rg[u].x, nf2[u].x);
+            const float a1 = fmaf(magic_hi(w[u]) - mk[u].y, rg[u].y, nf2[u].y);
+            const uint32_t bb = (a0 > thr[u] ? 1u : 0u) | (a1 > thr[u] ? 2u : 0u);
+            if (bb) atomicOr(&imask[itu[u]], bb << (2 * pju[u]));
           }
         }
       }
       __syncwarp();
-      const int nb = min(kListCap, total - b0);
+      // ---- candidates of the items, in order, kListCap at a time -> 3: exact evaluation ----
       for (int i0 = 0; i0 < nb; i0 += 32) {
-        const bool have = i0 + lane < nb;
-        const uint32_t e = have ? list[i0 + lane] : 0u;
-        const int q = (int)(e >> 28), row = ra + (int)((e >> 20) & 0xffu), col = (int)(e & 0xfffffu);
-        const int fl = sw + q * NWS;
-        bool seed = false;
-        HitRec h{0.f, 0.f, 0.f, 0};
-        if (have) {
-          const float *cmf = cmring + (size_t)fl * ring_rows * k.nseg;
-          const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
-          const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : nullptr;
-          const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : nullptr;
-          const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + fl) * npix, cm_m1, cm_0, cm_p1, p, row, col);
-          seed = e9.seed;
-          if (seed) h = make_rec(e9, k.dE_ph);
+        const bool hv = i0 + lane < nb;
+        const uint32_t m = hv ? imask[i0 + lane] : 0u;
+        const uint32_t e = hv ? items[i0 + lane] : 0u;
+        int cn = __popc(m), cincl = cn;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int u = __shfl_up_sync(FULL, cincl, o);
+          if (lane >= o) cincl += u;
         }
-        if (!__any_sync(FULL, seed)) continue;
-        const unsigned lt = (1u << lane) - 1u;
-        unsigned mymask = 0u;
-        int add = 0, addph = 0;
-        for (int qq = 0; qq < nfr; ++qq) {
-          const unsigned m = __ballot_sync(FULL, seed && q == qq);
-          if (!m) continue;
-          const int phq = __reduce_add_sync(FULL, seed && q == qq ? h.n : 0);
-          if (q == qq) mymask = m;
-          if (lane == qq) add = __popc(m), addph = phq;
+        const int ctotal = __shfl_sync(FULL, cincl, 31);
+        if (ctotal == 0) continue;
+        const int cfirst = cincl - cn;
+        {
+          const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
+          const int l = fb / NU, un = fb - l * NU;
+          const int colb = sg * k.S + l * N + un * U;
+          int idx = cfirst;
+          for (uint32_t mm = m; mm; mm &= mm - 1, ++idx)      // ctotal <= 32 * U <= kListCap
+            cand[idx] = ((uint32_t)q << 28) | ((uint32_t)rr << 20) | (uint32_t)(colb + __ffs(mm) - 1);
         }
-        const uint32_t b_q = __shfl_sync(FULL, base, q);
-        if (seed) {
-          const uint32_t pos = b_q + __popc(mymask & lt);
-          const uint32_t pix = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
-          if (pos < k.cap) {
-            const size_t o = (size_t)(f0 + fl) * k.cap + pos;
-            k.hit_pixel[o] = pix;
-            k.hit_charge[o] = h.E;
-            k.hit_nphot[o] = h.n;
-            k.hit_dx[o] = h.dx;
-            k.hit_dy[o] = h.dy;
-          } else {
-            overflow_accum(k.accum + pix, (uint32_t)h.n, k.status);
+        __syncwarp();
+        for (int c0 = 0; c0 < ctotal; c0 += 32) {
+          const bool have = c0 + lane < ctotal;
+          const uint32_t ce = have ? cand[c0 + lane] : 0u;
+          const int q = (int)(ce >> 28), row = ra + (int)((ce >> 20) & 0xffu), col = (int)(ce & 0xfffffu);
+          bool seed = false;
+          HitRec h{0.f, 0.f, 0.f, 0};
+          if (have) {
+            const float *cmf = cmring + (size_t)q * ring_rows * k.nseg;
+            const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
+            const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : nullptr;
+            const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : nullptr;
+            const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + q) * npix, cm_m1, cm_0, cm_p1, p, row, col);
+            seed = e9.seed;
+            if (seed) h = make_rec(e9, k.dE_ph);
           }
+          const unsigned sm = __ballot_sync(FULL, seed);
+          if (!sm) continue;
+          if (ns + __popc(sm) > kSeedCap) flush();
+          if (seed) {
+            const int o = ns + __popc(sm & ((1u << lane) - 1u));
+            s_pix[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
+            s_E[o] = h.E;
+            s_n[o] = h.n;
+            s_dx[o] = h.dx;
+            s_dy[o] = h.dy;
+            s_q[o] = (uint32_t)q;
+          }
+          ns += __popc(sm);
+          __syncwarp();
         }
-        base += (uint32_t)add;
-        ph += addph;
       }
       __syncwarp();
-    }
-    if (rmask) {   // consumed: clear the words and the summary
-      for (unsigned long long m = rmask; m; m &= m - 1) rowbits[__ffsll((long long)m) - 1] = 0u;
-      rowmask[rowslot] = 0ull;
     }
   }
-  if (lane < nfr) {
-    const int fl = sw + lane * NWS;
-    const uint32_t pht = phot[fl] + (uint32_t)ph;
-    if (bd.band == k.n_bands - 1) {  // the frame is complete
-      k.hit_count[f0 + fl] = base;
-      k.frame_photons[f0 + fl] = pht;
-      pref[fl] = 0u;
-      phot[fl] = 0u;
-      seeds_total += base;
+  flush();   // also waits for the band before when nothing was buffered: the running totals are passed on in order
+  if (lane < nf) {
+    const uint32_t cnt = base_s[lane], pht = phot[lane] + pht_s[lane];
+    if (band == k.n_bands - 1) {   // the frame is complete
+      k.hit_count[f0 + lane] = cnt;
+      k.frame_photons[f0 + lane] = pht;
+      pref[lane] = 0u;
+      phot[lane] = 0u;
     } else {
-      pref[fl] = base;
-      phot[fl] = pht;
+      pref[lane] = cnt;
+      phot[lane] = pht;
     }
   }
   __syncwarp();
   if (lane == 0) {
     __threadfence_block();
-    done[sw] = bd.gb + 1;
+    *band_done = gb + 1;
   }
   __syncwarp();
 }
@@ -655,14 +704,14 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
   constexpr int CH = V / CS;                 // chunks per vector
   constexpr uint32_t VB = V * 2;             // bytes per raw vector
   constexpr uint32_t kStepBytes = 32u * N * 2u;   // one step of one warp in the raw ring
+  constexpr int NU = flag_units(N, LPS), U = flag_unit_px(N, LPS);
   extern __shared__ __align__(128) unsigned char smem[];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nthreads = blockDim.x, NWD = k.NWD, NWS = k.NWS;
-  const int R = k.R, ring_rows = kNB * R;
-  float *cmring = reinterpret_cast<float *>(smem + k.off_cm);          // [kFCH][kNB*R][nseg]
-  uint32_t *flags = reinterpret_cast<uint32_t *>(smem + k.off_flag);   // [kFCH][kNB*R][nseg]
-  uint64_t *bar = reinterpret_cast<uint64_t *>(smem + k.off_bar);      // [kNB][NWS] mbarriers: NWD arrivals
-  volatile int *done = reinterpret_cast<volatile int *>(smem + k.off_done);  // [NWS]
+  const int R = k.R, kNBr = k.NB, ring_rows = kNBr * R;
+  float *cmring = reinterpret_cast<float *>(smem + k.off_cm);                               // [kFCH][NB*R][nseg]
+  unsigned long long *flags = reinterpret_cast<unsigned long long *>(smem + k.off_flag);    // [kFCH][NB*R][nseg]
+  volatile int *band_done = reinterpret_cast<volatile int *>(smem + k.off_done);
   uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);    // [kFCH]
   uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);    // [kFCH]
 
@@ -670,42 +719,22 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
   const int fe = (int)(((long long)(blockIdx.x + 1) * k.n_frames) / gridDim.x);
   const int FCn = fe - fs;
   if (FCn <= 0) return;
+  const int n_chunks = (FCn + kFCH - 1) / kFCH;
+  const int sync_threads = (NWD + 1) * 32;      // the dense warps and the ONE sparse warp that owns the band
 
-  {  // prologue: zero the sparse warps' private bitmaps, initialise barriers and per-slot state
-    uint32_t *z = reinterpret_cast<uint32_t *>(smem + k.off_sparse);
-    const uint32_t nz = (uint32_t)NWS * k.sparse_stride / 4u;
-    for (uint32_t i = tid; i < nz; i += nthreads) z[i] = 0u;
-    if (tid == 0) {
-      for (int i = 0; i < kNB * NWS; ++i) mbar_init(&bar[i], (uint32_t)NWD);
-      fence_mbar_init();
-    }
-    for (int i = tid; i < kFCH; i += nthreads) pref[i] = 0u, phot[i] = 0u;
-    for (int i = tid; i < NWS; i += nthreads) done[i] = 0;
-  }
+  for (int i = tid; i < kFCH; i += nthreads) pref[i] = 0u, phot[i] = 0u;
+  if (tid == 0) *band_done = 0;
   __syncthreads();
 
   if (warp >= NWD) {
-    // ===== sparse warps =====
+    // ===== sparse warps: warp s owns the bands gb = s, s + NWS, ... (gb runs over the chunks) =====
     const int sw = warp - NWD;
-    BandDesc bd{0, 0, 0, 0};
-    unsigned long long seeds_total = 0ull;   // per lane: seeds of the frames this lane finished
-    for (int c0 = 0; c0 < FCn; c0 += kFCH) {
-      const int nf = min(kFCH, FCn - c0);
-      bd.band = 0, bd.p = 0, bd.bi = 0;
-      for (; bd.band < k.n_bands; ++bd.band, ++bd.gb) {
-        // every dense warp has published the band: acquire on my barrier of the band's ring slot
-        while (!mbar_test(&bar[(bd.gb % kNB) * NWS + sw], (uint32_t)(bd.gb / kNB) & 1u))
-          __nanosleep(2000);   // a sleeping warp costs no issue slots; a band of dense work lasts tens of microseconds
-        chain_sparse<N, LPS>(k, smem, sw, nf, bd, fs + c0, seeds_total);
-        if (++bd.bi == k.bands_per_panel) bd.bi = 0, ++bd.p;
-      }
-    }
-    if (k.stats) {   // density hint for the host (plain stores, one slot per sparse warp)
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) seeds_total += __shfl_xor_sync(FULL, seeds_total, o);
-      if (lane == 0) k.stats[1 + blockIdx.x * kMaxSparseWarps + sw] = seeds_total;
-      if (lane == 0 && sw == 0 && blockIdx.x == 0)
-        k.stats[0] = (unsigned long long)k.n_frames * (unsigned long long)k.P * (unsigned long long)k.H * (unsigned long long)k.W;
+    const int total_bands = n_chunks * k.n_bands;
+    for (int gb = sw; gb < total_bands; gb += NWS) {
+      const int chunk = gb / k.n_bands, band = gb - chunk * k.n_bands;
+      const int c0 = chunk * kFCH, nf = min(kFCH, FCn - c0);
+      named_sync(1 + gb % kNBr, sync_threads);   // parked until every dense warp has published the band
+      chain_sparse<N, LPS>(k, smem, sw, nf, gb, band, fs + c0);
     }
     return;
   }
@@ -766,7 +795,7 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
       const int p = band / k.bands_per_panel, r0 = (band - p * k.bands_per_panel) * R;
       const int row = r0 + tr;
       const bool active = row < k.H;
-      const int slot = (gb % kNB) * R + tr;
+      const int slot = (gb % kNBr) * R + tr;
       if (active) {   // maps of this warp's row segment: global (L2) -> lane-major tile, once per band and chunk
         const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
         __syncwarp();
@@ -774,38 +803,41 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
           // chunk ci of the tile holds pixels j .. j+CS-1 of lane-slot ll: tile index (ck * LPS + ll)
           const int ck = ci / LPS, ll = ci - ck * LPS;
           const int j = ll * N + ck * CS;
-          float pd[CS], rr[CS];
+          float mk[CS], rr[CS], nf[CS];
           if (j < k.S) {
             if constexpr (CS == 4) {
-              const float4 a = __ldg(reinterpret_cast<const float4 *>(k.ped + rowoff + j));
+              const float4 a = __ldg(reinterpret_cast<const float4 *>(k.mapK + rowoff + j));
               const float4 b = __ldg(reinterpret_cast<const float4 *>(k.rg + rowoff + j));
-              pd[0] = a.x, pd[1] = a.y, pd[2] = a.z, pd[3] = a.w;
+              const float4 c = __ldg(reinterpret_cast<const float4 *>(k.mapNpf + rowoff + j));
+              mk[0] = a.x, mk[1] = a.y, mk[2] = a.z, mk[3] = a.w;
               rr[0] = b.x, rr[1] = b.y, rr[2] = b.z, rr[3] = b.w;
+              nf[0] = c.x, nf[1] = c.y, nf[2] = c.z, nf[3] = c.w;
             } else {
-              const float2 a = __ldg(reinterpret_cast<const float2 *>(k.ped + rowoff + j));
+              const float2 a = __ldg(reinterpret_cast<const float2 *>(k.mapK + rowoff + j));
               const float2 b = __ldg(reinterpret_cast<const float2 *>(k.rg + rowoff + j));
-              pd[0] = a.x, pd[1] = a.y;
+              const float2 c = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + rowoff + j));
+              mk[0] = a.x, mk[1] = a.y;
               rr[0] = b.x, rr[1] = b.y;
+              nf[0] = c.x, nf[1] = c.y;
             }
-          } else {   // padding: a = (raw - 3e38) * 1 = -3e38: outside the mask, never a candidate
+          } else {   // padding: a = fma(x - K, 0, -3e38) = -3e38: outside the mask, never a candidate
 #pragma unroll
-            for (int e = 0; e < CS; ++e) pd[e] = 3.0e38f, rr[e] = 1.f;
+            for (int e = 0; e < CS; ++e) mk[e] = 8388608.f, rr[e] = 0.f, nf[e] = -3.0e38f;
           }
 #pragma unroll
           for (int e = 0; e < CS; ++e) {
-            maps_ptr[ci * CS + e] = pd[e];
+            maps_ptr[ci * CS + e] = mk[e];
             maps_ptr[kMapFloats + ci * CS + e] = rr[e];
+            maps_ptr[2 * kMapFloats + ci * CS + e] = nf[e];
           }
         }
         __syncwarp();
       }
-      // the ring slot about to be written held band gb-kNB, last read by the sparse stage of band gb-kNB+1
-      for (int s = 0; s < NWS; ++s)
-        while (done[s] < gb - (kNB - 2)) {
-        }
+      // the ring slot about to be written held band gb-NB, last read by the sparse stage of band gb-NB+1
+      while (*band_done < gb - (kNBr - 2)) __nanosleep(100);
 
       float *cm_p = cmring + ((size_t)g * ring_rows + slot) * k.nseg + sg;
-      uint32_t *fl_p = flags + ((size_t)g * ring_rows + slot) * k.nseg + sg;
+      unsigned long long *fl_p = flags + ((size_t)g * ring_rows + slot) * k.nseg + sg;
       const int step_stride = FPS * ring_rows * k.nseg;
       for (int s = 0; s < nsteps; ++s) {
         issue();
@@ -813,7 +845,10 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
         const int fl = s * FPS + g;
         const bool act = active && fl < nf;
         if (__any_sync(FULL, act)) {
-          float c = 0.f, amax = __int_as_float(0xff800000);
+          float c = 0.f;
+          float amax[NU];   // maximum of a over every flag unit of this lane's run
+#pragma unroll
+          for (int u = 0; u < NU; ++u) amax[u] = __int_as_float(0xff800000);
           if constexpr (MODE == 0) {
             // ================= exact median common mode (north_star (a)) =================
             float b[N];
@@ -824,20 +859,21 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
 #pragma unroll
               for (int h = 0; h < CH; ++h) {
-                float pd[CS], rr[CS];
-                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), pd);
+                float mk[CS], rr[CS], nf2[CS];
+                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
                 lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+                lds_f<CS>(maps_lane + 2 * kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), nf2);
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = (u16lo_to_f(ww) - pd[e]) * rr[e];
-                  const float a1 = (u16hi_to_f(ww) - pd[e + 1]) * rr[e + 1];
+                  const float a0 = fmaf(magic_lo(ww) - mk[e], rr[e], nf2[e]);
+                  const float a1 = fmaf(magic_hi(ww) - mk[e + 1], rr[e + 1], nf2[e + 1]);
                   const int j = v * V + h * CS + e;
                   b[j] = fabsf(a0) < T_cm ? a0 : BIG;          // pixels WITHOUT signal keep their value
                   b[j + 1] = fabsf(a1) < T_cm ? a1 : BIG;
                   sb0 += b[j];
                   sb1 += b[j + 1];
-                  amax = max3(amax, a0, a1);
+                  amax[j / U] = max3(amax[j / U], a0, a1);
                 }
               }
             }
@@ -861,20 +897,21 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
 #pragma unroll
               for (int h = 0; h < CH; ++h) {
-                float pd[CS], rr[CS];
-                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), pd);
+                float mk[CS], rr[CS], nf2[CS];
+                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
                 lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+                lds_f<CS>(maps_lane + 2 * kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), nf2);
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = (u16lo_to_f(ww) - pd[e]) * rr[e];
-                  const float a1 = (u16hi_to_f(ww) - pd[e + 1]) * rr[e + 1];
+                  const float a0 = fmaf(magic_lo(ww) - mk[e], rr[e], nf2[e]);
+                  const float a1 = fmaf(magic_hi(ww) - mk[e + 1], rr[e + 1], nf2[e + 1]);
                   if constexpr (MODE == 1) {
                     const float m0 = set_lt_abs(a0, T_cm), m1 = set_lt_abs(a1, T_cm);
                     n0 += m0, n1 += m1;
                     s0 = fmaf(m0, a0, s0), s1 = fmaf(m1, a1, s1);
                   }
-                  amax = max3(amax, a0, a1);
+                  amax[(v * V + h * CS + e) / U] = max3(amax[(v * V + h * CS + e) / U], a0, a1);
                 }
               }
             }
@@ -884,11 +921,30 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               c = __fdiv_rn(tot, fmaxf(n, k.sqrtS));
             }
           }
-          // ---- publish: common-mode estimate and one candidate flag per lane ----
-          const unsigned bal = __ballot_sync(FULL, act && amax > k.cand_thr + c);
+          // ---- publish: common-mode estimate and one candidate flag per unit of every lane's run ----
+          float am = amax[0];
+#pragma unroll
+          for (int u = 1; u < NU; ++u) am = fmaxf(am, amax[u]);
+          const float thr = k.cand_thr + c;
+          unsigned long long word = 0ull;
+          if (__ballot_sync(FULL, act && am > thr)) {   // some lane of the warp holds a candidate: flag its units
+            // flag bit = lane-in-group * NU + unit (ascending bits = ascending columns)
+            unsigned mine_bits = 0u;
+#pragma unroll
+            for (int u = 0; u < NU; ++u) mine_bits |= (act && amax[u] > thr ? 1u : 0u) << u;
+            unsigned long long w64 = (unsigned long long)mine_bits << (l * NU);
+            if constexpr (LPS == 32) {
+              word = (unsigned long long)__reduce_or_sync(FULL, (unsigned)w64) |
+                     ((unsigned long long)__reduce_or_sync(FULL, (unsigned)(w64 >> 32)) << 32);
+            } else {
+#pragma unroll
+              for (int o = LPS / 2; o > 0; o >>= 1) w64 |= __shfl_xor_sync(FULL, w64, o);
+              word = w64;
+            }
+          }
           if (act && l == 0) {
             *cm_p = c;
-            *fl_p = LPS == 32 ? bal : (bal >> (g * LPS)) & ((1u << (LPS & 31)) - 1u);
+            *fl_p = word;
             if (k.cm_keep)   // debug only
               k.cm_keep[(((size_t)(fs + c0 + fl) * k.P + p) * k.H + row) * k.nseg + sg] = c;
           }
@@ -897,9 +953,9 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
         cm_p += step_stride;
         fl_p += step_stride;
       }
-      // ---- arrive (release) on every sparse warp's barrier of this band slot ----
+      // ---- arrive on the band slot's named barrier (the sparse warp that owns the band syncs on it) ----
       __syncwarp();
-      if (lane < NWS) mbar_arrive(bar + (gb % kNB) * NWS + lane);
+      named_arrive(1 + gb % kNBr, sync_threads);
     }
   }
 }

@@ -10,4 +10,12 @@ ChainFn chain_lookup_v2(int nv, int lps, int mode) {
   PDP_CHAIN_CASE(2, 16, 32)
   return nullptr;
 }
+DenseFn dense_lookup_v2(int nv, int mode) {
+  PDP_DENSE_CASE(2, 1)
+  PDP_DENSE_CASE(2, 2)
+  PDP_DENSE_CASE(2, 4)
+  PDP_DENSE_CASE(2, 8)
+  PDP_DENSE_CASE(2, 16)
+  return nullptr;
+}
 }  // namespace pdp

@@ -13,4 +13,11 @@ ChainFn chain_lookup_v8(int nv, int lps, int mode) {
   PDP_CHAIN_CASE(8, 4, 32)
   return nullptr;
 }
+DenseFn dense_lookup_v8(int nv, int mode) {
+  PDP_DENSE_CASE(8, 1)
+  PDP_DENSE_CASE(8, 2)
+  PDP_DENSE_CASE(8, 3)
+  PDP_DENSE_CASE(8, 4)
+  return nullptr;
+}
 }  // namespace pdp

@@ -1,0 +1,173 @@
+// pdp_dense.cuh — dense photon counting for areas of high flux: after dark, gain and common mode every
+// pixel is divided by the single-photon gain and rounded to the nearest integer; the counts are summed over the
+// frames into a photon-counting image, optionally zeroing pixels within noise first.
+//
+// Decomposition: pixel-owner.  A warp owns one row segment (panel, row, segment) for ALL frames of the batch: its
+// pedestal and 1/gain stay in registers, its slice of the image is accumulated in registers and written once with
+// plain read-modify-write stores (no atomics: every pixel has one owner), and the common-mode estimate needs no
+// exchange because a row segment is local to the warp.  Raw pixels stream through a per-lane cp.async ring.
+// Per-frame totals are summed per CTA in shared memory and merged by a second, tiny kernel.
+#pragma once
+#include "pdp_chain.cuh"
+
+namespace pdp {
+
+constexpr int kDenseThreads = 512;
+constexpr int kDenseRing = 4;     // frames in flight per warp
+
+struct DParams {
+  const uint16_t *raw;
+  int n_frames;
+  const float *ped, *rg;
+  const double *rg64;
+  int P, H, W, S, nseg, n_tasks;
+  float T_cm, sqrtS, big, zero_below, inv_Eph;
+  double dE_ph, dzero_below;
+  int cm_mode, cm_min_count;
+  uint32_t *image;            // [npix], +=
+  uint32_t *partial_totals;   // [grid][n_frames] or nullptr
+  uint32_t *frame_totals;     // [n_frames] (merge kernel), or nullptr
+  int n_partials;
+};
+
+// V pixels per vector, NV vectors per lane (32 lanes cover S <= 32 * V * NV pixels), MODE as in pdp_chain_kernel.
+template <int V, int NV, int MODE>
+__global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DParams k) {
+  constexpr int N = V * NV;
+  constexpr uint32_t VB = V * 2;
+  constexpr uint32_t kSlot = 32u * N * 2u;
+  extern __shared__ __align__(128) unsigned char smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  uint32_t *tot = reinterpret_cast<uint32_t *>(smem);                          // [n_frames] (if wanted)
+  const uint32_t tot_bytes = k.partial_totals ? (((uint32_t)k.n_frames * 4u + 127u) & ~127u) : 0u;
+  const uint32_t ring_lane = smem_u32(smem + tot_bytes) + (uint32_t)warp * kDenseRing * kSlot + (uint32_t)lane * VB;
+  if (k.partial_totals) {
+    for (int i = threadIdx.x; i < k.n_frames; i += blockDim.x) tot[i] = 0u;
+    __syncthreads();
+  }
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  const float T_cm = k.T_cm, BIG = k.big;
+  float apr = 0.375f * T_cm / (float)k.S;
+  uint32_t vmask = 0;
+#pragma unroll
+  for (int v = 0; v < NV; ++v) vmask |= (lane * N + v * V < k.S ? 1u : 0u) << v;
+
+  for (int task = blockIdx.x * nwarps + warp; task < k.n_tasks; task += gridDim.x * nwarps) {
+    const int seg = task % k.nseg, prow = task / k.nseg;          // prow = panel * H + row
+    const size_t off = (size_t)prow * k.W + (size_t)seg * k.S + (size_t)lane * N;   // this lane's run
+    float pd[N], rg[N];
+    uint32_t acc[N];
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      const bool ok = lane * N + j < k.S;
+      pd[j] = ok ? __ldg(k.ped + off + j) : 3.0e38f;
+      rg[j] = ok ? __ldg(k.rg + off + j) : 1.f;
+      acc[j] = 0u;
+    }
+    const uint16_t *src = k.raw + off;
+    uint32_t islot = 0, rslot = 0;
+    int i_frame = 0;
+    auto issue = [&]() {
+      if (i_frame < k.n_frames) {
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+          if ((vmask >> v) & 1u) cp_async_s<VB>(ring_lane + islot + v * (32 * VB), src + v * V);
+      }
+      asm volatile("cp.async.commit_group;" ::: "memory");
+      src += npix;
+      ++i_frame;
+      islot = islot + kSlot == kDenseRing * kSlot ? 0u : islot + kSlot;
+    };
+#pragma unroll 1
+    for (int d = 0; d < kDenseRing - 1; ++d) issue();
+    for (int f = 0; f < k.n_frames; ++f) {
+      issue();
+      asm volatile("cp.async.wait_group %0;" ::"n"(kDenseRing - 1) : "memory");
+      float a[N], b[N];
+      float sb0 = 0.f, sb1 = 0.f, n0 = 0.f, s0 = 0.f;
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        uint32_t w[V / 2];
+        VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
+#pragma unroll
+        for (int e = 0; e < V; e += 2) {
+          const int j = v * V + e;
+          a[j] = (u16lo_to_f(w[e / 2]) - pd[j]) * rg[j];
+          a[j + 1] = (u16hi_to_f(w[e / 2]) - pd[j + 1]) * rg[j + 1];
+          if constexpr (MODE == 0) {
+            b[j] = fabsf(a[j]) < T_cm ? a[j] : BIG;
+            b[j + 1] = fabsf(a[j + 1]) < T_cm ? a[j + 1] : BIG;
+            sb0 += b[j];
+            sb1 += b[j + 1];
+          } else if constexpr (MODE == 1) {
+            const float m0 = set_lt_abs(a[j], T_cm), m1 = set_lt_abs(a[j + 1], T_cm);
+            n0 += m0 + m1;
+            s0 = fmaf(m0, a[j], fmaf(m1, a[j + 1], s0));
+          }
+        }
+      }
+      rslot = rslot + kSlot == kDenseRing * kSlot ? 0u : rslot + kSlot;
+      float c = 0.f;
+      if constexpr (MODE == 0) {
+        const float sb = sb0 + sb1;
+        const float n_out_l = rintf(sb * (1.f / BIG));
+        const float s_l = fmaf(-n_out_l, BIG, sb);
+        const int n = 32 * N - (int)group_count<32>(n_out_l);
+        const float tsum = group_sum<32>(s_l);
+        const bool need = n >= k.cm_min_count && n > 0;
+        c = group_median<N, 32>(b, n, tsum * rcp_approx(fmaxf((float)n, 1.f)), T_cm, BIG, need, apr);
+        if (!need) c = 0.f;
+      } else if constexpr (MODE == 1) {
+        const float n = group_count<32>(n0);
+        const float tsum = group_sum<32>(s0);
+        c = __fdiv_rn(tsum, fmaxf(n, k.sqrtS));
+      }
+      // divide by the single-photon gain and round to the nearest integer
+      int fsum = 0;
+#pragma unroll
+      for (int j = 0; j < N; ++j) {
+        const float v2 = a[j] - c;
+        const float ratio = v2 * k.inv_Eph;
+        float r = rintf(ratio);
+        // close to a rounding boundary or to the zeroing threshold: decide in double, in the oracle's order
+        if (fabsf(ratio - floorf(ratio) - 0.5f) < 2e-3f || fabsf(v2 - k.zero_below) < 1e-2f) {
+          const size_t gi = off + j;
+          if (lane * N + j < k.S) {
+            const double x = ((double)__ldg(k.raw + (size_t)f * npix + gi) - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - (double)c;
+            const double rr = rint(x / k.dE_ph);
+            r = x < k.dzero_below ? 0.f : (float)rr;
+          }
+        } else if (v2 < k.zero_below) {
+          r = 0.f;
+        }
+        const int n_px = r > 0.f ? (int)r : 0;
+        acc[j] += (uint32_t)n_px;
+        fsum += n_px;
+      }
+      if (k.partial_totals) {
+        const int ft = __reduce_add_sync(FULL, fsum);
+        if (lane == 0 && ft) atomicAdd(&tot[f], (uint32_t)ft);   // shared memory
+      }
+    }
+    // drain the ring bookkeeping (the copies issued beyond the last frame were empty groups)
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+    for (int j = 0; j < N; ++j)
+      if (lane * N + j < k.S && acc[j]) k.image[off + j] += acc[j];
+  }
+  if (k.partial_totals) {
+    __syncthreads();
+    uint32_t *out = k.partial_totals + (size_t)blockIdx.x * k.n_frames;
+    for (int i = threadIdx.x; i < k.n_frames; i += blockDim.x) out[i] = tot[i];
+  }
+}
+
+static __global__ void pdp_dense_totals_kernel(const DParams k) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= k.n_frames) return;
+  uint32_t s = 0;
+  for (int c = 0; c < k.n_partials; ++c) s += k.partial_totals[(size_t)c * k.n_frames + f];
+  k.frame_totals[f] = s;
+}
+
+}  // namespace pdp

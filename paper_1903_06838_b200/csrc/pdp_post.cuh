@@ -53,4 +53,68 @@ __global__ void __launch_bounds__(kPostThreads, 1) pdp_accum_kernel(const PostPa
     if (acc[i]) q.accum[lo + i] += acc[i];
 }
 
+// ---- histogram summarization ("functions for histogramming"; L109 Fig. 7 energy spectrum;
+// L113 Fig. 8 centroid histogram) -----------------------------------------------------------------------------
+// Uniform bins [lo + b*w, lo + (b+1)*w): b = floor((x - lo) / w) evaluated in double on the stored float32 value,
+// values outside are dropped.  pdp_hist_kernel: CTA c takes the frames c, c + grid, ...; a warp walks a frame's
+// list with coalesced loads and adds to privatised histograms in shared memory; the CTA's partial histograms go
+// to a workspace with plain stores.  pdp_hist_merge_kernel: one thread per bin adds the partials to the caller's
+// histogram (every bin has one owner: no global atomics).
+struct HistParams {
+  int n_frames;
+  uint32_t cap;
+  const uint32_t *hit_count;
+  const float *hit_charge, *hit_dx, *hit_dy;
+  double e_lo, e_w, d_lo, d_w;
+  int e_bins, d_bins;          // 0: that histogram is not wanted
+  uint32_t *partial;           // [grid][e_bins + 2 * d_bins]
+  uint32_t *hist_e, *hist_dx, *hist_dy;
+  int n_partials;
+};
+
+__device__ __forceinline__ int hist_bin(float x, double lo, double w, int nbins) {
+  const double b = floor(((double)x - lo) / w);
+  return (b >= 0.0 && b < (double)nbins) ? (int)b : -1;
+}
+
+__global__ void __launch_bounds__(kPostThreads, 1) pdp_hist_kernel(const HistParams q) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  uint32_t *h = reinterpret_cast<uint32_t *>(smem);
+  const int total = q.e_bins + 2 * q.d_bins;
+  for (int i = threadIdx.x; i < total; i += blockDim.x) h[i] = 0u;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+  for (int f = blockIdx.x + warp * gridDim.x; f < q.n_frames; f += nwarps * gridDim.x) {
+    const uint32_t cnt = min(q.hit_count[f], q.cap);
+    const size_t base = (size_t)f * q.cap;
+    for (uint32_t i = lane; i < cnt; i += 32) {
+      if (q.e_bins) {
+        const int b = hist_bin(__ldg(q.hit_charge + base + i), q.e_lo, q.e_w, q.e_bins);
+        if (b >= 0) atomicAdd(&h[b], 1u);
+      }
+      if (q.d_bins) {
+        const int bx = hist_bin(__ldg(q.hit_dx + base + i), q.d_lo, q.d_w, q.d_bins);
+        const int by = hist_bin(__ldg(q.hit_dy + base + i), q.d_lo, q.d_w, q.d_bins);
+        if (bx >= 0) atomicAdd(&h[q.e_bins + bx], 1u);
+        if (by >= 0) atomicAdd(&h[q.e_bins + q.d_bins + by], 1u);
+      }
+    }
+  }
+  __syncthreads();
+  uint32_t *out = q.partial + (size_t)blockIdx.x * total;
+  for (int i = threadIdx.x; i < total; i += blockDim.x) out[i] = h[i];
+}
+
+__global__ void pdp_hist_merge_kernel(const HistParams q) {
+  const int total = q.e_bins + 2 * q.d_bins;
+  const int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= total) return;
+  uint32_t s = 0;
+  for (int c = 0; c < q.n_partials; ++c) s += q.partial[(size_t)c * total + b];
+  if (!s) return;
+  if (b < q.e_bins) q.hist_e[b] += s;
+  else if (b < q.e_bins + q.d_bins) q.hist_dx[b - q.e_bins] += s;
+  else q.hist_dy[b - q.e_bins - q.d_bins] += s;
+}
+
 }  // namespace pdp
