@@ -37,8 +37,8 @@ constexpr int kFCH = 16;          // frame slots per chunk
 constexpr int kRingD = 2;         // raw-pixel ring depth in steps (kRingD - 1 steps of prefetch in flight; a step of a warp
                                   // lasts microseconds because the sub-partition's other warps run in between)
 constexpr int kMaxIt = 7;         // counting passes before the search switches to walking / bisection
-constexpr int kListCap = 32 * 16; // candidates of 32 items (at most 16 pixels each)
-constexpr int kItemCap = 128;     // flagged units expanded per batch by a sparse warp
+constexpr int kListCap = 3 * 32 * 16;   // candidate list: at least one more group of 32 items (<= 16 pixels each) always fits
+constexpr int kItemCap = 256;     // flagged units expanded per batch by a sparse warp
 constexpr int kChainMaxThreads = 640;
 constexpr int kMaxSparseWarps = 8;
 
@@ -379,13 +379,18 @@ __device__ __forceinline__ float group_median(const float (&b)[N], int n, float 
 }
 
 // fp64 evaluation of the 3x3 window of (row, col) of panel p: v2 = (raw - ped) * (1/gain) - c with the
-// common-mode estimates of the three rows passed as pointers (nullptr: the row does not exist).
+// common-mode estimates of the three rows passed as pointers (rows that do not exist: any valid pointer).
+// Branch-free: neighbours outside the panel are loaded from clamped coordinates and masked afterwards, so that
+// all 27 loads of a candidate are in flight together (one L2 round trip per batch of 32 candidates).
 __device__ __forceinline__ Exact9 exact9_rows(const CParams &k, const uint16_t *frame_raw, const float *cm_m1,
                                               const float *cm_0, const float *cm_p1, int p, int row, int col) {
   const int sgc = col / k.S, cs = col - sgc * k.S;
-  const int sg3[3] = {cs == 0 ? sgc - 1 : sgc, sgc, cs == k.S - 1 ? sgc + 1 : sgc};
+  const int sg3[3] = {max(cs == 0 ? sgc - 1 : sgc, 0), sgc, min(cs == k.S - 1 ? sgc + 1 : sgc, k.nseg - 1)};
   const float *cmr[3] = {cm_m1, cm_0, cm_p1};
-  double v[9];
+  const uint32_t prow = (uint32_t)p * (uint32_t)k.H;
+  unsigned rawv[9];
+  float pedv[9], cmv[9];
+  double rgv[9];
   bool ex[9];
 #pragma unroll
   for (int dr = -1; dr <= 1; ++dr)
@@ -394,14 +399,15 @@ __device__ __forceinline__ Exact9 exact9_rows(const CParams &k, const uint16_t *
       const int i = (dr + 1) * 3 + dc + 1;
       const int r = row + dr, c = col + dc;
       ex[i] = (r >= 0 && r < k.H && c >= 0 && c < k.W);
-      v[i] = 0.0;
-      if (ex[i]) {
-        const size_t gi = ((size_t)p * k.H + r) * k.W + c;
-        const unsigned rawv = __ldg(frame_raw + gi);
-        const double cm = (double)cmr[dr + 1][sg3[dc + 1]];
-        v[i] = ((double)rawv - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - cm;
-      }
+      const uint32_t gi = (prow + (uint32_t)min(max(r, 0), k.H - 1)) * (uint32_t)k.W + (uint32_t)min(max(c, 0), k.W - 1);
+      rawv[i] = __ldg(frame_raw + gi);
+      pedv[i] = __ldg(k.ped + gi);
+      rgv[i] = __ldg(k.rg64 + gi);
+      cmv[i] = cmr[dr + 1][sg3[dc + 1]];
     }
+  double v[9];
+#pragma unroll
+  for (int i = 0; i < 9; ++i) v[i] = ex[i] ? ((double)rawv[i] - (double)pedv[i]) * rgv[i] - (double)cmv[i] : 0.0;
   Exact9 o;
   const double x = v[4];
   o.seed = x > k.dT_seed;
@@ -410,14 +416,13 @@ __device__ __forceinline__ Exact9 exact9_rows(const CParams &k, const uint16_t *
   o.sy = 0.0;
 #pragma unroll
   for (int i = 0; i < 9; ++i) {
-    if (!ex[i]) continue;
-    const double y = v[i];
+    const double y = v[i];     // 0 for a missing neighbour: adds nothing to the sums
     o.E += y;
     o.sx += (double)(i % 3 - 1) * y;
     o.sy += (double)(i / 3 - 1) * y;
     if (i == 4) continue;
     // strict maximum; a tie goes to the lower linear index (i < 4 <=> neighbour has lower index)
-    if (!(x > y || (x == y && i > 4))) o.seed = false;
+    if (ex[i] && !(x > y || (x == y && i > 4))) o.seed = false;
   }
   return o;
 }
@@ -539,7 +544,121 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
     ns = 0;
   };
 
-  // ---- 1-3 over the (frame, row, segment) tasks in output order ----
+  // ---- 3: exact evaluation of the candidate list, full batches of 32 ----
+  int ncand = 0;            // candidates in the list (warp-uniform)
+  auto eval_cands = [&]() {
+    for (int c0 = 0; c0 < ncand; c0 += 32) {
+      const bool have = c0 + lane < ncand;
+      const uint32_t ce = have ? cand[c0 + lane] : 0u;
+      const int q = (int)(ce >> 28), row = ra + (int)((ce >> 20) & 0xffu), col = (int)(ce & 0xfffffu);
+      bool seed = false;
+      HitRec h{0.f, 0.f, 0.f, 0};
+#ifdef PDP_DBG_SKIP_EXACT
+      if (false) {
+#else
+      if (have) {
+#endif
+        const float *cmf = cmring + (size_t)q * ring_rows * k.nseg;
+        const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
+        const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : cm_0;
+        const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : cm_0;
+        const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + q) * npix, cm_m1, cm_0, cm_p1, p, row, col);
+        seed = e9.seed;
+        if (seed) h = make_rec(e9, k.dE_ph);
+      }
+      const unsigned sm = __ballot_sync(FULL, seed);
+      if (!sm) continue;
+      if (ns + __popc(sm) > kSeedCap) flush();
+      if (seed) {
+        const int o = ns + __popc(sm & ((1u << lane) - 1u));
+        s_pix[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
+        s_E[o] = h.E;
+        s_n[o] = h.n;
+        s_dx[o] = h.dx;
+        s_dy[o] = h.dy;
+        s_q[o] = (uint32_t)q;
+      }
+      ns += __popc(sm);
+      __syncwarp();
+    }
+    ncand = 0;
+  };
+
+  // ---- 2: pixel test of the item list, then the candidates of the items, in order, into the candidate list ----
+  int n_items = 0;          // items in the list (warp-uniform)
+  auto process_items = [&]() {
+    const int nb = n_items;
+    for (int i = lane; i < nb; i += 32) imask[i] = 0u;
+    __syncwarp();
+    // a lane takes kPxU (item, pixel pair) tasks at a time and issues all their loads before it tests any of them;
+    // consecutive lanes take consecutive pairs of an item (coalesced 4-/8-byte loads)
+    constexpr int PP = U / 2, kPxU = 8;
+    const int n_px_tasks = nb * PP;
+    for (int u0 = 0; u0 < n_px_tasks; u0 += 32 * kPxU) {
+      uint32_t w[kPxU];
+      float2 mk[kPxU], rg[kPxU], nf2[kPxU];
+      float thr[kPxU];
+      int itu[kPxU], pju[kPxU];
+#pragma unroll
+      for (int u = 0; u < kPxU; ++u) {   // branch-free: out-of-range tasks load the last valid pair and are dropped
+        const int tt = u0 + u * 32 + lane;
+        const int tc = min(tt, n_px_tasks - 1);
+        const int it = tc / PP, pj = tc - it * PP;
+        const uint32_t e = items[it];
+        const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
+        const int l = fb / NU, un = fb - l * NU;
+        const int j = un * U + 2 * pj;                 // pixel of the lane's run
+        const int col = sg * k.S + l * N + j;
+        const bool ok = tt < n_px_tasks && j < N && col < (sg + 1) * k.S;
+        const int row = ra + rr;
+        const uint32_t gi = ((uint32_t)p * (uint32_t)k.H + (uint32_t)row) * (uint32_t)k.W + (uint32_t)min(col, k.W - 2);
+        w[u] = __ldg(reinterpret_cast<const uint32_t *>(k.raw + (size_t)(f0 + q) * npix + gi));
+        mk[u] = __ldg(reinterpret_cast<const float2 *>(k.mapK + gi));
+        rg[u] = __ldg(reinterpret_cast<const float2 *>(k.rg + gi));
+        nf2[u] = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + gi));
+        thr[u] = k.cand_thr + cmring[((size_t)q * ring_rows + slot_of(row)) * k.nseg + sg];
+        itu[u] = ok ? it : -1;
+        pju[u] = pj;
+      }
+#pragma unroll
+      for (int u = 0; u < kPxU; ++u) {
+        if (itu[u] >= 0) {
+          const float a0 = fmaf(magic_lo(w[u]) - mk[u].x, rg[u].x, nf2[u].x);
+          const float a1 = fmaf(magic_hi(w[u]) - mk[u].y, rg[u].y, nf2[u].y);
+          const uint32_t bb = (a0 > thr[u] ? 1u : 0u) | (a1 > thr[u] ? 2u : 0u);
+          if (bb) atomicOr(&imask[itu[u]], bb << (2 * pju[u]));
+        }
+      }
+    }
+    __syncwarp();
+    for (int i0 = 0; i0 < nb; i0 += 32) {
+      const bool hv = i0 + lane < nb;
+      const uint32_t m = hv ? imask[i0 + lane] : 0u;
+      const uint32_t e = hv ? items[i0 + lane] : 0u;
+      int cn = __popc(m), cincl = cn;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int u = __shfl_up_sync(FULL, cincl, o);
+        if (lane >= o) cincl += u;
+      }
+      const int ctotal = __shfl_sync(FULL, cincl, 31);    // <= 32 * U
+      if (ctotal) {
+        const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
+        const int l = fb / NU, un = fb - l * NU;
+        const int colb = sg * k.S + l * N + un * U;
+        int idx = ncand + cincl - cn;
+        for (uint32_t mm = m; mm; mm &= mm - 1, ++idx)
+          cand[idx] = ((uint32_t)q << 28) | ((uint32_t)rr << 20) | (uint32_t)(colb + __ffs(mm) - 1);
+        ncand += ctotal;
+        __syncwarp();
+      }
+      // evaluate when the next group of items might not fit, and at the end
+      if (ncand > kListCap - 32 * U || (i0 + 32 >= nb && ncand)) eval_cands();
+    }
+    n_items = 0;
+  };
+
+  // ---- 1: flagged units of all (frame, row, segment) tasks of the call, in output order, into the item list ----
   const int n_ft = nrows > 0 ? nf * nrows * k.nseg : 0;
   for (int t0 = 0; t0 < n_ft; t0 += 32) {
     const int t = t0 + lane;
@@ -552,6 +671,9 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
       trr = u - tq * nrows;
       fw = flags[((size_t)tq * ring_rows + slot_of(ra + trr)) * k.nseg + tsg];
     }
+#ifdef PDP_DBG_SKIP_PX
+    fw = 0ull;
+#endif
     if (!__any_sync(FULL, fw != 0ull)) continue;
     int mine_n = __popcll(fw), incl = mine_n;
 #pragma unroll
@@ -561,117 +683,21 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
     }
     const int total = __shfl_sync(FULL, incl, 31);
     const int first = incl - mine_n;
-    for (int b0 = 0; b0 < total; b0 += kItemCap) {
-      // ---- 1: items [b0, b0 + kItemCap) of this group of tasks ----
-      if (first < b0 + kItemCap && first + mine_n > b0) {
+    for (int b0 = 0; b0 < total;) {
+      if (n_items == kItemCap) process_items();
+      const int take = min(kItemCap - n_items, total - b0);   // items [b0, b0 + take) of this group of tasks
+      if (first < b0 + take && first + mine_n > b0) {
         int idx = first;
         for (unsigned long long m = fw; m; m &= m - 1, ++idx)
-          if (idx >= b0 && idx < b0 + kItemCap)   // flag bit = lane-in-group * NU + unit: ascending bits = ascending columns
-            items[idx - b0] = ((uint32_t)tq << 24) | ((uint32_t)trr << 16) | ((uint32_t)tsg << 8) | (uint32_t)(__ffsll((long long)m) - 1);
+          if (idx >= b0 && idx < b0 + take)   // flag bit = lane-in-group * NU + unit: ascending bits = ascending columns
+            items[n_items + idx - b0] = ((uint32_t)tq << 24) | ((uint32_t)trr << 16) | ((uint32_t)tsg << 8) | (uint32_t)(__ffsll((long long)m) - 1);
       }
-      const int nb = min(kItemCap, total - b0);
-      for (int i = lane; i < nb; i += 32) imask[i] = 0u;
-      __syncwarp();
-      // ---- 2: pixel test; a lane takes kPxU (item, pixel pair) tasks at a time, all loads first ----
-      constexpr int PP = U / 2, kPxU = 8;
-      const int n_px_tasks = nb * PP;
-      for (int u0 = 0; u0 < n_px_tasks; u0 += 32 * kPxU) {
-        uint32_t w[kPxU];
-        float2 mk[kPxU], rg[kPxU], nf2[kPxU];
-        float thr[kPxU];
-        int itu[kPxU], pju[kPxU];
-#pragma unroll
-        for (int u = 0; u < kPxU; ++u) {
-          const int tt = u0 + u * 32 + lane;
-          itu[u] = -1;
-          if (tt < n_px_tasks) {
-            const int it = tt / PP, pj = tt - it * PP;
-            const uint32_t e = items[it];
-            const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
-            const int l = fb / NU, un = fb - l * NU;
-            const int j = un * U + 2 * pj;                 // pixel of the lane's run
-            const int col = sg * k.S + l * N + j;
-            if (j < N && col < (sg + 1) * k.S) {
-              const int row = ra + rr;
-              const size_t gi = ((size_t)p * k.H + row) * k.W + col;
-              w[u] = __ldg(reinterpret_cast<const uint32_t *>(k.raw + (size_t)(f0 + q) * npix + gi));
-              mk[u] = __ldg(reinterpret_cast<const float2 *>(k.mapK + gi));
-              rg[u] = __ldg(reinterpret_cast<const float2 *>(k.rg + gi));
-              nf2[u] = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + gi));
-              thr[u] = k.cand_thr + cmring[((size_t)q * ring_rows + slot_of(row)) * k.nseg + sg];
-              itu[u] = it;
-              pju[u] = pj;
-            }
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < kPxU; ++u) {
-          if (itu[u] >= 0) {
-            const float a0 = fmaf(magic_lo(w[u]) - mk[u].x, rg[u].x, nf2[u].x);
-            const float a1 = fmaf(magic_hi(w[u]) - mk[u].y, rg[u].y, nf2[u].y);
-            const uint32_t bb = (a0 > thr[u] ? 1u : 0u) | (a1 > thr[u] ? 2u : 0u);
-            if (bb) atomicOr(&imask[itu[u]], bb << (2 * pju[u]));
-          }
-        }
-      }
-      __syncwarp();
-      // ---- candidates of the items, in order, kListCap at a time -> 3: exact evaluation ----
-      for (int i0 = 0; i0 < nb; i0 += 32) {
-        const bool hv = i0 + lane < nb;
-        const uint32_t m = hv ? imask[i0 + lane] : 0u;
-        const uint32_t e = hv ? items[i0 + lane] : 0u;
-        int cn = __popc(m), cincl = cn;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const int u = __shfl_up_sync(FULL, cincl, o);
-          if (lane >= o) cincl += u;
-        }
-        const int ctotal = __shfl_sync(FULL, cincl, 31);
-        if (ctotal == 0) continue;
-        const int cfirst = cincl - cn;
-        {
-          const int q = (int)(e >> 24), rr = (int)((e >> 16) & 0xffu), sg = (int)((e >> 8) & 0xffu), fb = (int)(e & 0xffu);
-          const int l = fb / NU, un = fb - l * NU;
-          const int colb = sg * k.S + l * N + un * U;
-          int idx = cfirst;
-          for (uint32_t mm = m; mm; mm &= mm - 1, ++idx)      // ctotal <= 32 * U <= kListCap
-            cand[idx] = ((uint32_t)q << 28) | ((uint32_t)rr << 20) | (uint32_t)(colb + __ffs(mm) - 1);
-        }
-        __syncwarp();
-        for (int c0 = 0; c0 < ctotal; c0 += 32) {
-          const bool have = c0 + lane < ctotal;
-          const uint32_t ce = have ? cand[c0 + lane] : 0u;
-          const int q = (int)(ce >> 28), row = ra + (int)((ce >> 20) & 0xffu), col = (int)(ce & 0xfffffu);
-          bool seed = false;
-          HitRec h{0.f, 0.f, 0.f, 0};
-          if (have) {
-            const float *cmf = cmring + (size_t)q * ring_rows * k.nseg;
-            const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
-            const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : nullptr;
-            const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : nullptr;
-            const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + q) * npix, cm_m1, cm_0, cm_p1, p, row, col);
-            seed = e9.seed;
-            if (seed) h = make_rec(e9, k.dE_ph);
-          }
-          const unsigned sm = __ballot_sync(FULL, seed);
-          if (!sm) continue;
-          if (ns + __popc(sm) > kSeedCap) flush();
-          if (seed) {
-            const int o = ns + __popc(sm & ((1u << lane) - 1u));
-            s_pix[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
-            s_E[o] = h.E;
-            s_n[o] = h.n;
-            s_dx[o] = h.dx;
-            s_dy[o] = h.dy;
-            s_q[o] = (uint32_t)q;
-          }
-          ns += __popc(sm);
-          __syncwarp();
-        }
-      }
+      n_items += take;
+      b0 += take;
       __syncwarp();
     }
   }
+  if (n_items) process_items();
   flush();   // also waits for the band before when nothing was buffered: the running totals are passed on in order
   if (lane < nf) {
     const uint32_t cnt = base_s[lane], pht = phot[lane] + pht_s[lane];
