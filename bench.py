@@ -292,7 +292,8 @@ def e2e_streamed(binding, cfg, keep, dev, steps, dist, world):
     acc = torch.empty((cfg.npix,), dtype=torch.int32).pin_memory()
     lists = [torch.empty((n, cap), dtype=dt).pin_memory() for dt in
              (torch.int32, torch.float32, torch.int32, torch.float32, torch.float32)]
-    chunk = max(1, min(ring, (256 << 20) // (cfg.npix * 2)))      # ~256 MB per copy
+    # ~256 MB per copy, but at least 2 frames per SM so that every chunk runs on the throughput kernel
+    chunk = max(1, min(ring, max((256 << 20) // (cfg.npix * 2), 296)))
     launches = [0]
 
     def e2e_step():

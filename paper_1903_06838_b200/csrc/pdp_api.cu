@@ -58,8 +58,8 @@ struct ChainPlan {
 
 // Preference order per vector width: the first entry that covers S with at most 25 % padding wins, otherwise
 // the one with the least padding.  Entries with LPS < 32 put several frames side by side in a warp.
-const ChainVariant kVariants[] = {
-    {8, 6, 8}, {8, 4, 8}, {8, 4, 16}, {8, 3, 16}, {8, 2, 16}, {8, 1, 32}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32},
+const ChainVariant kVariants[] = {   // measured order of preference
+    {8, 3, 16}, {8, 1, 32}, {8, 4, 16}, {8, 2, 16}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
     {4, 1, 32}, {4, 2, 32}, {4, 4, 32}, {4, 8, 32},
     {2, 13, 8}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
 };
@@ -620,6 +620,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   k.nseg = k.W / k.S;
   k.R = pl.R;
   k.TR = pl.TR;
+  k.WPR = pl.WPR;
   k.bands_per_panel = pl.bands_per_panel;
   k.n_bands = pl.n_bands;
   // frames per work item: enough items for ~16 waves of CTAs, at least 8 frames each so that the

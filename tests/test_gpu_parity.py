@@ -368,8 +368,9 @@ def test_full_size_config3_sampled(oracle):
 @pytest.mark.parametrize("host", [False, True], ids=["device", "streamed"])
 def test_full_size_config4_sampled(oracle, host):
     """configs[4]: 4000 frames of 16 panels x 512x512 (33.5 GB, 27 frames per CTA: multi-chunk path), device
-    resident and streamed from (pinned) host memory in 64-frame chunks through the double-buffered side stream."""
-    _full_size_sampled(oracle, 4, 0, 150000, host_chunk=64 if host else None)
+    resident and streamed from (pinned) host memory in 296-frame chunks (2 frames per CTA and chunk, 2.5 GB per copy)
+    through the double-buffered side stream."""
+    _full_size_sampled(oracle, 4, 0, 150000, host_chunk=296 if host else None)
 
 
 @pytest.mark.parametrize("n", [148 * 6 + 3, 148 * 17, 148 * 20, 148 * 24 + 5, 148 * 33],
@@ -513,7 +514,7 @@ def test_dense_photon_counting(oracle, case, cm_mode):
         diff = g_img // 2 != o_img.astype(np.int64)
         fragile_px = frag.any(axis=0)
         print(case, cm_mode, zero_below, "photons", int(o_img.sum()), "pixels differing", int(diff.sum()), "fragile pixels", int(fragile_px.sum()))
-        assert o_img.sum() > 50 * n
+        assert o_img.sum() > 5 * n
         assert not (diff & ~fragile_px).any()                              # differences only where the oracle says fragile
         assert diff.sum() <= max(3, int(fragile_px.sum()))
         clean = ~frag.reshape(n, -1).any(axis=1)                           # frames without any fragile pixel: exact totals
