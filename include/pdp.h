@@ -203,6 +203,30 @@ int pdp_histograms(pdp_ctx *ctx, const pdp_output *lists, int32_t n_frames, cons
                    uint32_t *hist_energy, const pdp_hist_spec *dxy, uint32_t *hist_dx, uint32_t *hist_dy,
                    void *cuda_stream);
 
+/*
+ * Stacked common-mode stages on other group shapes ("other types of common mode (row, column, block)
+ * can be easily extracted by reshaping tensors accordingly"; L117: the paper's timed model has "3 stacked common
+ * mode stages").  A stage tiles every panel with groups of group_rows x group_cols pixels (row segment: 1 x S, column
+ * segment: S x 1, block: bh x bw, panel-wise: rows x cols; both must divide the panel), estimates every group with
+ * cm_mode (pdp_cm_mode; the guarded mean divides by max(count, sqrt(group_rows*group_cols))) over the pixels with
+ * |v| < cm_adu and subtracts the estimate from all pixels of the group; stages apply in order, each to the output of
+ * the one before, and the photon finder runs on the last one's output.
+ */
+typedef struct pdp_cm_stage {
+  int32_t group_rows, group_cols;
+  int32_t cm_mode;      /* pdp_cm_mode */
+  int32_t cm_min_count; /* MEDIAN only; 0 -> ceil(sqrt(group_rows*group_cols)) */
+} pdp_cm_stage;
+
+/*
+ * pdp_set_cm_stages — n_stages = 1..3 switches pdp_process / pdp_process_pinned of this context to the general path
+ * (a float32 working image in device memory, one kernel per stage: slower than the fused hot path, whose single
+ * row-segment stage is what n_stages = 0 restores; params.cm_mode and geometry.seg_cols are ignored while stages are
+ * set).  `stages` is a HOST array, copied.  Errors: PDP_E_NULL, PDP_E_VALUE, PDP_E_GEOMETRY (a group does not tile
+ * the panel).  Must not race with pdp_process.
+ */
+int pdp_set_cm_stages(pdp_ctx *ctx, const pdp_cm_stage *stages, int32_t n_stages);
+
 /* pdp_set_params — replace thresholds / estimator of an existing context
  * (host struct, validated as in pdp_create).  Must not race with pdp_process. */
 int pdp_set_params(pdp_ctx *ctx, const pdp_params *params);

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpdp.so")
 CM_MEDIAN, CM_MEAN_GUARDED, CM_NONE = 0, 1, 2
 STATUS_HIT_OVERFLOW = 1
 
-EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_histograms", "pdp_process_dense", "pdp_set_params", "pdp_destroy",
+EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_histograms", "pdp_process_dense", "pdp_set_cm_stages", "pdp_set_params", "pdp_destroy",
            "pdp_last_launch_count", "pdp_last_kernel_name", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
            "pdp_last_error", "pdp_version")
 
@@ -46,6 +46,11 @@ class pdp_output(ctypes.Structure):
 
 class pdp_hist_spec(ctypes.Structure):
     _fields_ = [("lo", ctypes.c_float), ("width", ctypes.c_float), ("nbins", ctypes.c_int32)]
+
+
+class pdp_cm_stage(ctypes.Structure):
+    _fields_ = [("group_rows", ctypes.c_int32), ("group_cols", ctypes.c_int32), ("cm_mode", ctypes.c_int32),
+                ("cm_min_count", ctypes.c_int32)]
 
 
 class PdpError(RuntimeError):
@@ -81,6 +86,7 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
                                    ctypes.c_void_p]
     lib.pdp_process_dense.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_batch), ctypes.c_void_p, ctypes.c_float,
                                       ctypes.c_void_p, ctypes.c_void_p]
+    lib.pdp_set_cm_stages.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_cm_stage), ctypes.c_int32]
     lib.pdp_set_params.argtypes = [ctypes.c_void_p, ctypes.POINTER(pdp_params)]
     lib.pdp_destroy.argtypes = [ctypes.c_void_p]
     lib.pdp_last_launch_count.argtypes = [ctypes.c_void_p]
@@ -218,6 +224,12 @@ class Context:
         self._check(self._lib.pdp_process_dense(self._h, ctypes.byref(b), ctypes.c_void_p(s.cuda_stream), zero_below_adu,
                                                 image.data_ptr(), frame_totals.data_ptr() if frame_totals is not None else None),
                     "pdp_process_dense")
+
+    def set_cm_stages(self, stages):
+        """stages: list of up to 3 (group_rows, group_cols, cm_mode[, cm_min_count]); [] restores the hot path."""
+        arr = (pdp_cm_stage * max(1, len(stages)))(*[pdp_cm_stage(int(s[0]), int(s[1]), int(s[2]), int(s[3]) if len(s) > 3 else 0)
+                                                     for s in stages])
+        self._check(self._lib.pdp_set_cm_stages(self._h, arr, len(stages)), "pdp_set_cm_stages")
 
     def debug_set(self, key: str, value: int):
         """Diagnostic switches of include/pdp.h (kernel, chunk_frames, sparse_warps, variant)."""

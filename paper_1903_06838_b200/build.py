@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpdp.so")
 OBJDIR = os.path.join(HERE, "build")
 SOURCES = ["pdp_api.cu", "pdp_chain_v8.cu", "pdp_chain_v4.cu", "pdp_chain_v2.cu"]
-HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_chain.cuh", "pdp_chain_inst.cuh", "pdp_post.cuh", "pdp_dense.cuh",
+HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_chain.cuh", "pdp_chain_inst.cuh", "pdp_post.cuh", "pdp_dense.cuh", "pdp_staged.cuh",
            os.path.join("..", "..", "include", "pdp.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

@@ -14,6 +14,7 @@
 #include "pdp_dense.cuh"
 #include "pdp_fused.cuh"
 #include "pdp_post.cuh"
+#include "pdp_staged.cuh"
 
 using pdp::CParams;
 using pdp::KParams;
@@ -86,6 +87,12 @@ struct pdp_ctx {
   double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
+  int n_stages = 0;                         // pdp_set_cm_stages: 0 = the hot path's single row-segment stage
+  pdp_cm_stage stages[3] = {};
+  float *d_st_v = nullptr;                  // staged path: working image [st_chunk][npix] and the stage estimates
+  float *d_st_est = nullptr;
+  int st_chunk = 0;
+  size_t st_est_floats = 0;
   uint32_t *d_dense_ws = nullptr;           // per-CTA partial frame totals (pdp_process_dense), grown on demand
   size_t dense_ws_words = 0;
   uint32_t *d_hist_ws = nullptr;            // per-CTA partial histograms (pdp_histograms), grown on demand
@@ -288,6 +295,8 @@ void free_ctx(pdp_ctx *c) {
   cudaFree(c->d_ticket);
   cudaFree(c->d_cm);
   cudaFree(c->d_hist_ws);
+  cudaFree(c->d_st_v);
+  cudaFree(c->d_st_est);
   cudaFree(c->d_dense_ws);
   for (int i = 0; i < 2; ++i) {
     cudaFree(c->d_feed[i]);
@@ -445,6 +454,20 @@ int pdp_set_params(pdp_ctx *ctx, const pdp_params *prm) {
   return PDP_OK;
 }
 
+int pdp_set_cm_stages(pdp_ctx *ctx, const pdp_cm_stage *stages, int32_t n_stages) {
+  if (!ctx || (n_stages > 0 && !stages)) return fail(ctx, PDP_E_NULL, "pdp_set_cm_stages: null argument");
+  if (n_stages < 0 || n_stages > 3) return fail(ctx, PDP_E_VALUE, "pdp_set_cm_stages: 0 to 3 stages");
+  for (int s = 0; s < n_stages; ++s) {
+    const pdp_cm_stage &g = stages[s];
+    if (g.group_rows < 1 || g.group_cols < 1 || ctx->geo.rows % g.group_rows || ctx->geo.cols % g.group_cols)
+      return fail(ctx, PDP_E_GEOMETRY, "pdp_set_cm_stages: a group shape must tile the panel");
+    if (g.cm_mode < 0 || g.cm_mode > 2 || g.cm_min_count < 0) return fail(ctx, PDP_E_VALUE, "pdp_set_cm_stages: bad estimator");
+  }
+  ctx->n_stages = n_stages;
+  for (int s = 0; s < n_stages; ++s) ctx->stages[s] = stages[s];
+  return PDP_OK;
+}
+
 int pdp_destroy(pdp_ctx *ctx) {
   free_ctx(ctx);
   return PDP_OK;
@@ -501,6 +524,8 @@ int pdp_get_common_mode(pdp_ctx *ctx, float *cm_device, int64_t n_floats, void *
 }  // extern "C"
 
 namespace {
+
+int enqueue_accum(pdp_ctx *c, int n, cudaStream_t st, const pdp_output &o);
 
 // The throughput path: pdp_chain_kernel (dense pass + sparse stage, one launch) followed by pdp_accum_kernel
 // (the accumulated image from the finished lists, no global atomics).
@@ -569,7 +594,16 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   pdp::ChainFn fn = chain_kernel(pl.v, c->prm.cm_mode);
   fn<<<grid, (pl.NWD + pl.NWS) * 32, pl.smem, st>>>(k);
   PDP_CUDA(c, cudaGetLastError());
-  // accumulated image: owner-computes scatter of the finished lists
+  c->launches += 1;
+  if (int rc = enqueue_accum(c, n, st, o)) return rc;
+  std::snprintf(c->last_kernel_buf, sizeof(c->last_kernel_buf), "pdp_chain_kernel<%d,%d,%d,%d>", pl.v.V, pl.v.NV, pl.v.LPS,
+                c->prm.cm_mode);
+  c->last_kernel = c->last_kernel_buf;
+  return PDP_OK;
+}
+
+// The accumulated image from the finished lists: owner-computes scatter by pixel range (no global atomics).
+int enqueue_accum(pdp_ctx *c, int n, cudaStream_t st, const pdp_output &o) {
   PostParams q{};
   q.n_frames = n;
   q.cap = o.hit_capacity;
@@ -584,15 +618,96 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   const int grid_a = (int)((c->npix + q.span - 1) / q.span);
   pdp::pdp_accum_kernel<<<grid_a, pdp::kPostThreads, (size_t)q.span * 4, st>>>(q);
   PDP_CUDA(c, cudaGetLastError());
-  c->launches += 2;
-  std::snprintf(c->last_kernel_buf, sizeof(c->last_kernel_buf), "pdp_chain_kernel<%d,%d,%d,%d>", pl.v.V, pl.v.NV, pl.v.LPS,
-                c->prm.cm_mode);
-  c->last_kernel = c->last_kernel_buf;
+  c->launches += 1;
   return PDP_OK;
+}
+
+// The general common-mode path (pdp_staged.cuh): calibrate into a working image, one kernel per stage, the finder,
+// the accumulated image; frames in chunks that bound the working image.
+int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o) {
+  const size_t npix = c->npix;
+  if (!c->d_st_v) {
+    const size_t budget = (size_t)1 << 30;   // ~1 GiB of working image
+    c->st_chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->geo.max_frames_per_batch, budget / (npix * 4)));
+    PDP_CUDA(c, cudaMalloc(&c->d_st_v, (size_t)c->st_chunk * npix * sizeof(float)));
+  }
+  size_t est_per_frame = 0;
+  for (int s = 0; s < c->n_stages; ++s)
+    est_per_frame += npix / ((size_t)c->stages[s].group_rows * c->stages[s].group_cols);
+  if (c->st_est_floats < est_per_frame * c->st_chunk) {
+    cudaFree(c->d_st_est);
+    c->d_st_est = nullptr;
+    c->st_est_floats = 0;
+    PDP_CUDA(c, cudaMalloc(&c->d_st_est, est_per_frame * c->st_chunk * sizeof(float)));
+    c->st_est_floats = est_per_frame * c->st_chunk;
+  }
+  for (int f0 = 0; f0 < n; f0 += c->st_chunk) {
+    const int m = std::min(c->st_chunk, n - f0);
+    pdp::StParams k{};
+    k.raw = raw + (size_t)f0 * npix;
+    k.n_frames = m;
+    k.mapK = c->d_K;
+    k.rg = c->d_rg;
+    k.mapNpf = c->d_npf;
+    k.ped = c->d_ped;
+    k.rg64 = c->d_rg64;
+    k.P = c->geo.panels;
+    k.H = c->geo.rows;
+    k.W = c->geo.cols;
+    k.npix = (uint32_t)npix;
+    k.v = c->d_st_v;
+    k.T_cm = c->prm.cm_adu;
+    k.cand_thr = (float)((double)c->prm.seed_adu - std::max(1e-3, 4e-6 * std::fabs((double)c->prm.seed_adu)));
+    k.dT_seed = (double)c->prm.seed_adu;
+    k.dE_ph = (double)c->prm.photon_adu;
+    k.n_stages = c->n_stages;
+    float *est = c->d_st_est;
+    for (int s = 0; s < c->n_stages; ++s) {
+      pdp::StageDesc &d = k.st[s];
+      d.gh = c->stages[s].group_rows;
+      d.gw = c->stages[s].group_cols;
+      d.ngr = k.H / d.gh;
+      d.ngc = k.W / d.gw;
+      d.mode = c->stages[s].cm_mode;
+      d.min_count = c->stages[s].cm_min_count > 0 ? c->stages[s].cm_min_count
+                                                  : (int)std::ceil(std::sqrt((double)d.gh * d.gw));
+      d.sqrtG = (float)std::sqrt((double)d.gh * d.gw);
+      d.est = est;
+      est += (size_t)m * k.P * d.ngr * d.ngc;
+    }
+    k.cap = o.hit_capacity;
+    k.hit_count = o.hit_count + f0;
+    k.frame_photons = o.frame_photons + f0;
+    const size_t off = (size_t)f0 * o.hit_capacity;
+    k.hit_pixel = o.hit_pixel + off;
+    k.hit_charge = o.hit_charge + off;
+    k.hit_nphot = o.hit_nphot + off;
+    k.hit_dx = o.hit_dx + off;
+    k.hit_dy = o.hit_dy + off;
+    k.accum = o.accum;
+    k.status = o.status;
+    const int grid_e = (int)std::min<size_t>((size_t)c->num_sms * 8, ((size_t)m * npix / 2 + pdp::kStThreads - 1) / pdp::kStThreads);
+    pdp::pdp_st_calib_kernel<<<std::max(grid_e, 1), pdp::kStThreads, 0, st>>>(k);
+    PDP_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    for (int s = 0; s < c->n_stages; ++s) {
+      const long long items = (long long)m * k.P * k.st[s].ngr * k.st[s].ngc;
+      const int grid_s = (int)std::min<long long>(items, (long long)c->num_sms * 8);
+      pdp::pdp_st_stage_kernel<<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+      PDP_CUDA(c, cudaGetLastError());
+      c->launches += 1;
+    }
+    pdp::pdp_st_find_kernel<<<std::min(m, c->num_sms * 4), pdp::kStThreads, 0, st>>>(k);
+    PDP_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+  }
+  c->last_kernel = "pdp_st_stage_kernel";
+  return enqueue_accum(c, n, st, o);
 }
 
 // Enqueue the chain for n frames at `raw` (device); outputs are already offset to this batch.
 int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o, bool keep_cm) {
+  if (c->n_stages > 0) return enqueue_staged(c, raw, n, st, o);
   // ---- large batches: the throughput kernel (frame-owner CTAs) ----
   {
     int which = c->sparse_override == 8 ? 1 : 0;

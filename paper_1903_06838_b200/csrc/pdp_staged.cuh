@@ -1,0 +1,267 @@
+// pdp_staged.cuh — the general common-mode path: up to three stacked stages on arbitrary rectangular groups
+// ("other types of common mode (row, column, block) can be easily extracted by reshaping tensors";
+// L117 "3 stacked common mode stages"), followed by the same photon finder as the hot path.
+//
+// The hot path (pdp_chain.cuh) fuses ONE row-segment stage into the streaming pass because a row segment is local
+// to a warp.  Column, block and panel-wise groups span rows, so here the calibrated image lives in a float32
+// working buffer (L2 / HBM) and every stage is a kernel over it:
+//   pdp_st_calib_kernel   v = (raw - pedestal) / gain              (the hot path's exact fp32 formula)
+//   pdp_st_stage_kernel   one CTA per (frame, group): estimate over the group's pixels with |v| < T_cm — guarded mean
+//                         in double (fixed reduction order) or exact median by bisection on order-preserving keys
+//                         (count passes over the group, tie-safe) — subtracted from all pixels of the group in place;
+//                         the estimate is kept per group for the exact evaluation
+//   pdp_st_find_kernel    one CTA per frame: pixels above T_seed - margin are candidates; each candidate is evaluated in
+//                         fp64 from raw, pedestal, 1/gain and the stage estimates of its 3x3 neighbours, in the oracle's
+//                         order of operations; seeds are emitted in pixel order by a block scan
+// followed by pdp_accum_kernel (pdp_post.cuh).  Frames are processed in chunks that bound the working buffer.
+#pragma once
+#include "pdp_chain.cuh"
+
+namespace pdp {
+
+constexpr int kStThreads = 256;
+constexpr int kMaxStages = 3;
+
+struct StageDesc {
+  int gh, gw, ngr, ngc;       // group shape and groups per panel (rows, cols)
+  int mode, min_count;        // pdp_cm_mode; MEDIAN: c = 0 below min_count
+  float sqrtG;
+  float *est;                 // [frames of the chunk][P * ngr * ngc]
+};
+
+struct StParams {
+  const uint16_t *raw;        // first frame of the chunk
+  int n_frames;               // frames of the chunk
+  const float *mapK, *rg, *mapNpf, *ped;
+  const double *rg64;
+  int P, H, W;
+  uint32_t npix;
+  float *v;                   // [n_frames][npix]
+  float T_cm, cand_thr;
+  double dT_seed, dE_ph;
+  int n_stages;
+  StageDesc st[kMaxStages];
+  // outputs (already offset to the chunk's first frame)
+  uint32_t cap;
+  uint32_t *hit_count, *hit_pixel;
+  float *hit_charge;
+  int32_t *hit_nphot;
+  float *hit_dx, *hit_dy;
+  uint32_t *frame_photons, *accum, *status;
+};
+
+__global__ void __launch_bounds__(kStThreads) pdp_st_calib_kernel(const StParams k) {
+  const size_t pairs = (size_t)k.n_frames * (k.npix / 2);
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < pairs; i += (size_t)gridDim.x * blockDim.x) {
+    const size_t f = i / (k.npix / 2), j = (i - f * (k.npix / 2)) * 2;
+    const uint32_t w = __ldg(reinterpret_cast<const uint32_t *>(k.raw + f * k.npix + j));
+    const float2 mk = __ldg(reinterpret_cast<const float2 *>(k.mapK + j));
+    const float2 rg = __ldg(reinterpret_cast<const float2 *>(k.rg + j));
+    const float2 nf = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + j));
+    float2 o;
+    o.x = fmaf(magic_lo(w) - mk.x, rg.x, nf.x);
+    o.y = fmaf(magic_hi(w) - mk.y, rg.y, nf.y);
+    *reinterpret_cast<float2 *>(k.v + f * k.npix + j) = o;
+  }
+}
+
+// block-wide sums in a fixed order (deterministic): warp shuffles, then warp 0 over the warp totals
+__device__ __forceinline__ double block_sum_d(double x, double *scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(FULL, x, o);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();
+  if (lane == 0) scratch[warp] = x;
+  __syncthreads();
+  double t = 0.0;
+  for (int i = 0; i < nw; ++i) t += scratch[i];
+  return t;
+}
+__device__ __forceinline__ unsigned block_sum_u(unsigned x, unsigned *scratch) {
+  x = __reduce_add_sync(FULL, x);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();
+  if (lane == 0) scratch[warp] = x;
+  __syncthreads();
+  unsigned t = 0;
+  for (int i = 0; i < nw; ++i) t += scratch[i];
+  return t;
+}
+
+// One CTA per (frame, group).  `s` = stage index.
+__global__ void __launch_bounds__(kStThreads) pdp_st_stage_kernel(const StParams k, int s) {
+  __shared__ double sd[kStThreads / 32];
+  __shared__ unsigned su[kStThreads / 32];
+  const StageDesc &st = k.st[s];
+  const int groups_per_frame = k.P * st.ngr * st.ngc;
+  const int G = st.gh * st.gw;
+  for (int item = blockIdx.x; item < k.n_frames * groups_per_frame; item += gridDim.x) {
+    const int f = item / groups_per_frame, gidx = item - f * groups_per_frame;
+    const int p = gidx / (st.ngr * st.ngc), rem = gidx - p * (st.ngr * st.ngc);
+    const int br = rem / st.ngc, bc = rem - br * st.ngc;
+    float *base = k.v + (size_t)f * k.npix + ((size_t)p * k.H + (size_t)br * st.gh) * k.W + (size_t)bc * st.gw;
+    auto at = [&](int i) -> float * { return base + (size_t)(i / st.gw) * k.W + (i % st.gw); };
+    float c = 0.f;
+    if (st.mode == 1) {
+      // guarded mean: sum of the pixels without signal / max(their number, sqrt(G))
+      double sum = 0.0;
+      unsigned cnt = 0;
+      for (int i = threadIdx.x; i < G; i += blockDim.x) {
+        const float x = *at(i);
+        if (fabsf(x) < k.T_cm) sum += (double)x, ++cnt;
+      }
+      const double tot = block_sum_d(sum, sd);
+      const unsigned n = block_sum_u(cnt, su);
+      c = (float)(tot / fmax((double)n, (double)st.sqrtG));
+    } else if (st.mode == 0) {
+      // exact median of the pixels without signal: the k-th order statistic is the smallest key K with
+      // #{key <= K} > k; bisection on order-preserving integer keys (tie-safe, at most 32 counting passes)
+      unsigned cnt = 0;
+      for (int i = threadIdx.x; i < G; i += blockDim.x) cnt += fabsf(*at(i)) < k.T_cm ? 1u : 0u;
+      const unsigned n = block_sum_u(cnt, su);
+      if (n > 0 && (int)n >= st.min_count) {
+        const unsigned kl = (n - 1) >> 1, kh = n >> 1;
+        auto count_le = [&](unsigned key) {
+          unsigned cc = 0;
+          for (int i = threadIdx.x; i < G; i += blockDim.x) {
+            const float x = *at(i);
+            cc += (fabsf(x) < k.T_cm && f2key(x) <= key) ? 1u : 0u;
+          }
+          return block_sum_u(cc, su);
+        };
+        auto select = [&](unsigned kk) {
+          unsigned lo = f2key(-k.T_cm), hi = f2key(k.T_cm);   // #{<= lo} = 0 <= kk < n = #{<= hi}
+          while (hi - lo > 1u) {
+            const unsigned mid = lo + ((hi - lo) >> 1);
+            if (count_le(mid) > kk) hi = mid;
+            else lo = mid;
+          }
+          return hi;
+        };
+        const unsigned key_l = select(kl);
+        unsigned key_h = key_l;
+        if (kh != kl && !(count_le(key_l) > kh)) key_h = select(kh);
+        c = 0.5f * (key2f(key_l) + key2f(key_h));
+      }
+    }
+    __syncthreads();
+    if (st.mode != 2)
+      for (int i = threadIdx.x; i < G; i += blockDim.x) *at(i) -= c;   // "subtracted from the input signal": ALL pixels
+    if (threadIdx.x == 0) st.est[(size_t)f * groups_per_frame + gidx] = c;
+    __syncthreads();
+  }
+}
+
+// fp64 value of pixel (p, r, c) of frame f after all stages, in the oracle's order: ((raw - ped) / gain - c1) - c2 - c3
+__device__ __forceinline__ double st_value(const StParams &k, int f, int p, int r, int c) {
+  const uint32_t gi = ((uint32_t)p * (uint32_t)k.H + (uint32_t)r) * (uint32_t)k.W + (uint32_t)c;
+  double x = ((double)__ldg(k.raw + (size_t)f * k.npix + gi) - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi);
+  for (int s = 0; s < k.n_stages; ++s) {
+    const StageDesc &st = k.st[s];
+    const int gidx = (p * st.ngr + r / st.gh) * st.ngc + c / st.gw;
+    x -= (double)__ldg(st.est + (size_t)f * (k.P * st.ngr * st.ngc) + gidx);
+  }
+  return x;
+}
+
+// One CTA per frame: scan the pixels in index order, kStThreads * 4 at a time.
+__global__ void __launch_bounds__(kStThreads) pdp_st_find_kernel(const StParams k) {
+  __shared__ unsigned s_warp[kStThreads / 32];
+  __shared__ unsigned s_base, s_phot;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int f = blockIdx.x; f < k.n_frames; f += gridDim.x) {
+    if (threadIdx.x == 0) s_base = 0u, s_phot = 0u;
+    __syncthreads();
+    const float *vf = k.v + (size_t)f * k.npix;
+    constexpr int PX = 4;
+    for (uint32_t b0 = 0; b0 < k.npix; b0 += kStThreads * PX) {
+      // thread t owns the PX consecutive pixels b0 + t*PX ..: pixel order = (thread, j) order
+      bool seed[PX];
+      HitRec rec[PX];
+      unsigned nseed = 0;
+      int my_ph = 0;
+#pragma unroll
+      for (int j = 0; j < PX; ++j) {
+        const uint32_t idx = b0 + threadIdx.x * PX + j;
+        seed[j] = false;
+        if (idx < k.npix && vf[idx] > k.cand_thr) {
+          const int c = (int)(idx % k.W), r = (int)((idx / k.W) % k.H), p = (int)(idx / ((uint32_t)k.W * k.H));
+          double v9[9];
+          bool ex[9];
+#pragma unroll
+          for (int dr = -1; dr <= 1; ++dr)
+#pragma unroll
+            for (int dc = -1; dc <= 1; ++dc) {
+              const int i = (dr + 1) * 3 + dc + 1;
+              const int rr = r + dr, cc = c + dc;
+              ex[i] = rr >= 0 && rr < k.H && cc >= 0 && cc < k.W;
+              v9[i] = ex[i] ? st_value(k, f, p, rr, cc) : 0.0;
+            }
+          Exact9 o;
+          const double x = v9[4];
+          o.seed = x > k.dT_seed;
+          o.E = 0.0, o.sx = 0.0, o.sy = 0.0;
+#pragma unroll
+          for (int i = 0; i < 9; ++i) {
+            const double y = v9[i];
+            o.E += y;
+            o.sx += (double)(i % 3 - 1) * y;
+            o.sy += (double)(i / 3 - 1) * y;
+            if (i == 4) continue;
+            if (ex[i] && !(x > y || (x == y && i > 4))) o.seed = false;   // strict maximum, ties to the lower index
+          }
+          if (o.seed) {
+            seed[j] = true;
+            rec[j] = make_rec(o, k.dE_ph);
+            ++nseed;
+            my_ph += rec[j].n;
+          }
+        }
+      }
+      // ordered slots: exclusive scan of the per-thread seed counts over the block
+      unsigned incl = nseed;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += t;
+      }
+      const int wph = __reduce_add_sync(FULL, my_ph);
+      __syncthreads();
+      if (lane == 31) s_warp[warp] = incl;
+      __syncthreads();
+      unsigned woff = 0, total = 0;
+      for (int i = 0; i < nw; ++i) {
+        if (i < warp) woff += s_warp[i];
+        total += s_warp[i];
+      }
+      unsigned pos = s_base + woff + incl - nseed;
+#pragma unroll
+      for (int j = 0; j < PX; ++j) {
+        if (!seed[j]) continue;
+        const uint32_t idx = b0 + threadIdx.x * PX + j;
+        if (pos < k.cap) {
+          const size_t o = (size_t)f * k.cap + pos;
+          k.hit_pixel[o] = idx;
+          k.hit_charge[o] = rec[j].E;
+          k.hit_nphot[o] = rec[j].n;
+          k.hit_dx[o] = rec[j].dx;
+          k.hit_dy[o] = rec[j].dy;
+        } else {
+          overflow_accum(k.accum + idx, (uint32_t)rec[j].n, k.status);
+        }
+        ++pos;
+      }
+      if (lane == 0 && wph) atomicAdd(&s_phot, (unsigned)wph);   // shared memory
+      __syncthreads();
+      if (threadIdx.x == 0) s_base += total;
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+      k.hit_count[f] = s_base;
+      k.frame_photons[f] = s_phot;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace pdp

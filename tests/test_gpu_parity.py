@@ -520,3 +520,48 @@ def test_dense_photon_counting(oracle, case, cm_mode):
         clean = ~frag.reshape(n, -1).any(axis=1)                           # frames without any fragile pixel: exact totals
         assert np.array_equal(tot.cpu().numpy().astype(np.int64)[clean], o_tot.astype(np.int64)[clean])
         assert np.abs(tot.cpu().numpy().astype(np.int64) - o_tot.astype(np.int64)).max() <= max(3, int(frag.reshape(n, -1).any(axis=1).sum() and frag.sum()))
+
+
+STAGE_SETS = {
+    "row_col_mean": [(1, 64, 1), (8, 1, 1)],
+    "paper_3_stacked_mean": [(1, 128, 1), (8, 1, 1), (40, 128, 1)],          # row, column, panel-wise: PAPER.md:L117
+    "row_median_block_mean": [(1, 64, 0), (8, 16, 1)],
+    "panel_median": [(40, 128, 0)],
+    "col_median_then_none": [(10, 1, 0), (1, 128, 2)],
+}
+
+
+@pytest.mark.parametrize("name", list(STAGE_SETS), ids=list(STAGE_SETS))
+def test_stacked_common_mode_stages(oracle, name):
+    """NEXT-1: up to three stacked common-mode stages on row, column, block and panel-wise
+    groups, mean and median estimators, against the oracle's staged chain: hits bit-exact outside the pixels the
+    oracle flags, floats within tolerance."""
+    stages = STAGE_SETS[name]
+    cfg, n = small(0, panels=2, rows=40, cols=128, seg_cols=64, occupancy=0.01), 9
+    raw, ped, gain = make(cfg, n)
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, max_frames_per_batch=n,
+                          pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu)
+    ctx.set_cm_stages(stages)
+    out = binding.alloc_output(n, cfg.npix, cfg.max_hits, DEV)
+    ctx.process(raw, out)
+    torch.cuda.synchronize()
+    assert ctx.last_launch_count == 1 + len(stages) + 1 + 1            # calibrate, stages, finder, accumulated image
+    g = {k: getattr(out, k).cpu().numpy() for k in
+         ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum", "status")}
+    g["hit_count"] = g["hit_count"].astype(np.int64) & 0xFFFFFFFF
+    g["frame_photons"] = g["frame_photons"].astype(np.int64) & 0xFFFFFFFF
+    o = oracle_run(oracle, cfg, raw, ped, gain, 0, stages=stages)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, cm_adu=cfg.cm_adu)
+    print(name, rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 300 and rep.exempt_hits <= 3
+    # back to the hot path: [] restores the fused single row-segment stage
+    ctx.set_cm_stages([])
+    out2 = binding.alloc_output(n, cfg.npix, cfg.max_hits, DEV)
+    ctx.process(raw, out2)
+    torch.cuda.synchronize()
+    o1 = oracle_run(oracle, cfg, raw, ped, gain, 0)
+    assert np.array_equal(out2.hit_count.cpu().numpy().astype(np.int64), o1.hit_count)
+    with pytest.raises(binding.PdpError):
+        ctx.set_cm_stages([(7, 128, 1)])                                # does not tile 40 rows
+    ctx.close()
