@@ -327,6 +327,54 @@ def e2e_streamed(binding, cfg, keep, dev, steps, dist, world):
             "api": "pdp_process_host (pinned host frames, double-buffered side-stream copies)"}
 
 
+def _timed(fn, reps=3):
+    fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def time_next_rows(binding, dev):
+    """configs[1] (2000 frames of 704x768): the summarization histograms over the finished lists, dense photon
+    counting, and the paper's three stacked mean stages (row, column, panel-wise) on the general path."""
+    cfg = synth.CONFIGS[1]
+    n = cfg.n_frames
+    peak, _ = measured_peak()
+    ped, gain = synth.make_maps(cfg, dev)
+    raw = synth.make_frames(cfg, 0, n, ped, gain, block_pixels=1 << 27)
+    res = {"workload": workload_name(cfg)}
+    ctx = make_context(binding, cfg, n, ped, gain, CM_MODES["median"])
+    out = binding.alloc_output(n, cfg.npix, 2048, dev)
+    ctx.process(raw, out)
+    he = torch.zeros(256, dtype=torch.int32, device=dev)
+    hx = torch.zeros(64, dtype=torch.int32, device=dev)
+    hy = torch.zeros(64, dtype=torch.int32, device=dev)
+    ms = _timed(lambda: ctx.histograms(out, n, energy=(0.0, 2.0, 256), dxy=(-1.0, 1.0 / 32, 64), hist_energy=he, hist_dx=hx, hist_dy=hy))
+    hits = float((out.hit_count.to(torch.int64) & 0xFFFFFFFF).sum().item())
+    res["histograms"] = {"ms": ms, "hits": hits, "gbs": (12 * hits + 4 * n) / ms / 1e6, "bytes": "12 B per hit read (E, dx, dy) + 4 B per frame"}
+    img = torch.zeros(cfg.npix, dtype=torch.int32, device=dev)
+    tot = torch.zeros(n, dtype=torch.int32, device=dev)
+    ms = _timed(lambda: ctx.process_dense(raw, img, tot))
+    res["dense_photon_counting_median"] = {"ms": ms, "frames_per_s": n / ms * 1e3, "raw_gbs": n * cfg.npix * 2 / ms / 1e6,
+                                           "frac_of_measured": n * cfg.npix * 2 / ms / 1e6 / peak, "kernel": ctx.last_kernel_name}
+    m = 256                                                    # the general path keeps a float32 working image: a sample
+    ctx.set_cm_stages([(1, cfg.seg_cols, 1), (cfg.rows, 1, 1), (cfg.rows, cfg.cols, 1)])
+    out2 = binding.alloc_output(m, cfg.npix, 2048, dev)
+    ms = _timed(lambda: ctx.process(raw[:m], out2, n_frames=m))
+    # bytes the general path must move per pixel and frame: raw 2 + image write 4 + per stage read 4 + write 4 + finder read 4
+    bpp = 2 + 4 + 3 * 8 + 4
+    res["stacked_3_mean_stages"] = {"ms": ms, "frames": m, "frames_per_s": m / ms * 1e3, "launches": ctx.last_launch_count,
+                                    "alg_gbs": m * cfg.npix * bpp / ms / 1e6, "frac_of_measured": m * cfg.npix * bpp / ms / 1e6 / peak,
+                                    "bytes": "%d B per pixel and frame (raw, working image written once, read+written per stage, read by the finder)" % bpp}
+    ctx.close()
+    return res
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -341,6 +389,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the timings of the rows beyond the hot path")
     ap.add_argument("--per-config", default="0,1,2,3,4", help="configs for the per_config table ('' = none)")
     ap.add_argument("--per-config-modes", default="median", help="comma list of cm modes for the per_config table")
     args = ap.parse_args()
@@ -450,6 +499,12 @@ def main():
                     r.pop(drop, None)
                 table[key] = r
         line["config"]["per_config"] = table
+    # ---- the rows beyond the hot path: histograms, dense photon counting, stacked CM stages ----
+    if rank == 0 and world == 1 and not args.no_extras:
+        try:
+            line["config"]["next_rows"] = time_next_rows(binding, dev)
+        except Exception as exc:
+            line["config"]["next_rows"] = {"error": str(exc)[:200]}
     if rank == 0:
         print(json.dumps(line))
     if dist:

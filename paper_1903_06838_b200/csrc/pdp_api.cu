@@ -87,6 +87,8 @@ struct pdp_ctx {
   double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
+  uint32_t *d_seed_scratch = nullptr;       // throughput kernel: seed buffers [SMs][8 warps][6][seed_cap], on first use
+  int seed_cap = 0;
   int n_stages = 0;                         // pdp_set_cm_stages: 0 = the hot path's single row-segment stage
   pdp_cm_stage stages[3] = {};
   float *d_st_v = nullptr;                  // staged path: working image [st_chunk][npix] and the stage estimates
@@ -238,11 +240,11 @@ bool make_plan_chain(const pdp_geometry &g, const ChainVariant &v, int dense_war
     uint32_t off = 0;
     pl.off_cm = off;      off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 4u);
     pl.off_flag = off;    off = al(off + pdp::kFCH * ring * (uint32_t)nseg * 8u);
-    pl.off_done = off;    off = al(off + 16u);
-    pl.off_pref = off;    off = al(off + pdp::kFCH * 4u);
-    pl.off_phot = off;    off = al(off + pdp::kFCH * 4u);
-    // per sparse warp: item list + masks, candidate list, seed buffer (6 words per seed), per-frame working totals
-    pl.sparse_stride = al((uint32_t)(2 * pdp::kItemCap + pdp::kListCap + 6 * pdp::kSeedCap + 2 * pdp::kFCH) * 4u);
+    pl.off_done = off;    off = al(off + 2u * (uint32_t)NB * 4u);
+    pl.off_pref = off;    off = al(off + (uint32_t)NB * pdp::kFCH * 4u);
+    pl.off_phot = off;    off = al(off + (uint32_t)NB * pdp::kFCH * 4u);
+    // per sparse warp: item list + masks, candidate list, per-frame working totals
+    pl.sparse_stride = al((uint32_t)(2 * pdp::kItemCap + pdp::kListCap + 3 * pdp::kFCH) * 4u);
     pl.off_sparse = off;  off = al(off + (uint32_t)nws * pl.sparse_stride);
     pl.ring_warp_bytes = (uint32_t)pdp::kRingD * 32u * (uint32_t)N * 2u;
     pl.off_ring = off;    off = al(off + (uint32_t)NWD * pl.ring_warp_bytes);
@@ -295,6 +297,7 @@ void free_ctx(pdp_ctx *c) {
   cudaFree(c->d_ticket);
   cudaFree(c->d_cm);
   cudaFree(c->d_hist_ws);
+  cudaFree(c->d_seed_scratch);
   cudaFree(c->d_st_v);
   cudaFree(c->d_st_est);
   cudaFree(c->d_dense_ws);
@@ -580,6 +583,15 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   k.accum = o.accum;
   k.status = o.status;
   k.cm_keep = keep_cm ? c->d_cm : nullptr;
+  if (!c->d_seed_scratch) {
+    // a band of all 16 frame slots can hold at most 16 * R * W / 2 seeds per panel row block; 8192 buffered seeds
+    // let several bands be evaluated at the same time even on dense data (a full buffer only chains earlier)
+    const long long most = (long long)pdp::kFCH * (pl.R + 1) * ((c->geo.cols + 1) / 2);
+    c->seed_cap = (int)std::min<long long>(8192, std::max<long long>(256, (most + 31) / 32 * 32));
+    PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 8 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
+  }
+  k.seed_scratch = c->d_seed_scratch;
+  k.seed_cap = c->seed_cap;
   k.off_cm = pl.off_cm;
   k.off_flag = pl.off_flag;
   k.off_pref = pl.off_pref;

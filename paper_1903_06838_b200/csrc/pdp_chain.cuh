@@ -72,6 +72,8 @@ struct CParams {
   float *hit_dx, *hit_dy;
   uint32_t *frame_photons, *accum, *status;
   float *cm_keep;                            // optional [n][P][H][nseg]
+  uint32_t *seed_scratch;                    // [grid][NWS][6][seed_cap] words: seeds between evaluation and ordered emission
+  int seed_cap;                              //   (device memory, L2 resident; a multiple of 32)
   // shared-memory carve-up (byte offsets)
   uint32_t off_cm, off_flag, off_done, off_pref, off_phot, off_sparse, sparse_stride, off_ring, off_maps;
   uint32_t ring_warp_bytes, maps_warp_bytes;
@@ -456,7 +458,6 @@ __device__ __forceinline__ void named_sync(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 
-constexpr int kSeedCap = 256;     // seeds buffered per sparse warp between evaluation and ordered emission
 
 // ---- sparse stage of ONE band for ALL frame slots of the chunk: one warp ------------------------------------------
 // Sparse warp s owns the bands gb = s, s + NWS, ...: several bands are evaluated at the same time by different
@@ -477,21 +478,18 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
   const int R = k.R, kNBr = k.NB, ring_rows = kNBr * R;
   const float *cmring = reinterpret_cast<const float *>(smem + k.off_cm);
   const unsigned long long *flags = reinterpret_cast<const unsigned long long *>(smem + k.off_flag);
-  volatile int *band_done = reinterpret_cast<volatile int *>(smem + k.off_done);
-  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);      // [kFCH] hits of the frame so far
-  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);      // [kFCH] photons of the frame so far
+  // per band slot: inclusive per-frame prefixes (hits, photons) over the bands up to this one, and two flags
+  volatile int *bready = reinterpret_cast<volatile int *>(smem + k.off_done);          // [NB] gb + 1: prefix published
+  volatile int *bdone = bready + kNBr;                                                   // [NB] gb + 1: band consumed
+  uint32_t *bpre_hits = reinterpret_cast<uint32_t *>(smem + k.off_pref);                // [NB][kFCH]
+  uint32_t *bpre_phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);                // [NB][kFCH]
   unsigned char *mine = smem + k.off_sparse + (size_t)sw * k.sparse_stride;
   uint32_t *items = reinterpret_cast<uint32_t *>(mine);                  // [kItemCap] flagged units
   uint32_t *imask = items + kItemCap;                                    // [kItemCap] candidate pixels of the unit
   uint32_t *cand = imask + kItemCap;                                     // [kListCap] candidates (q, row, col)
-  uint32_t *s_pix = cand + kListCap;                                     // [kSeedCap] seed buffer
-  float *s_E = reinterpret_cast<float *>(s_pix + kSeedCap);
-  int32_t *s_n = reinterpret_cast<int32_t *>(s_E + kSeedCap);
-  float *s_dx = reinterpret_cast<float *>(s_n + kSeedCap);
-  float *s_dy = s_dx + kSeedCap;
-  uint32_t *s_q = reinterpret_cast<uint32_t *>(s_dy + kSeedCap);
-  uint32_t *base_s = s_q + kSeedCap;                                     // [kFCH] working copy of pref
-  uint32_t *pht_s = base_s + kFCH;                                       // [kFCH] photons added by this band
+  uint32_t *base_s = cand + kListCap;                                    // [kFCH] next free slot of every frame's list
+  uint32_t *pht_s = base_s + kFCH;                                       // [kFCH] photons found by this band
+  uint32_t *cnt_s = pht_s + kFCH;                                        // [kFCH] seeds found by this band
 
   const int p = band / k.bands_per_panel, bi = band - p * k.bands_per_panel, r0 = bi * R;
   const int ra = bi == 0 ? 0 : r0 - 1;
@@ -501,21 +499,56 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
   const int s_prev = ((gb + kNBr - 1) % kNBr) * R, s_cur = (gb % kNBr) * R;
   auto slot_of = [&](int r) { return r < r0 ? s_prev + (r - r0 + R) : s_cur + (r - r0); };
   const size_t npix = (size_t)k.P * k.H * k.W;
-  bool waited = false;      // the band before has been emitted and base_s / pht_s are loaded
+  // seed buffer of this warp (device memory): evaluated seeds wait here, in output order, until the band before is
+  // emitted; several bands are evaluated at the same time by different warps, only this copy-out is chained
+  const int kSeedCap = k.seed_cap;
+  uint32_t *s_pix = k.seed_scratch + ((size_t)blockIdx.x * k.NWS + sw) * 6 * (size_t)kSeedCap;
+  float *s_E = reinterpret_cast<float *>(s_pix + kSeedCap);
+  int32_t *s_n = reinterpret_cast<int32_t *>(s_E + kSeedCap);
+  float *s_dx = reinterpret_cast<float *>(s_n + kSeedCap);
+  float *s_dy = s_dx + kSeedCap;
+  uint32_t *s_q = reinterpret_cast<uint32_t *>(s_dy + kSeedCap);
+  bool have_base = false;   // the prefixes of the band before are known: base_s is loaded
+  bool published = false;   // this band's inclusive prefixes are published
   int ns = 0;               // seeds in the buffer (warp-uniform)
-  if (lane < kFCH) pht_s[lane] = 0u;
+  uint32_t pre_phot = 0u;   // lane q: photons of frame q in the bands before
+  if (lane < kFCH) pht_s[lane] = 0u, cnt_s[lane] = 0u;
+  __syncwarp();
 
-  auto flush = [&]() {      // ordered emission of the buffered seeds
-    if (!waited) {
+  // The per-frame list offsets are a prefix over the bands: a band needs the inclusive prefixes of the band before
+  // (published as soon as THAT band has counted its seeds, before it copies them out), adds its own counts and
+  // publishes; only these few words are chained from band to band, the copy-out of different bands overlaps.
+  auto get_base = [&]() {
+    if (band > 0) {
       if (lane == 0)
-        while (*band_done < gb) {
+        while (bready[(gb + kNBr - 1) % kNBr] < gb) {
         }
       __syncwarp();
       __threadfence_block();
-      if (lane < kFCH) base_s[lane] = pref[lane];
-      __syncwarp();
-      waited = true;
     }
+    if (lane < kFCH) {
+      base_s[lane] = band > 0 ? bpre_hits[((gb + kNBr - 1) % kNBr) * kFCH + lane] : 0u;
+      pre_phot = band > 0 ? bpre_phot[((gb + kNBr - 1) % kNBr) * kFCH + lane] : 0u;
+    }
+    __syncwarp();
+    have_base = true;
+  };
+  auto publish = [&](bool final_counts) {   // inclusive prefixes of this band; base_s may already have advanced
+    if (lane < kFCH) {
+      bpre_hits[(gb % kNBr) * kFCH + lane] = final_counts ? base_s[lane] + cnt_s[lane] : base_s[lane];
+      bpre_phot[(gb % kNBr) * kFCH + lane] = pre_phot + pht_s[lane];
+    }
+    __syncwarp();
+    if (lane == 0) {
+      __threadfence_block();
+      bready[gb % kNBr] = gb + 1;
+    }
+    __syncwarp();
+    published = true;
+  };
+
+  auto flush = [&]() {      // ordered copy-out of the buffered seeds
+    if (!have_base) get_base();
     for (int i0 = 0; i0 < ns; i0 += 32) {
       const int i = i0 + lane;
       const bool have = i < ns;
@@ -535,7 +568,6 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
         } else {
           overflow_accum(k.accum + pix, (uint32_t)n, k.status);
         }
-        if (n) atomicAdd(&pht_s[q], (uint32_t)n);   // shared memory; integer sum: order-independent
       }
       __syncwarp();
       if (have && (same >> lane) <= 1u) base_s[q] += __popc(same);   // the last lane of each frame's run
@@ -568,8 +600,10 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
       }
       const unsigned sm = __ballot_sync(FULL, seed);
       if (!sm) continue;
-      if (ns + __popc(sm) > kSeedCap) flush();
+      if (ns + __popc(sm) > kSeedCap) flush();     // (a full buffer chains this band's copy-out earlier)
       if (seed) {
+        atomicAdd(&cnt_s[q], 1u);                   // shared memory; integer sums: order-independent
+        if (h.n) atomicAdd(&pht_s[q], (uint32_t)h.n);
         const int o = ns + __popc(sm & ((1u << lane) - 1u));
         s_pix[o] = (uint32_t)(((size_t)p * k.H + row) * k.W + col);
         s_E[o] = h.E;
@@ -698,23 +732,24 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
     }
   }
   if (n_items) process_items();
-  flush();   // also waits for the band before when nothing was buffered: the running totals are passed on in order
-  if (lane < nf) {
-    const uint32_t cnt = base_s[lane], pht = phot[lane] + pht_s[lane];
-    if (band == k.n_bands - 1) {   // the frame is complete
-      k.hit_count[f0 + lane] = cnt;
-      k.frame_photons[f0 + lane] = pht;
-      pref[lane] = 0u;
-      phot[lane] = 0u;
-    } else {
-      pref[lane] = cnt;
-      phot[lane] = pht;
-    }
+  __syncwarp();
+  // all seeds of the band are counted.  Nothing copied out yet: publish base + counts first, then copy out (the next
+  // band does not wait for the copy); after an early flush base_s has advanced past the copied seeds: cnt_s holds ALL
+  // seeds of the band, so subtract what was copied by publishing after the final flush instead.
+  if (!have_base) {
+    get_base();
+    publish(true);
+  }
+  flush();
+  if (!published) publish(false);
+  if (band == k.n_bands - 1 && lane < nf) {   // the frames are complete: base_s is the total, the photons likewise
+    k.hit_count[f0 + lane] = base_s[lane];
+    k.frame_photons[f0 + lane] = pre_phot + pht_s[lane];
   }
   __syncwarp();
   if (lane == 0) {
     __threadfence_block();
-    *band_done = gb + 1;
+    bdone[gb % kNBr] = gb + 1;
   }
   __syncwarp();
 }
@@ -737,9 +772,8 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
   const int R = k.R, kNBr = k.NB, ring_rows = kNBr * R;
   float *cmring = reinterpret_cast<float *>(smem + k.off_cm);                               // [kFCH][NB*R][nseg]
   unsigned long long *flags = reinterpret_cast<unsigned long long *>(smem + k.off_flag);    // [kFCH][NB*R][nseg]
-  volatile int *band_done = reinterpret_cast<volatile int *>(smem + k.off_done);
-  uint32_t *pref = reinterpret_cast<uint32_t *>(smem + k.off_pref);    // [kFCH]
-  uint32_t *phot = reinterpret_cast<uint32_t *>(smem + k.off_phot);    // [kFCH]
+  volatile int *bready = reinterpret_cast<volatile int *>(smem + k.off_done);   // [NB], then bdone [NB]
+  volatile int *bdone = bready + kNBr;
 
   const int fs = (int)(((long long)blockIdx.x * k.n_frames) / gridDim.x);
   const int fe = (int)(((long long)(blockIdx.x + 1) * k.n_frames) / gridDim.x);
@@ -748,8 +782,7 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
   const int n_chunks = (FCn + kFCH - 1) / kFCH;
   const int sync_threads = (NWD + 1) * 32;      // the dense warps and the ONE sparse warp that owns the band
 
-  for (int i = tid; i < kFCH; i += nthreads) pref[i] = 0u, phot[i] = 0u;
-  if (tid == 0) *band_done = 0;
+  for (int i = tid; i < 2 * kNBr; i += nthreads) bready[i] = 0;
   __syncthreads();
 
   if (warp >= NWD) {
@@ -859,8 +892,9 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
         }
         __syncwarp();
       }
-      // the ring slot about to be written held band gb-NB, last read by the sparse stage of band gb-NB+1
-      while (*band_done < gb - (kNBr - 2)) __nanosleep(100);
+      // the ring slot about to be written held band gb-NB, last read by the sparse stages of bands gb-NB, gb-NB+1
+      if (gb >= kNBr)
+        while (bdone[gb % kNBr] < gb - kNBr + 1 || bdone[(gb + 1) % kNBr] < gb - kNBr + 2) __nanosleep(100);
 
       float *cm_p = cmring + ((size_t)g * ring_rows + slot) * k.nseg + sg;
       unsigned long long *fl_p = flags + ((size_t)g * ring_rows + slot) * k.nseg + sg;
