@@ -103,7 +103,7 @@ struct pdp_ctx {
   int keep_cm = 0;
   int64_t cm_frames = 0;                    // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
-  ChainPlan cplan[2];                       // [0] 4 sparse warps (sparse data), [1] 8 sparse warps (dense data)
+  ChainPlan cplan[3];                       // 4, 8, 12 sparse warps (16, 12, 8 dense ones): sparse ... dense data
   int sparse_override = 0;                  // pdp_debug_set("sparse_warps"): 0 default (4), 4, 8
   ChainVariant forced{0, 0, 0};             // pdp_debug_set("variant")
   int kernel_override = 0;                  // pdp_debug_set("kernel"): 0 auto, 1 look-back kernel, 2 throughput kernel
@@ -248,7 +248,7 @@ bool make_plan_chain(const pdp_geometry &g, const ChainVariant &v, int dense_war
     pl.off_sparse = off;  off = al(off + (uint32_t)nws * pl.sparse_stride);
     pl.ring_warp_bytes = (uint32_t)pdp::kRingD * 32u * (uint32_t)N * 2u;
     pl.off_ring = off;    off = al(off + (uint32_t)NWD * pl.ring_warp_bytes);
-    pl.maps_warp_bytes = 3u * (uint32_t)v.LPS * (uint32_t)N * 4u;
+    pl.maps_warp_bytes = 2u * (uint32_t)v.LPS * (uint32_t)N * 4u;   // pedestal and 1/gain
     pl.off_maps = off;    off = al(off + (uint32_t)NWD * pl.maps_warp_bytes);
     if (off > smem_limit) continue;
     pl.v = v;
@@ -313,13 +313,13 @@ void free_ctx(pdp_ctx *c) {
 // (Re)build the throughput-kernel plans for the current variant choice.
 int build_chain_plans(pdp_ctx *c) {
   ChainVariant v{0, 0, 0};
-  c->cplan[0] = ChainPlan{};
-  c->cplan[1] = ChainPlan{};
+  for (ChainPlan &pl : c->cplan) pl = ChainPlan{};
   if (c->forced.V) v = c->forced;
   else if (!pick_variant(c->geo, v)) return PDP_OK;   // no variant: the small-batch kernel serves every batch
   make_plan_chain(c->geo, v, 16, 4, c->smem_limit, c->cplan[0]);
   make_plan_chain(c->geo, v, 12, 8, c->smem_limit, c->cplan[1]);
-  for (int i = 0; i < 2; ++i) {
+  make_plan_chain(c->geo, v, 8, 12, c->smem_limit, c->cplan[2]);
+  for (int i = 0; i < 3; ++i) {
     if (!c->cplan[i].ok) continue;
     for (int mode = 0; mode < 3; ++mode) {
       pdp::ChainFn fn = chain_kernel(v, mode);
@@ -328,7 +328,7 @@ int build_chain_plans(pdp_ctx *c) {
         break;
       }
       PDP_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)std::max(c->cplan[0].smem, c->cplan[1].smem)));
+                                       (int)std::max(std::max(c->cplan[0].smem, c->cplan[1].smem), c->cplan[2].smem)));
     }
   }
   if (c->forced.V && !c->cplan[0].ok) return fail(c, PDP_E_GEOMETRY, "pdp_debug_set: variant does not fit this geometry");
@@ -493,7 +493,8 @@ int pdp_debug_set(pdp_ctx *ctx, const char *key, int64_t value) {
     return PDP_OK;
   }
   if (!std::strcmp(key, "sparse_warps")) {
-    if (value != 0 && value != 4 && value != 8) return fail(ctx, PDP_E_VALUE, "pdp_debug_set: sparse_warps must be 0, 4 or 8");
+    if (value != 0 && value != 4 && value != 8 && value != 12)
+      return fail(ctx, PDP_E_VALUE, "pdp_debug_set: sparse_warps must be 0, 4, 8 or 12");
     ctx->sparse_override = (int)value;
     return PDP_OK;
   }
@@ -570,6 +571,7 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   }
   k.dT_seed = (double)c->prm.seed_adu;
   k.dE_ph = (double)c->prm.photon_adu;
+  k.dinv_E_ph = 1.0 / (double)c->prm.photon_adu;
   k.cm_mode = c->prm.cm_mode;
   k.cm_min_count = c->prm.cm_min_count > 0 ? c->prm.cm_min_count : (int)std::ceil(std::sqrt((double)k.S));
   k.cap = o.hit_capacity;
@@ -588,7 +590,7 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
     // let several bands be evaluated at the same time even on dense data (a full buffer only chains earlier)
     const long long most = (long long)pdp::kFCH * (pl.R + 1) * ((c->geo.cols + 1) / 2);
     c->seed_cap = (int)std::min<long long>(8192, std::max<long long>(256, (most + 31) / 32 * 32));
-    PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 8 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
+    PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 12 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
   }
   k.seed_scratch = c->d_seed_scratch;
   k.seed_cap = c->seed_cap;
@@ -722,8 +724,8 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   if (c->n_stages > 0) return enqueue_staged(c, raw, n, st, o);
   // ---- large batches: the throughput kernel (frame-owner CTAs) ----
   {
-    int which = c->sparse_override == 8 ? 1 : 0;
-    if (!c->cplan[which].ok) which ^= 1;
+    int which = c->sparse_override == 12 ? 2 : (c->sparse_override == 8 ? 1 : 0);
+    if (!c->cplan[which].ok) which = 0;
     const bool can = c->cplan[which].ok;
     const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
     if (c->kernel_override == 2 && !can)

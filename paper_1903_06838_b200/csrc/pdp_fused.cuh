@@ -356,7 +356,7 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_fused_kernel(const KParams k)
           const Exact9 e9 = exact9(k, tile, ctab, p, r0, tr_first, rr, col);
           if (!e9.seed) continue;
           seedword |= 1u << b;
-          const int n = photon_count(e9.E, k.dE_ph);
+          const int n = photon_count(e9.E, k.dE_ph, 1.0 / k.dE_ph);
           my_phot += n;
           acc[rr * k.W + col] += (uint32_t)n;   // this thread owns the pixel for this frame
         }
@@ -444,7 +444,7 @@ __global__ void __launch_bounds__(kThreads, 1) pdp_fused_kernel(const KParams k)
             const double inv = e9.E > 0.0 ? 1.0 / e9.E : 0.0;
             k.hit_pixel[fbase + pos] = (uint32_t)(((size_t)p * k.H + r0 + rr) * k.W + col);
             k.hit_charge[fbase + pos] = (float)e9.E;
-            k.hit_nphot[fbase + pos] = photon_count(e9.E, k.dE_ph);
+            k.hit_nphot[fbase + pos] = photon_count(e9.E, k.dE_ph, 1.0 / k.dE_ph);
             k.hit_dx[fbase + pos] = e9.E > 0.0 ? (float)(e9.sx / e9.E) : 0.f;
             k.hit_dy[fbase + pos] = e9.E > 0.0 ? (float)(e9.sy / e9.E) : 0.f;
             (void)inv;

@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(kStThreads) pdp_st_find_kernel(const StParams 
           }
           if (o.seed) {
             seed[j] = true;
-            rec[j] = make_rec(o, k.dE_ph);
+            rec[j] = make_rec(o, k.dE_ph, 1.0 / k.dE_ph);
             ++nseed;
             my_ph += rec[j].n;
           }
