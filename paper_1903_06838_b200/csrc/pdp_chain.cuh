@@ -36,11 +36,10 @@ namespace pdp {
 constexpr int kFCH = 16;          // frame slots per chunk
 constexpr int kRingD = 2;         // raw-pixel ring depth in steps (kRingD - 1 steps of prefetch in flight; a step of a warp
                                   // lasts microseconds because the sub-partition's other warps run in between)
-constexpr int kMaxIt = 7;         // counting passes before the search switches to walking / bisection
+constexpr int kMaxIt = 7;         // counting passes of the median search before it falls back to walking up from the bracket
 constexpr int kListCap = 3 * 32 * 16;   // candidate list: at least one more group of 32 items (<= 16 pixels each) always fits
 constexpr int kItemCap = 256;     // flagged units expanded per batch by a sparse warp
 constexpr int kChainMaxThreads = 640;
-constexpr int kMaxSparseWarps = 8;
 
 // Candidate flags are kept per UNIT of a lane's run: NU units of U pixels (the last one may be shorter), chosen so
 // that the LPS * NU flag bits of a row segment fit one 64-bit word and a unit is about 8 pixels.
@@ -583,11 +582,7 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
       const int q = (int)(ce >> 28), row = ra + (int)((ce >> 20) & 0xffu), col = (int)(ce & 0xfffffu);
       bool seed = false;
       HitRec h{0.f, 0.f, 0.f, 0};
-#ifdef PDP_DBG_SKIP_EXACT
-      if (false) {
-#else
       if (have) {
-#endif
         const float *cmf = cmring + (size_t)q * ring_rows * k.nseg;
         const float *cm_0 = cmf + (size_t)slot_of(row) * k.nseg;
         const float *cm_m1 = row > 0 ? cmf + (size_t)slot_of(row - 1) * k.nseg : cm_0;
@@ -702,9 +697,6 @@ __device__ __forceinline__ void chain_sparse(const CParams &k, unsigned char *sm
       trr = u - tq * nrows;
       fw = flags[((size_t)tq * ring_rows + slot_of(ra + trr)) * k.nseg + tsg];
     }
-#ifdef PDP_DBG_SKIP_PX
-    fw = 0ull;
-#endif
     if (!__any_sync(FULL, fw != 0ull)) continue;
     int mine_n = __popcll(fw), incl = mine_n;
 #pragma unroll
@@ -760,6 +752,7 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
   constexpr int FPS = 32 / LPS;              // frames per warp step
   constexpr int CS = V >= 4 ? 4 : 2;         // floats per map chunk (LDS.128 / LDS.64)
   constexpr int CH = V / CS;                 // chunks per vector
+  constexpr bool kRegMaps = MODE != 0 && N <= 24;   // maps in registers (measured: slower for the N = 26 variant)
   constexpr uint32_t VB = V * 2;             // bytes per raw vector
   constexpr uint32_t kStepBytes = 32u * N * 2u;   // one step of one warp in the raw ring
   constexpr int NU = flag_units(N, LPS), U = flag_unit_px(N, LPS);
@@ -852,7 +845,33 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
       const int row = r0 + tr;
       const bool active = row < k.H;
       const int slot = (gb % kNBr) * R + tr;
-      if (active) {   // maps of this warp's row segment: global (L2) -> lane-major tile, once per band and chunk
+      // Maps of this warp's row segment, once per band and chunk.  The guarded-mean and no-common-mode variants hold
+      // them in registers for all steps of the band (2 N registers; shared-memory wavefronts were their bound); the
+      // median variant needs the registers for the N values of the selection and stages a lane-major tile.
+      [[maybe_unused]] float mkr[kRegMaps ? N : 1], rrr[kRegMaps ? N : 1];
+      if constexpr (kRegMaps) {
+        const size_t rowoff = ((size_t)p * k.H + min(row, k.H - 1)) * k.W + (size_t)sg * k.S + (size_t)l * N;
+#pragma unroll
+        for (int j = 0; j < N; j += CS) {
+          if (l * N + j < k.S) {   // padding: a = (raw - 3e38) * 1 = -3e38: outside the mask, never a candidate
+            if constexpr (CS == 4) {
+              const float4 a = __ldg(reinterpret_cast<const float4 *>(k.ped + rowoff + j));
+              const float4 b = __ldg(reinterpret_cast<const float4 *>(k.rg + rowoff + j));
+              mkr[j] = a.x, mkr[j + 1] = a.y, mkr[j + 2] = a.z, mkr[j + 3] = a.w;
+              rrr[j] = b.x, rrr[j + 1] = b.y, rrr[j + 2] = b.z, rrr[j + 3] = b.w;
+            } else {
+              const float2 a = __ldg(reinterpret_cast<const float2 *>(k.ped + rowoff + j));
+              const float2 b = __ldg(reinterpret_cast<const float2 *>(k.rg + rowoff + j));
+              mkr[j] = a.x, mkr[j + 1] = a.y;
+              rrr[j] = b.x, rrr[j + 1] = b.y;
+            }
+          } else {
+#pragma unroll
+            for (int e = 0; e < CS; ++e) mkr[j + e] = 3.0e38f, rrr[j + e] = 1.f;
+          }
+        }
+      }
+      if (!kRegMaps && active) {
         const size_t rowoff = ((size_t)p * k.H + row) * k.W + (size_t)sg * k.S;
         __syncwarp();
         for (int ci = lane; ci < (int)(kMapFloats / CS); ci += 32) {
@@ -944,14 +963,18 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
               VecLoadS<V>::ld(ring_lane + rslot + v * (32 * VB), w);
 #pragma unroll
               for (int h = 0; h < CH; ++h) {
-                float mk[CS], rr[CS];
-                lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
-                lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+                [[maybe_unused]] float mk[CS], rr[CS];
+                if constexpr (!kRegMaps) {
+                  lds_f<CS>(maps_lane + (uint32_t)((v * CH + h) * LPS) * (CS * 4), mk);
+                  lds_f<CS>(maps_lane + kMapFloats * 4 + (uint32_t)((v * CH + h) * LPS) * (CS * 4), rr);
+                }
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = calib(u16lo_to_f(ww), mk[e], rr[e]);
-                  const float a1 = calib(u16hi_to_f(ww), mk[e + 1], rr[e + 1]);
+                  const int jj = kRegMaps ? v * V + h * CS + e : 0;
+                  const float a0 = calib(u16lo_to_f(ww), kRegMaps ? mkr[jj] : mk[e], kRegMaps ? rrr[jj] : rr[e]);
+                  const float a1 = calib(u16hi_to_f(ww), kRegMaps ? mkr[jj + (kRegMaps ? 1 : 0)] : mk[e + 1],
+                                         kRegMaps ? rrr[jj + (kRegMaps ? 1 : 0)] : rr[e + 1]);
                   if constexpr (MODE == 1) {
                     const float m0 = set_lt_abs(a0, T_cm), m1 = set_lt_abs(a1, T_cm);
                     n0 += m0, n1 += m1;
