@@ -58,7 +58,17 @@ def _n_groups(npix, seg_cols, stages):
 
 
 def build(force: bool = False) -> str:
-    """Compile pdp_oracle.c with gcc -O2 (no SIMD intrinsics, OpenMP over frames)."""
+    """Compile pdp_oracle.c with gcc -O2 (no SIMD intrinsics, OpenMP over frames).
+
+    PDP_ORACLE_SANITIZE=1 builds a separate AddressSanitizer + UndefinedBehaviorSanitizer library instead
+    (run the CPU tests with LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0)."""
+    if os.environ.get("PDP_ORACLE_SANITIZE") == "1":
+        lib = _LIB.replace(".so", "_san.so")
+        if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+            subprocess.check_call(["gcc", "-O1", "-g", "-std=c11", "-fopenmp", "-fsanitize=address,undefined",
+                                   "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-shared", "-fPIC",
+                                   _SRC, "-o", lib, "-lm"])
+        return lib
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         subprocess.check_call(["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", _SRC,
                                "-o", _LIB, "-lm"])
