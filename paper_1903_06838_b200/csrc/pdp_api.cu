@@ -103,6 +103,7 @@ struct pdp_ctx {
   int keep_cm = 0;
   int64_t cm_frames = 0;                    // frames of the last call whose estimates are in d_cm
   LaunchPlan plan;
+  uint32_t *h_stat = nullptr, *d_stat = nullptr;   // mapped host words {hits, frames} of the last batch (pdp_accum_kernel)
   ChainPlan cplan[3];                       // 4, 8, 12 sparse warps (16, 12, 8 dense ones): sparse ... dense data
   int sparse_override = 0;                  // pdp_debug_set("sparse_warps"): 0 default (4), 4, 8
   ChainVariant forced{0, 0, 0};             // pdp_debug_set("variant")
@@ -287,6 +288,7 @@ KernelFn kernel_for(int V, int G) {
 
 void free_ctx(pdp_ctx *c) {
   if (!c) return;
+  if (c->h_stat) cudaFreeHost(c->h_stat);
   cudaFree(c->d_ped);
   cudaFree(c->d_gain);
   cudaFree(c->d_K);
@@ -592,6 +594,15 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
     c->seed_cap = (int)std::min<long long>(8192, std::max<long long>(256, (most + 31) / 32 * 32));
     PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 12 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
   }
+  if (!c->h_stat) {   // density hint of the last batch, written by pdp_accum_kernel (failure to map: no hint)
+    if (cudaHostAlloc(&c->h_stat, 2 * sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess) {
+      c->h_stat[0] = c->h_stat[1] = 0u;
+      if (cudaHostGetDevicePointer(&c->d_stat, c->h_stat, 0) != cudaSuccess) c->d_stat = nullptr;
+    } else {
+      c->h_stat = nullptr;
+      (void)cudaGetLastError();
+    }
+  }
   k.seed_scratch = c->d_seed_scratch;
   k.seed_cap = c->seed_cap;
   k.off_cm = pl.off_cm;
@@ -629,6 +640,7 @@ int enqueue_accum(pdp_ctx *c, int n, cudaStream_t st, const pdp_output &o) {
   q.hit_pixel = o.hit_pixel;
   q.hit_nphot = o.hit_nphot;
   q.accum = o.accum;
+  q.stat = c->d_stat;
   const int grid_a = (int)((c->npix + q.span - 1) / q.span);
   pdp::pdp_accum_kernel<<<grid_a, pdp::kPostThreads, (size_t)q.span * 4, st>>>(q);
   PDP_CUDA(c, cudaGetLastError());
@@ -724,7 +736,18 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   if (c->n_stages > 0) return enqueue_staged(c, raw, n, st, o);
   // ---- large batches: the throughput kernel (frame-owner CTAs) ----
   {
-    int which = c->sparse_override == 12 ? 2 : (c->sparse_override == 8 ? 1 : 0);
+    // Sparse warps: 4 by default; 8 when the previous batch was dense in hits (measured: above 1 % of
+    // the pixels in any mode, above 0.25 % in the guarded-mean and no-common-mode variants, whose dense pass is light).
+    // The density is a hint read from mapped host memory without synchronisation; results never depend on it.
+    int which = 0;
+    if (c->sparse_override) which = c->sparse_override == 12 ? 2 : (c->sparse_override == 8 ? 1 : 0);
+    else if (c->h_stat) {
+      const uint32_t hits = ((volatile uint32_t *)c->h_stat)[0], fr = ((volatile uint32_t *)c->h_stat)[1];
+      if (fr) {
+        const double dens = (double)hits / ((double)fr * (double)c->npix);
+        if (dens > 0.01 || (dens > 0.0025 && c->prm.cm_mode != PDP_CM_MEDIAN)) which = 1;
+      }
+    }
     if (!c->cplan[which].ok) which = 0;
     const bool can = c->cplan[which].ok;
     const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));

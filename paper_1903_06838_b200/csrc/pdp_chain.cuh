@@ -901,7 +901,7 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
       }
       // the ring slot about to be written held band gb-NB, last read by the sparse stages of bands gb-NB, gb-NB+1
       if (gb >= kNBr)
-        while (bdone[gb % kNBr] < gb - kNBr + 1 || bdone[(gb + 1) % kNBr] < gb - kNBr + 2) __nanosleep(100);
+        while (bdone[gb % kNBr] < gb - kNBr + 1 || bdone[(gb + 1) % kNBr] < gb - kNBr + 2) __nanosleep(400);
 
       float *cm_p = cmring + ((size_t)g * ring_rows + slot) * k.nseg + sg;
       unsigned long long *fl_p = flags + ((size_t)g * ring_rows + slot) * k.nseg + sg;

@@ -19,6 +19,9 @@ struct PostParams {
   const uint32_t *hit_count, *hit_pixel;
   const int32_t *hit_nphot;
   uint32_t *accum;
+  // hit density of the batch for the next launch's choice of sparse warps: {total hits, frames}, written by CTA 0
+  // to mapped host memory (a performance hint only: no result depends on it)
+  volatile uint32_t *stat;
 };
 
 constexpr int kPostThreads = 512;
@@ -26,6 +29,20 @@ constexpr int kPostThreads = 512;
 __global__ void __launch_bounds__(kPostThreads, 1) pdp_accum_kernel(const PostParams q) {
   extern __shared__ __align__(16) unsigned char smem[];
   uint32_t *acc = reinterpret_cast<uint32_t *>(smem);
+  if (q.stat && blockIdx.x == 0) {
+    unsigned long long *total = reinterpret_cast<unsigned long long *>(smem);   // before the slice is zeroed
+    if (threadIdx.x == 0) *total = 0ull;
+    __syncthreads();
+    unsigned long long t = 0;
+    for (int f = threadIdx.x; f < q.n_frames; f += blockDim.x) t += q.hit_count[f];
+    if (t) atomicAdd(total, t);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      q.stat[0] = (uint32_t)min(*total, 0xffffffffull);
+      q.stat[1] = (uint32_t)q.n_frames;
+    }
+    __syncthreads();
+  }
   const uint32_t lo = blockIdx.x * q.span;
   if (lo >= q.npix) return;
   const uint32_t hi = min(q.npix, lo + q.span), len = hi - lo;
