@@ -210,15 +210,20 @@ def probe_capacity(binding, ctx, cfg, raw, n, dev, requested=0):
     return min(cfg.max_hits, max(256, 4 * seen))
 
 
-def time_config(binding, cfg, cm_name, dev, rank, steps, warmup, rotate=1, min_warm_s=0.0, dist=None, cap_req=0):
-    """Device-resident timing of one config: returns (result dict, objects kept for the caller)."""
+def time_config(binding, cfg, cm_name, dev, rank, steps, warmup, rotate=1, min_warm_s=0.0, dist=None, cap_req=0,
+                data=None):
+    """Device-resident timing of one config: returns (result dict, objects kept for the caller).
+    `data` = (ped, gain, raw) of an earlier call on the same config and rotation (another cm mode) is reused."""
     cm = CM_MODES[cm_name]
     n = cfg.n_frames
     t0 = time.perf_counter()
-    ped, gain = synth.make_maps(cfg, dev)
-    raw = torch.empty((rotate * n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
-    synth.make_frames(cfg, first_frame_of_rank(rank, rotate * n), rotate * n, ped, gain, out=raw, block_pixels=1 << 27)
-    torch.cuda.synchronize()
+    if data is None:
+        ped, gain = synth.make_maps(cfg, dev)
+        raw = torch.empty((rotate * n, cfg.panels, cfg.rows, cfg.cols), dtype=torch.uint16, device=dev)
+        synth.make_frames(cfg, first_frame_of_rank(rank, rotate * n), rotate * n, ped, gain, out=raw, block_pixels=1 << 27)
+        torch.cuda.synchronize()
+    else:
+        ped, gain, raw = data
     gen_s = time.perf_counter() - t0
     ctx = make_context(binding, cfg, n, ped, gain, cm)
     cap = probe_capacity(binding, ctx, cfg, raw, n, dev, cap_req)
@@ -391,7 +396,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the timings of the rows beyond the hot path")
     ap.add_argument("--per-config", default="0,1,2,3,4", help="configs for the per_config table ('' = none)")
-    ap.add_argument("--per-config-modes", default="median", help="comma list of cm modes for the per_config table")
+    ap.add_argument("--per-config-modes", default="median,mean,none", help="comma list of cm modes for the per_config table")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -475,22 +480,24 @@ def main():
             (torch.as_tensor(res_o.hit_count) == (keep["out"].hit_count[:m].cpu().to(torch.int64) & 0xFFFFFFFF)).all()) \
             if rotate == 1 else None
     keep["ctx"].close()
+    head_data = (keep["ped"], keep["gain"], keep["raw"]) if rotate == 1 and not args.frames else None
     del keep
 
-    # ---- the other configs, same protocol with fewer steps (rank 0 of a single-GPU run only) ----
+    # ---- every config and common-mode estimator, same protocol with fewer steps (rank 0 of a single-GPU run only) ----
     if rank == 0 and world == 1 and args.per_config:
         table = {}
-        for mode in [m for m in args.per_config_modes.split(",") if m]:
-            for ci in [int(x) for x in args.per_config.split(",") if x != ""]:
+        for ci in [int(x) for x in args.per_config.split(",") if x != ""]:
+            data = head_data if ci == cfg.cfg_id else None
+            for mode in [m for m in args.per_config_modes.split(",") if m]:
                 key = f"cfg{ci}_{mode}"
                 if ci == cfg.cfg_id and mode == args.cm_mode and not args.frames:
                     r = dict(res)
                 else:
-                    torch.cuda.empty_cache()
                     c2 = synth.CONFIGS[ci]
                     rot = ROTATE_COPIES if c2.n_frames * c2.npix * 2 < (200 << 20) else 1
                     try:
-                        r, k2 = time_config(binding, c2, mode, dev, 0, 5, 3, rotate=rot)
+                        r, k2 = time_config(binding, c2, mode, dev, 0, 5, 3, rotate=rot, data=data)
+                        data = (k2["ped"], k2["gain"], k2["raw"])
                         k2["ctx"].close()
                         del k2
                     except Exception as exc:
@@ -498,6 +505,8 @@ def main():
                 for drop in ("generation_s", "warmup_steps_run", "launches_per_step"):
                     r.pop(drop, None)
                 table[key] = r
+            del data
+            torch.cuda.empty_cache()
         line["config"]["per_config"] = table
     # ---- the rows beyond the hot path: histograms, dense photon counting, stacked CM stages ----
     if rank == 0 and world == 1 and not args.no_extras:
