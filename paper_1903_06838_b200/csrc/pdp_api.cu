@@ -60,7 +60,7 @@ struct ChainPlan {
 // Preference order per vector width: the first entry that covers S with at most 25 % padding wins, otherwise
 // the one with the least padding.  Entries with LPS < 32 put several frames side by side in a warp.
 const ChainVariant kVariants[] = {   // measured order of preference
-    {8, 3, 16}, {8, 1, 32}, {8, 4, 16}, {8, 2, 16}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
+    {8, 3, 16}, {8, 2, 16}, {8, 1, 32}, {8, 4, 16}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
     {4, 1, 32}, {4, 2, 32}, {4, 4, 32}, {4, 8, 32},
     {2, 13, 8}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
 };
