@@ -62,8 +62,12 @@ struct ChainPlan {
 const ChainVariant kVariants[] = {   // measured order of preference
     {8, 3, 16}, {8, 2, 16}, {8, 1, 32}, {8, 4, 16}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
     {4, 1, 32}, {4, 2, 32}, {4, 4, 32}, {4, 8, 32},
-    {2, 13, 8}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
+    {2, 13, 8}, {2, 7, 16}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
 };
+// The guarded-mean and no-common-mode variants prefer fewer pixels per lane (maps in registers, two frames per warp):
+// measured on configs 0 and 2 (S = 194): <2,7,16> 2.10 / 1.63 ms against <2,13,8> 2.61 / 2.16 ms; the median is
+// the other way round (5.20 against 4.68 ms).
+const ChainVariant kVariantsLight[] = {{2, 7, 16}};
 
 pdp::ChainFn chain_kernel(const ChainVariant &v, int mode) {
   switch (v.V) {
@@ -199,7 +203,7 @@ bool make_plan(const pdp_geometry &g, size_t smem_limit, LaunchPlan &pl) {
   return false;
 }
 
-bool pick_variant(const pdp_geometry &g, ChainVariant &out) {
+bool pick_variant(const pdp_geometry &g, int cm_mode, ChainVariant &out) {
   const int S = g.seg_cols, W = g.cols;
   int V = 0;
   for (int v : {8, 4, 2})
@@ -208,6 +212,14 @@ bool pick_variant(const pdp_geometry &g, ChainVariant &out) {
       break;
     }
   if (!V) return false;
+  if (cm_mode != PDP_CM_MEDIAN)
+    for (const ChainVariant &c : kVariantsLight) {
+      const int cap = c.V * c.NV * c.LPS, pad = cap - S;
+      if (c.V == V && pad >= 0 && 4 * pad <= cap) {
+        out = c;
+        return true;
+      }
+    }
   const ChainVariant *best = nullptr;
   int best_pad = 1 << 30;
   for (const ChainVariant &c : kVariants) {
@@ -317,7 +329,7 @@ int build_chain_plans(pdp_ctx *c) {
   ChainVariant v{0, 0, 0};
   for (ChainPlan &pl : c->cplan) pl = ChainPlan{};
   if (c->forced.V) v = c->forced;
-  else if (!pick_variant(c->geo, v)) return PDP_OK;   // no variant: the small-batch kernel serves every batch
+  else if (!pick_variant(c->geo, c->prm.cm_mode, v)) return PDP_OK;   // no variant: the small-batch kernel serves every batch
   make_plan_chain(c->geo, v, 16, 4, c->smem_limit, c->cplan[0]);
   make_plan_chain(c->geo, v, 12, 8, c->smem_limit, c->cplan[1]);
   make_plan_chain(c->geo, v, 8, 12, c->smem_limit, c->cplan[2]);
@@ -455,7 +467,9 @@ int pdp_create(const pdp_geometry *geo, const float *ped, const float *gain, con
 int pdp_set_params(pdp_ctx *ctx, const pdp_params *prm) {
   if (!ctx || !prm) return fail(ctx, PDP_E_NULL, "pdp_set_params: null argument");
   if (int rc = validate_params(prm)) return fail(ctx, rc, "pdp_set_params: invalid params");
+  const bool replan = (prm->cm_mode == PDP_CM_MEDIAN) != (ctx->prm.cm_mode == PDP_CM_MEDIAN);
   ctx->prm = *prm;
+  if (replan) return build_chain_plans(ctx);   // the layout preference depends on the estimator
   return PDP_OK;
 }
 

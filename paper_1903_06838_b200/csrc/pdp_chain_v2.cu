@@ -3,6 +3,7 @@
 namespace pdp {
 ChainFn chain_lookup_v2(int nv, int lps, int mode) {
   PDP_CHAIN_CASE(2, 13, 8)   // S = 194
+  PDP_CHAIN_CASE(2, 7, 16)
   PDP_CHAIN_CASE(2, 1, 32)
   PDP_CHAIN_CASE(2, 2, 32)
   PDP_CHAIN_CASE(2, 4, 32)
