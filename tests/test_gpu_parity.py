@@ -259,6 +259,41 @@ def test_many_frames_dense(oracle, cm_mode):
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
 
 
+def test_set_params_switches_estimator_and_layout(oracle):
+    """One context, estimator changed with pdp_set_params: the throughput kernel's layout preference depends on the
+    estimator (194-pixel segments: <2,13,8> for the median, <2,7,16> otherwise), so the plans are rebuilt; every call
+    must match the oracle for the estimator in force.  The second call of each estimator runs with the sparse-warp
+    count chosen from the first call's hit density and must give the same lists."""
+    cfg, n = small(0, panels=2, occupancy=0.02), 160
+    raw, ped, gain = make(cfg, n)
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, max_frames_per_batch=n,
+                          pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu,
+                          photon_adu=cfg.photon_adu, cm_mode=0)
+    names = {}
+    for cm_mode in (0, 1, 0, 2):
+        ctx.set_params(seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu, cm_mode=cm_mode)
+        o = oracle_run(oracle, cfg, raw, ped, gain, cm_mode)
+        prev = None
+        for call in range(2):
+            out = binding.alloc_output(n, cfg.npix, cfg.max_hits, DEV)
+            ctx.process(raw, out)
+            torch.cuda.synchronize()
+            g = {k: getattr(out, k).cpu().numpy() for k in
+                 ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum", "status")}
+            g["hit_count"] = g["hit_count"].astype(np.int64) & 0xFFFFFFFF
+            g["frame_photons"] = g["frame_photons"].astype(np.int64) & 0xFFFFFFFF
+            rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu)
+            assert rep.ok, (cm_mode, call, rep.failures[:10])
+            if prev is not None:
+                for k in g:
+                    assert np.array_equal(prev[k], g[k]), (cm_mode, k)
+            prev = g
+        names[cm_mode] = ctx.last_kernel_name
+    ctx.close()
+    assert names[0] == "pdp_chain_kernel<2,13,8,0>" and names[1] == "pdp_chain_kernel<2,7,16,1>" \
+        and names[2] == "pdp_chain_kernel<2,7,16,2>", names
+
+
 @pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
 def test_many_frames_auto_kernel(oracle, cm_mode):
     """More frames than SMs: the library picks the frame-owner kernel, every CTA owns ~3 frames
