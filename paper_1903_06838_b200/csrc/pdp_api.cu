@@ -60,14 +60,14 @@ struct ChainPlan {
 // Preference order per vector width: the first entry that covers S with at most 25 % padding wins, otherwise
 // the one with the least padding.  Entries with LPS < 32 put several frames side by side in a warp.
 const ChainVariant kVariants[] = {   // measured order of preference
-    {8, 3, 16}, {8, 2, 16}, {8, 1, 32}, {8, 4, 16}, {8, 2, 32}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
+    {8, 3, 16}, {8, 1, 32}, {8, 2, 32}, {8, 4, 16}, {8, 2, 16}, {8, 3, 32}, {8, 4, 32}, {8, 6, 8}, {8, 4, 8},
     {4, 1, 32}, {4, 2, 32}, {4, 4, 32}, {4, 8, 32},
     {2, 13, 8}, {2, 7, 16}, {2, 1, 32}, {2, 2, 32}, {2, 4, 32}, {2, 8, 32}, {2, 16, 32},
 };
 // The guarded-mean and no-common-mode variants prefer fewer pixels per lane (maps in registers, two frames per warp):
 // measured on configs 0 and 2 (S = 194): <2,7,16> 2.10 / 1.63 ms against <2,13,8> 2.61 / 2.16 ms; the median is
 // the other way round (5.20 against 4.68 ms).
-const ChainVariant kVariantsLight[] = {{2, 7, 16}};
+const ChainVariant kVariantsLight[] = {{2, 7, 16}, {8, 2, 16}};   // S = 256: <8,2,16> 17.6 / 15.6 ms against <8,1,32> 22.0 / 17.9 (config 4)
 
 pdp::ChainFn chain_kernel(const ChainVariant &v, int mode) {
   switch (v.V) {

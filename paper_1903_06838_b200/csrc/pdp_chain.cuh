@@ -260,6 +260,32 @@ __device__ __forceinline__ float pass_down(const float (&b)[N], float p, float b
   return group_max<LPS>(fmaxf(m0, m1));
 }
 
+// up() and down() at the same pivot in one sweep: returns x[c] = min{b >= p}, `below` = x[c-1] = max{b < p}, c = #{b < p}.
+template <int N, int LPS>
+__device__ __forceinline__ float pass_updown(const float (&b)[N], float p, float big2, float &cnt, float &below) {
+  float c0 = 0.f, c1 = 0.f;
+  float u0 = __int_as_float(0x7f800000), u1 = u0, w0 = __int_as_float(0xff800000), w1 = w0;
+#pragma unroll
+  for (int j = 0; j + 1 < N; j += 2) {
+    const float d0 = set_lt(b[j], p), d1 = set_lt(b[j + 1], p);
+    c0 += d0;
+    c1 += d1;
+    const float t0 = fmaf(d0, big2, b[j]), t1 = fmaf(d1, big2, b[j + 1]);                  // values below p pushed up
+    const float s0 = fmaf(1.f - d0, -big2, b[j]), s1 = fmaf(1.f - d1, -big2, b[j + 1]);    // values >= p pushed down
+    if (j & 2) u1 = min3(u1, t0, t1), w1 = max3(w1, s0, s1);
+    else u0 = min3(u0, t0, t1), w0 = max3(w0, s0, s1);
+  }
+  if constexpr (N & 1) {
+    const float d0 = set_lt(b[N - 1], p);
+    c0 += d0;
+    u0 = fminf(u0, fmaf(d0, big2, b[N - 1]));
+    w0 = fmaxf(w0, fmaf(1.f - d0, -big2, b[N - 1]));
+  }
+  cnt = group_count<LPS>(c0 + c1);
+  below = group_max<LPS>(fmaxf(w0, w1));
+  return group_min<LPS>(fminf(u0, u1));
+}
+
 // Exact median of the masked values of a row segment held by a group of LPS lanes (N values per lane; values
 // outside the mask and padding are exactly `big`).  n = number of masked values (> 0), mean = their mean.
 // All lanes of the warp run this together; the lanes of a group hold identical scalar state.
@@ -282,6 +308,58 @@ __device__ __forceinline__ float group_median(const float (&b)[N], int n, float 
   int c_prev = 0, it = 0;
   float xl = 0.f, xh = 0.f, prev = 0.f;
   bool got = false, has_prev = false;
+  if constexpr (LPS >= 16) {
+    // ---- straight-line start for layouts with one or two lane groups per warp (with four, LPS = 8, it measured
+    // slower than the state machine alone): two counting passes steer a third pivot by the secant
+    // through them, and one up+down pass there reads x[c-1] and x[c].  When c falls on the wanted ranks the median is
+    // known; otherwise the state machine below continues from what is known (walking, or searching when still far).
+    const float p1 = fminf(fmaxf(mean, -T_cm), T_cm);
+    const float c1 = pass_count<N, LPS>(b, p1);
+    const float p2 = fminf(fmaxf(fmaf(tgt - c1, apr, p1), -T_cm), T_cm);
+    const float c2 = pass_count<N, LPS>(b, p2);
+    const float dc = c2 - c1;
+    const float sec = (p2 - p1) * rcp_approx(dc);
+    const bool sec_ok = dc != 0.f && sec > 0.f;
+    if (sec_ok && fabsf(dc) >= 8.f) apr = fmaf(0.25f, sec - apr, apr);
+    // bracket of the wanted pivot: c(lo) < tgt < c(hi) (so c(lo) <= kl: a walk up from lo is always valid)
+    if (c1 < tgt) lo = fmaxf(lo, p1);
+    if (c1 > tgt) hi = fminf(hi, p1);
+    if (c2 < tgt) lo = fmaxf(lo, p2);
+    if (c2 > tgt) hi = fminf(hi, p2);
+    float p3 = fabsf(tgt - c2) <= 0.5f ? p2 : fmaf(tgt - c2, sec_ok ? sec : apr, p2);
+    if (!(p3 >= lo && p3 <= hi)) p3 = 0.5f * (lo + hi);
+    float c3f, B3;
+    const float A3 = pass_updown<N, LPS>(b, p3, big2, c3f, B3);   // A3 = x[c3], B3 = x[c3 - 1]
+    const int c3 = (int)c3f;
+    if (c3f < tgt) lo = fmaxf(lo, p3);
+    if (c3f > tgt) hi = fminf(hi, p3);
+    phase = 4;
+    p = p3, p_prev = p3;
+    c_prev = c3, it = 1;
+    if (active) {
+      if (c3 == kh && kl != kh) xl = B3, xh = A3;                 // even count: the pivot separates the two middle ones
+      else if (c3 == kl && kl == kh) xl = xh = A3;                // odd count
+      else if (c3 == kh + 1 && kl == kh) xl = xh = B3;
+      else if (c3 <= kl && kl - c3 <= 2) {                        // walk up from x[c3]
+        phase = 1;
+        if (c3 == kl) xl = A3, got = true;
+        prev = A3, has_prev = true, p = next_up(A3);
+      } else if (c3 > kh && c3 - kh <= 3) {                       // walk down from x[c3 - 1]
+        phase = 2;
+        if (c3 - 1 == kh) xh = B3, got = true;
+        prev = B3, has_prev = true, p = B3;
+      } else {                                                    // still far: search on, from (p3, c3)
+        phase = 0;
+        float pn = fmaf(tgt - c3f, sec_ok ? sec : apr, p3);
+        if (!(pn > lo && pn < hi)) pn = 0.5f * (lo + hi);
+        if (!(pn > lo && pn < hi)) {
+          phase = 1;
+          pn = lo;
+        }
+        p = pn;
+      }
+    }
+  }
 #pragma unroll 1
   for (;;) {
     // which phases are present in the warp: one REDUX.OR (LPS < 32), or the warp-uniform state itself

@@ -4,6 +4,7 @@ namespace pdp {
 ChainFn chain_lookup_v4(int nv, int lps, int mode) {
   PDP_CHAIN_CASE(4, 1, 32)
   PDP_CHAIN_CASE(4, 2, 32)
+  PDP_CHAIN_CASE(4, 3, 32)
   PDP_CHAIN_CASE(4, 4, 32)
   PDP_CHAIN_CASE(4, 8, 32)
   return nullptr;
