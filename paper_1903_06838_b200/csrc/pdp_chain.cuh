@@ -1,29 +1,34 @@
-// pdp_chain.cuh — the throughput kernel of the reduction chain (one launch per pdp_process call).
+// pdp_chain.cuh — the throughput kernel of the reduction chain (one launch per pdp_process call, followed by the
+// accumulated-image pass of pdp_post.cuh).
 //
 // Decomposition: frame-owner.  CTA b owns the frames [b*n/grid, (b+1)*n/grid) and walks them in chunks of
 // kFCH frame slots, band by band (band = R rows of one panel), so the per-frame hit-list offsets are a
 // CTA-local running prefix (ordered, deterministic output without any inter-CTA exchange).
 //
-// Every warp has two jobs per band (one CTA barrier per band):
-//   * the dense pass of its (row of the band, row segment).  A warp handles FPS = 32/LPS frames at once:
+// Warp roles (dedicated; no CTA-wide barrier after the prologue):
+//   * dense warps, one per (row of the band, row segment).  A warp handles FPS = 32/LPS frames at once:
 //     LPS lanes share one row segment of one frame, every lane owns a contiguous run of N = V*NV pixels
-//     in registers.  The per-segment scalar work of the exact median (pivot policy, bracket, order-statistic
-//     read-out) is therefore amortised over N pixels per lane instead of S/32, the cross-lane reductions are
-//     log2(LPS) shuffles, and lanes of different frames run the same instruction stream.
+//     in registers.  The per-segment scalar work of the exact median is therefore amortised over N pixels per
+//     lane instead of S/32, the cross-lane reductions are log2(LPS) shuffles, and lanes of different frames run
+//     the same instruction stream.
 //       raw pixels : per-lane cp.async (LDGSTS) into a lane-major ring, kRingD steps deep (each lane copies
 //                    and later reads only its own vectors: cp.async.wait_group is the only synchronisation);
-//       maps       : K, 1/gain and npf of the segment, staged once per (band, chunk) into a lane-major
-//                    tile in shared memory (conflict-free LDS.128), shared by the FPS frames of a step;
-//       calibrate  : a = fma((2^23 + raw) - K, 1/gain, npf)        PAPER.md:L41, L51   (PRMT, FADD, FFMA; K = 2^23 +
-//                    rint(ped), npf = -(ped - rint(ped))/gain: the subtraction is exact, one rounding)
+//       maps       : pedestal and 1/gain of the lane's run, loaded once per (band, chunk): in registers for the
+//                    guarded-mean / no-common-mode variants, in a lane-major shared-memory tile (conflict-free
+//                    LDS.128) for the median variant, whose registers hold the N values of the selection;
+//       calibrate  : a = (float(raw) - ped) * (1/gain)              PAPER.md:L41, L51   (I2F.U16, FADD, FMUL; the
+//                    subtraction is exact for every pixel without signal, see calib())
 //       mask       : |a| < T_cm
-//       estimate   : exact median of the masked pixels (north_star (a)) by counting in value space, or the
-//                    paper's guarded mean sum/max(n, sqrt(S)), or none;
-//       candidates : one flag bit per unit (about 8 pixels) of the lane's run: max(a) > T_seed - margin + c.
-//   * the sparse stage of its frame slot for the band before (published by all warps before the last barrier):
-//     expand the flagged units to pixel candidates (same fp32 formula), apply the exact fp64
-//     seed rule (strict 3x3 maximum, ties to the lower index, panel edges) to every candidate, compute E, n,
-//     dx, dy in the oracle's order of operations and emit the hits in pixel order.
+//       estimate   : exact median of the masked pixels (north_star (a)) by counting in value space (a
+//                    straight-line start of three passes, then a small state machine), or the paper's guarded
+//                    mean sum/max(n, sqrt(S)), or none;
+//       candidates : one flag bit per unit (about 8 pixels) of the lane's run: max(a) > T_seed - margin + c;
+//       publish    : c and the flag word into shared-memory rings of NB band slots, bar.arrive on the slot's barrier.
+//   * sparse warps: warp s owns the bands gb = s (mod NWS) for all frame slots of the chunk: bar.sync on the slot,
+//     expand the flagged units to pixel candidates (same fp32 formula), apply the exact fp64 seed rule (strict 3x3
+//     maximum, ties to the lower index, panel edges) to every candidate, compute E, n, dx, dy in the oracle's order
+//     of operations, buffer the seeds in device scratch, chain the per-frame prefixes band to band through shared
+//     memory and copy the hits out in pixel order.
 //
 // Nothing dense is written to HBM: common-mode estimates, candidate flags and the prefix state of the ordered
 // compaction live in shared memory.  The accumulated image is NOT touched here (pdp_post.cuh scatters the
