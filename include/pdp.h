@@ -204,6 +204,26 @@ int pdp_histograms(pdp_ctx *ctx, const pdp_output *lists, int32_t n_frames, cons
                    void *cuda_stream);
 
 /*
+ * pdp_histograms_static — the same summarization for callers that cannot allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc).  It takes NO context and calls no cudaMalloc, cudaFree or
+ * allocating library routine: the workspace of per-CTA partial histograms is a file-scope static __device__ array
+ * of 128 x PDP_STATIC_HIST_MAX_BINS uint32 words (2 MiB), held by every GPU that loads the library until the
+ * process exits.  Arguments, bin rule, += semantics and results are those of pdp_histograms (bit-identical); it
+ * runs on the CURRENT device, on `cuda_stream`, and returns after enqueueing two kernels.
+ * Limit: energy->nbins + 2 * dxy->nbins <= PDP_STATIC_HIST_MAX_BINS, else PDP_E_VALUE (n_frames is not limited).
+ * Every call shares the array: calls that overlap on the GPU (two streams without an ordering between them, or two
+ * threads on one device) race on it and give wrong counts; calls on one stream, or ordered by events, are safe.
+ * The array keeps the last call's contents; nothing in it needs clearing (each call overwrites every word it
+ * later reads).  Errors: PDP_E_NULL, PDP_E_BATCH, PDP_E_VALUE, PDP_E_CUDA; pdp_static_last_error returns the
+ * message of the calling thread's last failing call ("" when none).
+ */
+#define PDP_STATIC_HIST_MAX_BINS 4096
+int pdp_histograms_static(const pdp_output *lists, int32_t n_frames, const pdp_hist_spec *energy,
+                          uint32_t *hist_energy, const pdp_hist_spec *dxy, uint32_t *hist_dx, uint32_t *hist_dy,
+                          void *cuda_stream);
+const char *pdp_static_last_error(void);
+
+/*
  * Stacked common-mode stages on other group shapes ("other types of common mode (row, column, block)
  * can be easily extracted by reshaping tensors accordingly"; L117: the paper's timed model has "3 stacked common
  * mode stages").  A stage tiles every panel with groups of group_rows x group_cols pixels (row segment: 1 x S, column

@@ -20,7 +20,8 @@ STATUS_HIT_OVERFLOW = 1
 
 EXPORTS = ("pdp_create", "pdp_process", "pdp_process_pinned", "pdp_process_host", "pdp_debug_set", "pdp_histograms", "pdp_process_dense", "pdp_set_cm_stages", "pdp_set_params", "pdp_destroy",
            "pdp_last_launch_count", "pdp_last_kernel_name", "pdp_keep_common_mode", "pdp_get_common_mode", "pdp_strerror",
-           "pdp_last_error", "pdp_version")
+           "pdp_last_error", "pdp_version", "pdp_histograms_static", "pdp_static_last_error")
+STATIC_HIST_MAX_BINS = 4096   # PDP_STATIC_HIST_MAX_BINS
 
 
 class pdp_geometry(ctypes.Structure):
@@ -99,6 +100,10 @@ def load_library(path: str | None = None) -> ctypes.CDLL:
     lib.pdp_last_error.argtypes = [ctypes.c_void_p]
     lib.pdp_last_error.restype = ctypes.c_char_p
     lib.pdp_version.restype = ctypes.c_int
+    lib.pdp_histograms_static.argtypes = [ctypes.POINTER(pdp_output), ctypes.c_int32, ctypes.POINTER(pdp_hist_spec),
+                                          ctypes.c_void_p, ctypes.POINTER(pdp_hist_spec), ctypes.c_void_p, ctypes.c_void_p,
+                                          ctypes.c_void_p]
+    lib.pdp_static_last_error.restype = ctypes.c_char_p
     if path is None:
         _lib = lib
     return lib
@@ -134,6 +139,24 @@ class Output:
     @property
     def bytes_per_frame_slots(self) -> int:
         return 20 * self.hit_capacity + 8
+
+
+def histograms_static(out: "Output", n_frames: int, *, energy=None, dxy=None, hist_energy=None, hist_dx=None, hist_dy=None,
+                      stream: torch.cuda.Stream | None = None):
+    """pdp_histograms_static: the histogram summarization with its workspace in a static device array (no context, no
+    allocation).  energy / dxy: (lo, width, nbins) or None, nbins_e + 2 * nbins_d <= STATIC_HIST_MAX_BINS; histograms:
+    CUDA int32 tensors of nbins words on the current device, +=.  Calls that overlap on the GPU race (include/pdp.h)."""
+    lib = load_library()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    o = out.c_struct()
+    es = pdp_hist_spec(*energy) if energy is not None else None
+    ds = pdp_hist_spec(*dxy) if dxy is not None else None
+    ptr = lambda t: t.data_ptr() if t is not None else None
+    rc = lib.pdp_histograms_static(ctypes.byref(o), n_frames, ctypes.byref(es) if es else None, ptr(hist_energy),
+                                   ctypes.byref(ds) if ds else None, ptr(hist_dx), ptr(hist_dy),
+                                   ctypes.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise PdpError(rc, "pdp_histograms_static", lib.pdp_static_last_error().decode())
 
 
 def alloc_output(n_frames: int, npix: int, hit_capacity: int, device="cuda", accum: torch.Tensor | None = None) -> Output:

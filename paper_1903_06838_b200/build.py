@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpdp.so")
 OBJDIR = os.path.join(HERE, "build")
-SOURCES = ["pdp_api.cu", "pdp_chain_v8.cu", "pdp_chain_v4.cu", "pdp_chain_v2.cu"]
+SOURCES = ["pdp_api.cu", "pdp_chain_v8.cu", "pdp_chain_v4.cu", "pdp_chain_v2.cu", "pdp_noalloc.cu"]
 HEADERS = ["pdp_device.cuh", "pdp_fused.cuh", "pdp_chain.cuh", "pdp_chain_inst.cuh", "pdp_post.cuh", "pdp_dense.cuh", "pdp_staged.cuh",
            os.path.join("..", "..", "include", "pdp.h")]
 
