@@ -25,7 +25,8 @@
  * estimate of the segment, v2 = v1 - c.
  *
  * All functions return 0 on success and a negative pdp_status on failure.
- * No function throws; no function allocates on the pdp_process() path.
+ * No function throws; nothing is allocated on the pdp_process() path: its workspaces are taken in pdp_create()
+ * and pdp_set_cm_stages(); pdp_process_pinned(), pdp_histograms() and pdp_process_dense() size theirs on first use.
  */
 #ifndef PDP_H
 #define PDP_H
@@ -242,7 +243,7 @@ typedef struct pdp_cm_stage {
  * pdp_set_cm_stages — n_stages = 1..3 switches pdp_process / pdp_process_pinned of this context to the general path
  * (a float32 working image in device memory, one kernel per stage: slower than the fused hot path, whose single
  * row-segment stage is what n_stages = 0 restores; params.cm_mode and geometry.seg_cols are ignored while stages are
- * set).  `stages` is a HOST array, copied.  Errors: PDP_E_NULL, PDP_E_VALUE, PDP_E_GEOMETRY (a group does not tile
+ * set; the working image, at most 1 GiB, is allocated here).  `stages` is a HOST array, copied.  Errors: PDP_E_NULL, PDP_E_VALUE, PDP_E_GEOMETRY (a group does not tile
  * the panel).  Must not race with pdp_process.
  */
 int pdp_set_cm_stages(pdp_ctx *ctx, const pdp_cm_stage *stages, int32_t n_stages);

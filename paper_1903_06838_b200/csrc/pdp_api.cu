@@ -91,7 +91,7 @@ struct pdp_ctx {
   double *d_rg64 = nullptr;
   unsigned long long *d_lookback = nullptr;
   unsigned *d_ticket = nullptr;
-  uint32_t *d_seed_scratch = nullptr;       // throughput kernel: seed buffers [SMs][8 warps][6][seed_cap], on first use
+  uint32_t *d_seed_scratch = nullptr;       // throughput kernel: seed buffers [SMs][12 warps][6][seed_cap] (build_chain_plans)
   int seed_cap = 0;
   int n_stages = 0;                         // pdp_set_cm_stages: 0 = the hot path's single row-segment stage
   pdp_cm_stage stages[3] = {};
@@ -324,6 +324,8 @@ void free_ctx(pdp_ctx *c) {
   delete c;
 }
 
+int alloc_staged(pdp_ctx *c);   // defined with the general common-mode path below
+
 // (Re)build the throughput-kernel plans for the current variant choice.
 int build_chain_plans(pdp_ctx *c) {
   ChainVariant v{0, 0, 0};
@@ -346,6 +348,26 @@ int build_chain_plans(pdp_ctx *c) {
     }
   }
   if (c->forced.V && !c->cplan[0].ok) return fail(c, PDP_E_GEOMETRY, "pdp_debug_set: variant does not fit this geometry");
+  // Workspace of the throughput kernel, allocated here (pdp_create / replanning), never on the pdp_process path.
+  int r_max = 0;
+  for (const ChainPlan &pl : c->cplan)
+    if (pl.ok) r_max = std::max(r_max, pl.R);
+  if (r_max > 0 && !c->d_seed_scratch) {
+    // a band of all 16 frame slots can hold at most 16 * R * W / 2 seeds per panel row block; 8192 buffered seeds
+    // let several bands be evaluated at the same time even on dense data (a full buffer only chains earlier)
+    const long long most = (long long)pdp::kFCH * (r_max + 1) * ((c->geo.cols + 1) / 2);
+    c->seed_cap = (int)std::min<long long>(8192, std::max<long long>(256, (most + 31) / 32 * 32));
+    PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 12 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
+  }
+  if (r_max > 0 && !c->h_stat) {   // density hint of the last batch, written by pdp_accum_kernel (failure to map: no hint)
+    if (cudaHostAlloc(&c->h_stat, 2 * sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess) {
+      c->h_stat[0] = c->h_stat[1] = 0u;
+      if (cudaHostGetDevicePointer(&c->d_stat, c->h_stat, 0) != cudaSuccess) c->d_stat = nullptr;
+    } else {
+      c->h_stat = nullptr;
+      (void)cudaGetLastError();
+    }
+  }
   return PDP_OK;
 }
 
@@ -484,6 +506,7 @@ int pdp_set_cm_stages(pdp_ctx *ctx, const pdp_cm_stage *stages, int32_t n_stages
   }
   ctx->n_stages = n_stages;
   for (int s = 0; s < n_stages; ++s) ctx->stages[s] = stages[s];
+  if (n_stages > 0) return alloc_staged(ctx);
   return PDP_OK;
 }
 
@@ -601,22 +624,6 @@ int enqueue_chain(pdp_ctx *c, const ChainPlan &pl, const uint16_t *raw, int n, c
   k.accum = o.accum;
   k.status = o.status;
   k.cm_keep = keep_cm ? c->d_cm : nullptr;
-  if (!c->d_seed_scratch) {
-    // a band of all 16 frame slots can hold at most 16 * R * W / 2 seeds per panel row block; 8192 buffered seeds
-    // let several bands be evaluated at the same time even on dense data (a full buffer only chains earlier)
-    const long long most = (long long)pdp::kFCH * (pl.R + 1) * ((c->geo.cols + 1) / 2);
-    c->seed_cap = (int)std::min<long long>(8192, std::max<long long>(256, (most + 31) / 32 * 32));
-    PDP_CUDA(c, cudaMalloc(&c->d_seed_scratch, (size_t)c->num_sms * 12 * 6 * (size_t)c->seed_cap * sizeof(uint32_t)));
-  }
-  if (!c->h_stat) {   // density hint of the last batch, written by pdp_accum_kernel (failure to map: no hint)
-    if (cudaHostAlloc(&c->h_stat, 2 * sizeof(uint32_t), cudaHostAllocMapped) == cudaSuccess) {
-      c->h_stat[0] = c->h_stat[1] = 0u;
-      if (cudaHostGetDevicePointer(&c->d_stat, c->h_stat, 0) != cudaSuccess) c->d_stat = nullptr;
-    } else {
-      c->h_stat = nullptr;
-      (void)cudaGetLastError();
-    }
-  }
   k.seed_scratch = c->d_seed_scratch;
   k.seed_cap = c->seed_cap;
   k.off_cm = pl.off_cm;
@@ -662,9 +669,9 @@ int enqueue_accum(pdp_ctx *c, int n, cudaStream_t st, const pdp_output &o) {
   return PDP_OK;
 }
 
-// The general common-mode path (pdp_staged.cuh): calibrate into a working image, one kernel per stage, the finder,
-// the accumulated image; frames in chunks that bound the working image.
-int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o) {
+// Working image and estimate buffers of the general common-mode path: allocated when the stages are set
+// (pdp_set_cm_stages), never on the pdp_process path.
+int alloc_staged(pdp_ctx *c) {
   const size_t npix = c->npix;
   if (!c->d_st_v) {
     const size_t budget = (size_t)1 << 30;   // ~1 GiB of working image
@@ -681,6 +688,13 @@ int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, cons
     PDP_CUDA(c, cudaMalloc(&c->d_st_est, est_per_frame * c->st_chunk * sizeof(float)));
     c->st_est_floats = est_per_frame * c->st_chunk;
   }
+  return PDP_OK;
+}
+
+// The general common-mode path (pdp_staged.cuh): calibrate into a working image, one kernel per stage, the finder,
+// the accumulated image; frames in chunks that bound the working image.
+int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_output &o) {
+  const size_t npix = c->npix;
   for (int f0 = 0; f0 < n; f0 += c->st_chunk) {
     const int m = std::min(c->st_chunk, n - f0);
     pdp::StParams k{};

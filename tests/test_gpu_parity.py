@@ -259,6 +259,32 @@ def test_many_frames_dense(oracle, cm_mode):
     assert rep.hits_oracle > 10000 and rep.exempt_hits <= rep.hits_oracle // 200
 
 
+@pytest.mark.parametrize("path", ["chain", "lookback", "staged"])
+def test_process_path_allocates_nothing(path):
+    """include/pdp.h: no allocation on the pdp_process path.  The workspaces are taken in pdp_create (throughput
+    kernel: seed scratch, density hint) and pdp_set_cm_stages (working image): the device's free memory is the
+    same before the first pdp_process call and after it."""
+    cfg, n = small(0, panels=2, occupancy=0.02), 160
+    raw, ped, gain = make(cfg, n)
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, max_frames_per_batch=n,
+                          pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu,
+                          photon_adu=cfg.photon_adu, cm_mode=0)
+    if path == "staged":
+        ctx.set_cm_stages([(1, cfg.seg_cols, 1), (cfg.rows, 1, 1)])
+    else:
+        ctx.debug_set("kernel", KERNELS[path])
+    out = binding.alloc_output(n, cfg.npix, cfg.max_hits, DEV)
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(2):
+        ctx.process(raw, out)
+    torch.cuda.synchronize()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 == free0, (free0, free1)
+    assert int((out.hit_count.to(torch.int64) & 0xFFFFFFFF).sum()) > 1000
+    ctx.close()
+
+
 def test_set_params_switches_estimator_and_layout(oracle):
     """One context, estimator changed with pdp_set_params: the throughput kernel's layout preference depends on the
     estimator (194-pixel segments: <2,13,8> for the median, <2,7,16> otherwise), so the plans are rebuilt; every call
