@@ -906,8 +906,10 @@ int pdp_process_pinned(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
     if (!ctx->copy_stream) PDP_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
     cs = ctx->copy_stream;
   }
-  // the copy stream must not overwrite a feed buffer that earlier work on `st` still reads
-  for (int i = 0; i < 2; ++i) PDP_CUDA(ctx, cudaEventRecord(ctx->ev_free[i], st));
+  // The copy stream must not overwrite a feed buffer that an earlier call's kernels still read: ev_free[b] was recorded
+  // after the last kernel that read buffer b (below), on whatever stream that call used, and a wait on an event that
+  // was never recorded is a no-op.  Nothing is recorded here, so back-to-back calls keep the copy engine busy while the
+  // previous call's last chunk is still being processed.
   int launches = 0;
   for (int f0 = 0, i = 0; f0 < n_frames; f0 += chunk_frames, ++i) {
     const int b = i & 1, n = std::min(chunk_frames, n_frames - f0);
