@@ -273,7 +273,7 @@ const char *pdp_last_kernel_name(const pdp_ctx *ctx);
  *   "chunk_frames"  frames per work item of the small-batch kernel (0 = automatic);
  *   "sparse_warps"  warps of the throughput kernel that evaluate seed candidates: 4, 8 or 12, or 0 = automatic
  *                   (default): 4, and 8 when the PREVIOUS batch of this context had hits on more than 1 % of its
- *                   pixels (0.25 % with PDP_CM_MEAN_GUARDED / PDP_CM_NONE).  The hit density of a batch is a
+ *                   pixels (0.25 % with PDP_CM_MEAN_GUARDED / PDP_CM_NONE, which take 12 above 2 %).  The hit density of a batch is a
  *                   performance hint the library reads from mapped host memory without synchronising;
  *   "variant"       V*10000 + NV*100 + LPS: pin the throughput kernel's layout (pixels per vector, vectors per
  *                   lane, lanes per row segment), 0 = automatic; PDP_E_GEOMETRY if it does not cover seg_cols.

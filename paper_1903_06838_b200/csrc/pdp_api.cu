@@ -765,7 +765,8 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
   // ---- large batches: the throughput kernel (frame-owner CTAs) ----
   {
     // Sparse warps: 4 by default; 8 when the previous batch was dense in hits (measured: above 1 % of
-    // the pixels in any mode, above 0.25 % in the guarded-mean and no-common-mode variants, whose dense pass is light).
+    // the pixels in any mode, above 0.25 % in the guarded-mean and no-common-mode variants, whose dense pass is light);
+    // 12 above 2 % in those two variants.
     // The density is a hint read from mapped host memory without synchronisation; results never depend on it.
     int which = 0;
     if (c->sparse_override) which = c->sparse_override == 12 ? 2 : (c->sparse_override == 8 ? 1 : 0);
@@ -774,6 +775,7 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
       if (fr) {
         const double dens = (double)hits / ((double)fr * (double)c->npix);
         if (dens > 0.01 || (dens > 0.0025 && c->prm.cm_mode != PDP_CM_MEDIAN)) which = 1;
+        if (dens > 0.02 && c->prm.cm_mode != PDP_CM_MEDIAN) which = 2;   // config 3: 5.6 -> 4.9 ms (mean), 6.3 -> 5.0 ms (none)
       }
     }
     if (!c->cplan[which].ok) which = 0;

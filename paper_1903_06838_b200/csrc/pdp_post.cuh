@@ -52,17 +52,34 @@ __global__ void __launch_bounds__(kPostThreads, 1) pdp_accum_kernel(const PostPa
     const uint32_t cnt = min(q.hit_count[f], q.cap);
     const uint32_t *px = q.hit_pixel + (size_t)f * q.cap;
     const int32_t *np = q.hit_nphot + (size_t)f * q.cap;
-    uint32_t a = 0, b = cnt;
-    while (a < b) {   // first hit with pixel >= lo
-      const uint32_t m = (a + b) >> 1;
-      if (__ldg(px + m) < lo) a = m + 1;
-      else b = m;
+    // [a, e) = the frame's hits inside the range: two binary searches run in lock-step (two independent chains of
+    // loads), then the hits are read four at a time with independent loads (a walk that stops at the first pixel
+    // >= hi would serialise one L2 round trip per hit)
+    uint32_t a = 0, a_hi = cnt, e = 0, e_hi = cnt;
+    while (a < a_hi || e < e_hi) {
+      const uint32_t ma = (a + a_hi) >> 1, me = (e + e_hi) >> 1;
+      const uint32_t va = a < a_hi ? __ldg(px + ma) : 0u, ve = e < e_hi ? __ldg(px + me) : 0u;
+      if (a < a_hi) {
+        if (va < lo) a = ma + 1;
+        else a_hi = ma;
+      }
+      if (e < e_hi) {
+        if (ve < hi) e = me + 1;
+        else e_hi = me;
+      }
     }
-    for (uint32_t i = a; i < cnt; ++i) {
-      const uint32_t pix = __ldg(px + i);
-      if (pix >= hi) break;
-      const int32_t n = __ldg(np + i);
-      if (n) atomicAdd(&acc[pix - lo], (uint32_t)n);   // shared memory (ATOMS)
+    for (uint32_t i = a; i < e; i += 4) {
+      uint32_t pix[4];
+      int32_t n[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const uint32_t ii = min(i + j, e - 1);
+        pix[j] = __ldg(px + ii);
+        n[j] = __ldg(np + ii);
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (i + j < e && n[j]) atomicAdd(&acc[pix[j] - lo], (uint32_t)n[j]);   // shared memory (ATOMS)
     }
   }
   __syncthreads();
