@@ -164,27 +164,71 @@ __device__ __forceinline__ double st_value(const StParams &k, int f, int p, int 
   return x;
 }
 
-// One CTA per frame: scan the pixels in index order, kStThreads * 4 at a time.
+// One CTA per frame, tiles of kStThreads * kFindPx pixels in index order.  Phase 1: every thread tests its kFindPx
+// consecutive pixels of the working image against the candidate threshold and the tile's candidates are compacted,
+// in pixel order, into a shared-memory list (one block scan per tile).  Phase 2: one candidate per thread is evaluated
+// exactly in fp64 (3x3 window from raw, pedestal, 1/gain and the stage estimates, the oracle's order of operations);
+// the seeds take their ordered slots by a second block scan.  Tiles without a candidate cost one scan.
+constexpr int kFindPx = 16;
+
+__device__ __forceinline__ unsigned block_excl_scan(unsigned x, unsigned *s_warp, unsigned &total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  unsigned incl = x;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned t = __shfl_up_sync(FULL, incl, o);
+    if (lane >= o) incl += t;
+  }
+  __syncthreads();            // s_warp may still be read by the previous scan
+  if (lane == 31) s_warp[warp] = incl;
+  __syncthreads();
+  unsigned woff = 0;
+  total = 0;
+  for (int i = 0; i < nw; ++i) {
+    if (i < warp) woff += s_warp[i];
+    total += s_warp[i];
+  }
+  return woff + incl - x;
+}
+
 __global__ void __launch_bounds__(kStThreads) pdp_st_find_kernel(const StParams k) {
+  __shared__ uint32_t s_list[kStThreads * kFindPx];
   __shared__ unsigned s_warp[kStThreads / 32];
   __shared__ unsigned s_base, s_phot;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const bool aligned = (k.npix & 3u) == 0u;   // every frame of the working image starts 16-byte aligned
   for (int f = blockIdx.x; f < k.n_frames; f += gridDim.x) {
     if (threadIdx.x == 0) s_base = 0u, s_phot = 0u;
     __syncthreads();
     const float *vf = k.v + (size_t)f * k.npix;
-    constexpr int PX = 4;
-    for (uint32_t b0 = 0; b0 < k.npix; b0 += kStThreads * PX) {
-      // thread t owns the PX consecutive pixels b0 + t*PX ..: pixel order = (thread, j) order
-      bool seed[PX];
-      HitRec rec[PX];
-      unsigned nseed = 0;
-      int my_ph = 0;
+    for (uint32_t b0 = 0; b0 < k.npix; b0 += kStThreads * kFindPx) {
+      // ---- phase 1: candidate mask of this thread's kFindPx consecutive pixels ----
+      const uint32_t i0 = b0 + threadIdx.x * kFindPx;
+      unsigned mask = 0u;
+      if (aligned && i0 + kFindPx <= k.npix) {
 #pragma unroll
-      for (int j = 0; j < PX; ++j) {
-        const uint32_t idx = b0 + threadIdx.x * PX + j;
-        seed[j] = false;
-        if (idx < k.npix && vf[idx] > k.cand_thr) {
+        for (int q = 0; q < kFindPx / 4; ++q) {
+          const float4 x = __ldg(reinterpret_cast<const float4 *>(vf + i0) + q);
+          mask |= (x.x > k.cand_thr ? 1u : 0u) << (4 * q) | (x.y > k.cand_thr ? 2u : 0u) << (4 * q) |
+                  (x.z > k.cand_thr ? 4u : 0u) << (4 * q) | (x.w > k.cand_thr ? 8u : 0u) << (4 * q);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < kFindPx; ++j)
+          if (i0 + j < k.npix && __ldg(vf + i0 + j) > k.cand_thr) mask |= 1u << j;
+      }
+      unsigned n_cand;
+      unsigned off = block_excl_scan(__popc(mask), s_warp, n_cand);
+      if (n_cand == 0u) continue;                       // uniform: n_cand comes from shared memory
+      for (unsigned m = mask; m; m &= m - 1u) s_list[off++] = i0 + (uint32_t)(__ffs(m) - 1);
+      __syncthreads();
+      // ---- phase 2: one candidate per thread, exact evaluation, ordered emission ----
+      for (unsigned c0 = 0; c0 < n_cand; c0 += kStThreads) {
+        const bool have = c0 + threadIdx.x < n_cand;
+        const uint32_t idx = have ? s_list[c0 + threadIdx.x] : 0u;
+        bool seed = false;
+        HitRec rec{0.f, 0.f, 0.f, 0};
+        if (have) {
           const int c = (int)(idx % k.W), r = (int)((idx / k.W) % k.H), p = (int)(idx / ((uint32_t)k.W * k.H));
           double v9[9];
           bool ex[9];
@@ -211,51 +255,32 @@ __global__ void __launch_bounds__(kStThreads) pdp_st_find_kernel(const StParams 
             if (ex[i] && !(x > y || (x == y && i > 4))) o.seed = false;   // strict maximum, ties to the lower index
           }
           if (o.seed) {
-            seed[j] = true;
-            rec[j] = make_rec(o, k.dE_ph, 1.0 / k.dE_ph);
-            ++nseed;
-            my_ph += rec[j].n;
+            seed = true;
+            rec = make_rec(o, k.dE_ph, 1.0 / k.dE_ph);
           }
         }
-      }
-      // ordered slots: exclusive scan of the per-thread seed counts over the block
-      unsigned incl = nseed;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned t = __shfl_up_sync(FULL, incl, o);
-        if (lane >= o) incl += t;
-      }
-      const int wph = __reduce_add_sync(FULL, my_ph);
-      __syncthreads();
-      if (lane == 31) s_warp[warp] = incl;
-      __syncthreads();
-      unsigned woff = 0, total = 0;
-      for (int i = 0; i < nw; ++i) {
-        if (i < warp) woff += s_warp[i];
-        total += s_warp[i];
-      }
-      unsigned pos = s_base + woff + incl - nseed;
-#pragma unroll
-      for (int j = 0; j < PX; ++j) {
-        if (!seed[j]) continue;
-        const uint32_t idx = b0 + threadIdx.x * PX + j;
-        if (pos < k.cap) {
-          const size_t o = (size_t)f * k.cap + pos;
-          k.hit_pixel[o] = idx;
-          k.hit_charge[o] = rec[j].E;
-          k.hit_nphot[o] = rec[j].n;
-          k.hit_dx[o] = rec[j].dx;
-          k.hit_dy[o] = rec[j].dy;
-        } else {
-          overflow_accum(k.accum + idx, (uint32_t)rec[j].n, k.status);
+        unsigned n_seed;
+        const unsigned pos = s_base + block_excl_scan(seed ? 1u : 0u, s_warp, n_seed);
+        const int wph = __reduce_add_sync(FULL, seed ? rec.n : 0);
+        if (seed) {
+          if (pos < k.cap) {
+            const size_t o = (size_t)f * k.cap + pos;
+            k.hit_pixel[o] = idx;
+            k.hit_charge[o] = rec.E;
+            k.hit_nphot[o] = rec.n;
+            k.hit_dx[o] = rec.dx;
+            k.hit_dy[o] = rec.dy;
+          } else {
+            overflow_accum(k.accum + idx, (uint32_t)rec.n, k.status);
+          }
         }
-        ++pos;
+        if (lane == 0 && wph) atomicAdd(&s_phot, (unsigned)wph);   // shared memory
+        __syncthreads();                                // every thread has read s_base
+        if (threadIdx.x == 0) s_base += n_seed;
+        __syncthreads();
       }
-      if (lane == 0 && wph) atomicAdd(&s_phot, (unsigned)wph);   // shared memory
-      __syncthreads();
-      if (threadIdx.x == 0) s_base += total;
-      __syncthreads();
     }
+    __syncthreads();
     if (threadIdx.x == 0) {
       k.hit_count[f] = s_base;
       k.frame_photons[f] = s_phot;
