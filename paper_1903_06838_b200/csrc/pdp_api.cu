@@ -745,9 +745,24 @@ int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, cons
     PDP_CUDA(c, cudaGetLastError());
     c->launches += 1;
     for (int s = 0; s < c->n_stages; ++s) {
-      const long long items = (long long)m * k.P * k.st[s].ngr * k.st[s].ngc;
-      const int grid_s = (int)std::min<long long>(items, (long long)c->num_sms * 8);
-      pdp::pdp_st_stage_kernel<<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+      const pdp::StageDesc &sd = k.st[s];
+      const long long items = (long long)m * k.P * sd.ngr * sd.ngc;
+      // guarded-mean stages whose rows can be read with 128-bit loads take the coalesced kernels (pdp_staged.cuh)
+      const bool vec4 = sd.mode == PDP_CM_MEAN_GUARDED && k.W % 4 == 0 && npix % 4 == 0;
+      if (vec4 && sd.gw % 4 == 0 && sd.gw >= 8 && (long long)sd.gh * sd.gw <= 2048) {   // a warp per group
+        const long long ctas = (items + pdp::kStThreads / 32 - 1) / (pdp::kStThreads / 32);
+        pdp::pdp_st_mean_small_kernel<<<(int)std::min<long long>(ctas, (long long)c->num_sms * 8), pdp::kStThreads, 0, st>>>(k, s);
+      } else if (vec4 && sd.gw % 4 == 0 && sd.gw >= 8) {
+        const int threads = (long long)sd.gh * sd.gw >= 32768 ? 1024 : pdp::kStThreads;
+        const int grid_s = (int)std::min<long long>(items, (long long)c->num_sms * (threads == 1024 ? 2 : 8));
+        pdp::pdp_st_mean_wide_kernel<<<grid_s, threads, 0, st>>>(k, s);
+      } else if (vec4 && (sd.gw == 1 || sd.gw == 2 || sd.gw == 4)) {
+        const long long citems = (long long)m * k.P * sd.ngr * ((k.W + pdp::kStColChunk - 1) / pdp::kStColChunk);
+        pdp::pdp_st_mean_cols_kernel<<<(int)std::min<long long>(citems, (long long)c->num_sms * 8), pdp::kStThreads, 0, st>>>(k, s);
+      } else {
+        const int grid_s = (int)std::min<long long>(items, (long long)c->num_sms * 8);
+        pdp::pdp_st_stage_kernel<<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+      }
       PDP_CUDA(c, cudaGetLastError());
       c->launches += 1;
     }

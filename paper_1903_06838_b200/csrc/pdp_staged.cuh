@@ -152,6 +152,170 @@ __global__ void __launch_bounds__(kStThreads) pdp_st_stage_kernel(const StParams
   }
 }
 
+// ---- guarded-mean stages, coalesced variants (the generic kernel above serves the median and odd shapes) -----------
+// Both read the group with 128-bit loads along the rows (W, the frame size and the group's first column are multiples
+// of 4 pixels) and keep the generic kernel's arithmetic: sum and count of the pixels with |v| < T_cm in double /
+// integer with a fixed reduction order, c = float(sum / max(count, sqrt(G))), subtracted from every pixel in place.
+
+// Wide groups (group_cols a multiple of 4, >= 8): one CTA per (frame, group); a warp covers 32 / lpr rows of the group
+// per pass with lpr = min(32, group_cols / 4) lanes per row.  256 threads, or 1024 for groups of >= 32768 pixels.
+__global__ void __launch_bounds__(1024) pdp_st_mean_wide_kernel(const StParams k, int s) {
+  __shared__ double sd[32];
+  __shared__ unsigned su[32];
+  const StageDesc &st = k.st[s];
+  const int groups_per_frame = k.P * st.ngr * st.ngc;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int q4 = st.gw / 4, lpr = min(32, q4), rpp = 32 / lpr;
+  const int lrow = lane / lpr, lc4 = lane - lrow * lpr;
+  const bool lane_on = lane < lpr * rpp;
+  for (int item = blockIdx.x; item < k.n_frames * groups_per_frame; item += gridDim.x) {
+    const int f = item / groups_per_frame, gidx = item - f * groups_per_frame;
+    const int p = gidx / (st.ngr * st.ngc), rem = gidx - p * (st.ngr * st.ngc);
+    const int br = rem / st.ngc, bc = rem - br * st.ngc;
+    float *base = k.v + (size_t)f * k.npix + ((size_t)p * k.H + (size_t)br * st.gh) * k.W + (size_t)bc * st.gw;
+    double sum = 0.0;
+    unsigned cnt = 0;
+    if (lane_on)
+      for (int row = warp * rpp + lrow; row < st.gh; row += nw * rpp) {
+        const float4 *rp = reinterpret_cast<const float4 *>(base + (size_t)row * k.W);
+        for (int c4 = lc4; c4 < q4; c4 += lpr) {
+          const float4 x = rp[c4];
+          if (fabsf(x.x) < k.T_cm) sum += (double)x.x, ++cnt;
+          if (fabsf(x.y) < k.T_cm) sum += (double)x.y, ++cnt;
+          if (fabsf(x.z) < k.T_cm) sum += (double)x.z, ++cnt;
+          if (fabsf(x.w) < k.T_cm) sum += (double)x.w, ++cnt;
+        }
+      }
+    const double tot = block_sum_d(sum, sd);
+    const unsigned n = block_sum_u(cnt, su);
+    const float c = (float)(tot / fmax((double)n, (double)st.sqrtG));
+    if (lane_on)
+      for (int row = warp * rpp + lrow; row < st.gh; row += nw * rpp) {
+        float4 *rp = reinterpret_cast<float4 *>(base + (size_t)row * k.W);
+        for (int c4 = lc4; c4 < q4; c4 += lpr) {
+          float4 x = rp[c4];
+          x.x -= c, x.y -= c, x.z -= c, x.w -= c;                         // "subtracted from the input signal": ALL pixels
+          rp[c4] = x;
+        }
+      }
+    if (threadIdx.x == 0) st.est[(size_t)f * groups_per_frame + gidx] = c;
+    __syncthreads();
+  }
+}
+
+// Small wide groups (<= 2048 pixels, e.g. row segments): one WARP per (frame, group), no block barrier; the lanes'
+// partial sums are added by a butterfly (the same order on every run).
+__global__ void __launch_bounds__(kStThreads) pdp_st_mean_small_kernel(const StParams k, int s) {
+  const StageDesc &st = k.st[s];
+  const int groups_per_frame = k.P * st.ngr * st.ngc;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int q4 = st.gw / 4, lpr = min(32, q4), rpp = 32 / lpr;
+  const int lrow = lane / lpr, lc4 = lane - lrow * lpr;
+  const bool lane_on = lane < lpr * rpp;
+  const long long items = (long long)k.n_frames * groups_per_frame;
+  for (long long item = (long long)blockIdx.x * nw + warp; item < items; item += (long long)gridDim.x * nw) {
+    const int f = (int)(item / groups_per_frame), gidx = (int)(item - (long long)f * groups_per_frame);
+    const int p = gidx / (st.ngr * st.ngc), rem = gidx - p * (st.ngr * st.ngc);
+    const int br = rem / st.ngc, bc = rem - br * st.ngc;
+    float *base = k.v + (size_t)f * k.npix + ((size_t)p * k.H + (size_t)br * st.gh) * k.W + (size_t)bc * st.gw;
+    double sum = 0.0;
+    unsigned cnt = 0;
+    if (lane_on)
+      for (int row = lrow; row < st.gh; row += rpp) {
+        const float4 *rp = reinterpret_cast<const float4 *>(base + (size_t)row * k.W);
+        for (int c4 = lc4; c4 < q4; c4 += lpr) {
+          const float4 x = rp[c4];
+          if (fabsf(x.x) < k.T_cm) sum += (double)x.x, ++cnt;
+          if (fabsf(x.y) < k.T_cm) sum += (double)x.y, ++cnt;
+          if (fabsf(x.z) < k.T_cm) sum += (double)x.z, ++cnt;
+          if (fabsf(x.w) < k.T_cm) sum += (double)x.w, ++cnt;
+        }
+      }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+    const unsigned n = __reduce_add_sync(FULL, cnt);
+    const float c = (float)(sum / fmax((double)n, (double)st.sqrtG));
+    if (lane_on)
+      for (int row = lrow; row < st.gh; row += rpp) {
+        float4 *rp = reinterpret_cast<float4 *>(base + (size_t)row * k.W);
+        for (int c4 = lc4; c4 < q4; c4 += lpr) {
+          float4 x = rp[c4];
+          x.x -= c, x.y -= c, x.z -= c, x.w -= c;
+          rp[c4] = x;
+        }
+      }
+    if (lane == 0) st.est[(size_t)f * groups_per_frame + gidx] = c;
+    __syncwarp();
+  }
+}
+
+// Narrow groups (group_cols 1, 2 or 4: column-wise common mode): one CTA per (frame, panel, group row, chunk of 128
+// columns); a lane owns 4 adjacent columns for all rows of the group, the 8 warps share the rows; the per-column sums
+// of the warps are added in a fixed order, then the columns of a group.
+constexpr int kStColChunk = 128;
+__global__ void __launch_bounds__(kStThreads) pdp_st_mean_cols_kernel(const StParams k, int s) {
+  __shared__ double sS[kStThreads / 32][kStColChunk];
+  __shared__ unsigned sN[kStThreads / 32][kStColChunk];
+  __shared__ double cS[kStColChunk];
+  __shared__ unsigned cN[kStColChunk];
+  __shared__ float sE[kStColChunk];
+  const StageDesc &st = k.st[s];
+  const int groups_per_frame = k.P * st.ngr * st.ngc;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const int nchunk = (k.W + kStColChunk - 1) / kStColChunk;
+  const int items = k.n_frames * k.P * st.ngr * nchunk;
+  for (int item = blockIdx.x; item < items; item += gridDim.x) {
+    const int ch = item % nchunk;
+    int t = item / nchunk;
+    const int br = t % st.ngr;
+    t /= st.ngr;
+    const int p = t % k.P, f = t / k.P;
+    const int col0 = ch * kStColChunk + lane * 4;
+    const bool on = col0 < k.W;
+    float *base = k.v + (size_t)f * k.npix + ((size_t)p * k.H + (size_t)br * st.gh) * k.W + col0;
+    double sm[4] = {0.0, 0.0, 0.0, 0.0};
+    unsigned nn[4] = {0u, 0u, 0u, 0u};
+    if (on)
+      for (int row = warp; row < st.gh; row += nw) {
+        const float4 x = *reinterpret_cast<const float4 *>(base + (size_t)row * k.W);
+        if (fabsf(x.x) < k.T_cm) sm[0] += (double)x.x, ++nn[0];
+        if (fabsf(x.y) < k.T_cm) sm[1] += (double)x.y, ++nn[1];
+        if (fabsf(x.z) < k.T_cm) sm[2] += (double)x.z, ++nn[2];
+        if (fabsf(x.w) < k.T_cm) sm[3] += (double)x.w, ++nn[3];
+      }
+#pragma unroll
+    for (int j = 0; j < 4; ++j) sS[warp][lane * 4 + j] = sm[j], sN[warp][lane * 4 + j] = nn[j];
+    __syncthreads();
+    if (threadIdx.x < kStColChunk) {
+      double a = 0.0;
+      unsigned b = 0u;
+      for (int w = 0; w < nw; ++w) a += sS[w][threadIdx.x], b += sN[w][threadIdx.x];
+      cS[threadIdx.x] = a, cN[threadIdx.x] = b;
+    }
+    __syncthreads();
+    if (threadIdx.x < kStColChunk / st.gw) {
+      const int g0 = threadIdx.x * st.gw, col = ch * kStColChunk + g0;
+      double a = 0.0;
+      unsigned b = 0u;
+      for (int j = 0; j < st.gw; ++j) a += cS[g0 + j], b += cN[g0 + j];
+      const float c = (float)(a / fmax((double)b, (double)st.sqrtG));
+      for (int j = 0; j < st.gw; ++j) sE[g0 + j] = c;
+      if (col < k.W) st.est[(size_t)f * groups_per_frame + ((size_t)p * st.ngr + br) * st.ngc + col / st.gw] = c;
+    }
+    __syncthreads();
+    if (on) {
+      const float c0 = sE[lane * 4], c1 = sE[lane * 4 + 1], c2 = sE[lane * 4 + 2], c3 = sE[lane * 4 + 3];
+      for (int row = warp; row < st.gh; row += nw) {
+        float4 *rp = reinterpret_cast<float4 *>(base + (size_t)row * k.W);
+        float4 x = *rp;
+        x.x -= c0, x.y -= c1, x.z -= c2, x.w -= c3;
+        *rp = x;
+      }
+    }
+    __syncthreads();
+  }
+}
+
 // fp64 value of pixel (p, r, c) of frame f after all stages, in the oracle's order: ((raw - ped) / gain - c1) - c2 - c3
 __device__ __forceinline__ double st_value(const StParams &k, int f, int p, int r, int c) {
   const uint32_t gi = ((uint32_t)p * (uint32_t)k.H + (uint32_t)r) * (uint32_t)k.W + (uint32_t)c;

@@ -589,6 +589,7 @@ STAGE_SETS = {
     "row_median_block_mean": [(1, 64, 0), (8, 16, 1)],
     "panel_median": [(40, 128, 0)],
     "col_median_then_none": [(10, 1, 0), (1, 128, 2)],
+    "narrow_mean_groups": [(2, 2, 1), (8, 4, 1), (40, 1, 1)],
 }
 
 
@@ -625,4 +626,28 @@ def test_stacked_common_mode_stages(oracle, name):
     assert np.array_equal(out2.hit_count.cpu().numpy().astype(np.int64), o1.hit_count)
     with pytest.raises(binding.PdpError):
         ctx.set_cm_stages([(7, 128, 1)])                                # does not tile 40 rows
+    ctx.close()
+
+
+def test_stacked_stages_large_groups(oracle):
+    """The coalesced guarded-mean kernels on groups that need their large forms: a panel-wise group of 49152 pixels
+    (1024-thread CTAs), columns of 256 rows in two column chunks (128 + 64), full rows."""
+    stages = [(1, 192, 1), (256, 1, 1), (256, 192, 1)]
+    cfg, n = small(0, panels=2, rows=256, cols=192, seg_cols=96, occupancy=0.01), 5
+    raw, ped, gain = make(cfg, n)
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, max_frames_per_batch=n,
+                          pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu, photon_adu=cfg.photon_adu)
+    ctx.set_cm_stages(stages)
+    out = binding.alloc_output(n, cfg.npix, cfg.max_hits, DEV)
+    ctx.process(raw, out)
+    torch.cuda.synchronize()
+    g = {k: getattr(out, k).cpu().numpy() for k in
+         ("hit_count", "hit_pixel", "hit_charge", "hit_nphot", "hit_dx", "hit_dy", "frame_photons", "accum", "status")}
+    g["hit_count"] = g["hit_count"].astype(np.int64) & 0xFFFFFFFF
+    g["frame_photons"] = g["frame_photons"].astype(np.int64) & 0xFFFFFFFF
+    o = oracle_run(oracle, cfg, raw, ped, gain, 0, stages=stages)
+    rep = compare(o, g, panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, cm_adu=cfg.cm_adu)
+    print(rep.summary())
+    assert rep.ok, rep.failures[:10]
+    assert rep.hits_oracle > 1000 and rep.exempt_hits <= 5
     ctx.close()
