@@ -174,7 +174,8 @@ int pdp_process_host(pdp_ctx *ctx, const uint16_t *raw_host, int32_t n_frames,
  * image[idx] += n (DEVICE uint32 [P*H*W], the photon-counting image of PAPER.md:L99, persists across calls, caller
  * zeroes) and, when frame_totals is not NULL, frame_totals[f] = sum of n over frame f (DEVICE uint32 [n_frames]).
  * zero_below_adu is the "zeroing the signal of pixels within noise" of PAPER.md:L91; pass -INFINITY for none.
- * Asynchronous on `cuda_stream`.  No atomics on global memory: a warp owns a row segment for all frames.
+ * Asynchronous on `cuda_stream`.  No atomics on global memory: a warp owns a row segment for all frames, or for a
+ * slice of them when the detector has few segments (the slices' images are then merged by a second kernel).
  * Errors: PDP_E_NULL, PDP_E_BATCH, PDP_E_ALIGN, PDP_E_VALUE (NaN), PDP_E_GEOMETRY, PDP_E_CUDA.
  */
 int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *raw_u16_batch, void *cuda_stream, float zero_below_adu,

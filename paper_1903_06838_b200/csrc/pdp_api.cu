@@ -1009,13 +1009,26 @@ int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *batch, void *stream, float 
   k.cm_mode = ctx->prm.cm_mode;
   k.cm_min_count = ctx->prm.cm_min_count > 0 ? ctx->prm.cm_min_count : (int)std::ceil(std::sqrt((double)S));
   k.image = image;
+  k.dinv_E_ph = 1.0 / (double)ctx->prm.photon_adu;
   const int nwarps = pdp::kDenseThreads / 32;
-  const int grid = std::max(1, std::min(ctx->num_sms, (k.n_tasks + nwarps - 1) / nwarps));
+  // A warp owns a row segment; with few segments (small detectors) the frames of a segment are split into slices so
+  // that every warp slot of the GPU gets about three tasks (slices of at least 64 frames); the slices accumulate into
+  // their own images, merged by pdp_dense_merge_kernel.
+  {
+    const long long slots = (long long)ctx->num_sms * nwarps;
+    long long ns = (3 * slots + k.n_tasks - 1) / k.n_tasks;
+    ns = std::max(1LL, std::min<long long>(std::min<long long>(ns, 16), n / 64));
+    k.n_slices = (int)ns;
+    k.slice_frames = (n + k.n_slices - 1) / k.n_slices;
+  }
+  const long long tasks_all = (long long)k.n_tasks * k.n_slices;
+  const int grid = (int)std::max<long long>(1, std::min<long long>(ctx->num_sms, (tasks_all + nwarps - 1) / nwarps));
   const size_t tot_bytes = frame_totals ? (((size_t)n * 4 + 127) & ~(size_t)127) : 0;
   const size_t smem = tot_bytes + (size_t)nwarps * pdp::kDenseRing * 32 * (size_t)(V * NV) * 2;
   if (smem > ctx->smem_limit) return fail(ctx, PDP_E_BATCH, "pdp_process_dense: too many frames per call for the per-frame totals");
-  if (frame_totals) {
-    const size_t need = (size_t)grid * n;
+  const size_t img_words = k.n_slices > 1 ? (size_t)k.n_slices * ctx->npix : 0;
+  {
+    const size_t need = (frame_totals ? (size_t)grid * n : 0) + img_words;
     if (ctx->dense_ws_words < need) {
       cudaFree(ctx->d_dense_ws);
       ctx->d_dense_ws = nullptr;
@@ -1023,7 +1036,10 @@ int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *batch, void *stream, float 
       PDP_CUDA(ctx, cudaMalloc(&ctx->d_dense_ws, need * sizeof(uint32_t)));
       ctx->dense_ws_words = need;
     }
-    k.partial_totals = ctx->d_dense_ws;
+  }
+  if (img_words) k.partial_image = ctx->d_dense_ws;
+  if (frame_totals) {
+    k.partial_totals = ctx->d_dense_ws + img_words;
     k.frame_totals = frame_totals;
     k.n_partials = grid;
   }
@@ -1032,10 +1048,15 @@ int pdp_process_dense(pdp_ctx *ctx, const pdp_batch *batch, void *stream, float 
   fn<<<grid, pdp::kDenseThreads, smem, st>>>(k);
   PDP_CUDA(ctx, cudaGetLastError());
   ctx->launches = 1;
+  if (k.n_slices > 1) {
+    pdp::pdp_dense_merge_kernel<<<(int)std::min<size_t>((ctx->npix + 255) / 256, (size_t)ctx->num_sms * 8), 256, 0, st>>>(k);
+    PDP_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 1;
+  }
   if (frame_totals) {
     pdp::pdp_dense_totals_kernel<<<(n + 255) / 256, 256, 0, st>>>(k);
     PDP_CUDA(ctx, cudaGetLastError());
-    ctx->launches = 2;
+    ctx->launches += 1;
   }
   std::snprintf(ctx->last_kernel_buf, sizeof(ctx->last_kernel_buf), "pdp_dense_kernel<%d,%d,%d>", V, NV, ctx->prm.cm_mode);
   ctx->last_kernel = ctx->last_kernel_buf;

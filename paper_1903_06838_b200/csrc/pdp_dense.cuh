@@ -25,6 +25,9 @@ struct DParams {
   double dE_ph, dzero_below;
   int cm_mode, cm_min_count;
   uint32_t *image;            // [npix], +=
+  uint32_t *partial_image;    // [n_slices][npix] when the frames of a segment are split over several warps, else nullptr
+  int n_slices, slice_frames; // task = (row segment, slice of slice_frames consecutive frames)
+  double dinv_E_ph;
   uint32_t *partial_totals;   // [grid][n_frames] or nullptr
   uint32_t *frame_totals;     // [n_frames] (merge kernel), or nullptr
   int n_partials;
@@ -52,7 +55,9 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
 #pragma unroll
   for (int v = 0; v < NV; ++v) vmask |= (lane * N + v * V < k.S ? 1u : 0u) << v;
 
-  for (int task = blockIdx.x * nwarps + warp; task < k.n_tasks; task += gridDim.x * nwarps) {
+  for (int task_s = blockIdx.x * nwarps + warp; task_s < k.n_tasks * k.n_slices; task_s += gridDim.x * nwarps) {
+    const int slice = task_s / k.n_tasks, task = task_s - slice * k.n_tasks;
+    const int f_lo = slice * k.slice_frames, f_hi = min(k.n_frames, f_lo + k.slice_frames);
     const int seg = task % k.nseg, prow = task / k.nseg;          // prow = panel * H + row
     const size_t off = (size_t)prow * k.W + (size_t)seg * k.S + (size_t)lane * N;   // this lane's run
     float pd[N], rg[N];
@@ -64,11 +69,11 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
       rg[j] = ok ? __ldg(k.rg + off + j) : 1.f;
       acc[j] = 0u;
     }
-    const uint16_t *src = k.raw + off;
+    const uint16_t *src = k.raw + (size_t)f_lo * npix + off;
     uint32_t islot = 0, rslot = 0;
-    int i_frame = 0;
+    int i_frame = f_lo;
     auto issue = [&]() {
-      if (i_frame < k.n_frames) {
+      if (i_frame < f_hi) {
 #pragma unroll
         for (int v = 0; v < NV; ++v)
           if ((vmask >> v) & 1u) cp_async_s<VB>(ring_lane + islot + v * (32 * VB), src + v * V);
@@ -80,7 +85,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
     };
 #pragma unroll 1
     for (int d = 0; d < kDenseRing - 1; ++d) issue();
-    for (int f = 0; f < k.n_frames; ++f) {
+    for (int f = f_lo; f < f_hi; ++f) {
       issue();
       asm volatile("cp.async.wait_group %0;" ::"n"(kDenseRing - 1) : "memory");
       float a[N], b[N];
@@ -134,7 +139,9 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
           const size_t gi = off + j;
           if (lane * N + j < k.S) {
             const double x = ((double)__ldg(k.raw + (size_t)f * npix + gi) - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - (double)c;
-            const double rr = rint(x / k.dE_ph);
+            double q = x * k.dinv_E_ph;                    // a double division is a ~130-450 cycle sequence: see photon_count()
+            if (fabs(q - floor(q) - 0.5) < 1e-9) q = exact_ratio(x, k.dE_ph);
+            const double rr = rint(q);
             r = x < k.dzero_below ? 0.f : (float)rr;
           }
         } else if (v2 < k.zero_below) {
@@ -151,14 +158,31 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
     }
     // drain the ring bookkeeping (the copies issued beyond the last frame were empty groups)
     asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (k.n_slices > 1) {   // the slices of a segment run on different warps: plain stores to the slice's own image
+      uint32_t *pim = k.partial_image + (size_t)slice * npix;
 #pragma unroll
-    for (int j = 0; j < N; ++j)
-      if (lane * N + j < k.S && acc[j]) k.image[off + j] += acc[j];
+      for (int j = 0; j < N; ++j)
+        if (lane * N + j < k.S) pim[off + j] = acc[j];
+    } else {
+#pragma unroll
+      for (int j = 0; j < N; ++j)
+        if (lane * N + j < k.S && acc[j]) k.image[off + j] += acc[j];
+    }
   }
   if (k.partial_totals) {
     __syncthreads();
     uint32_t *out = k.partial_totals + (size_t)blockIdx.x * k.n_frames;
     for (int i = threadIdx.x; i < k.n_frames; i += blockDim.x) out[i] = tot[i];
+  }
+}
+
+// image[i] += sum over the slices' images (every pixel has one owner thread: no atomics)
+static __global__ void pdp_dense_merge_kernel(const DParams k) {
+  const size_t npix = (size_t)k.P * k.H * k.W;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npix; i += (size_t)gridDim.x * blockDim.x) {
+    uint32_t s = 0;
+    for (int c = 0; c < k.n_slices; ++c) s += k.partial_image[(size_t)c * npix + i];
+    if (s) k.image[i] += s;
   }
 }
 

@@ -583,6 +583,37 @@ def test_dense_photon_counting(oracle, case, cm_mode):
         assert np.abs(tot.cpu().numpy().astype(np.int64) - o_tot.astype(np.int64)).max() <= max(3, int(frag.reshape(n, -1).any(axis=1).sum() and frag.sum()))
 
 
+@pytest.mark.parametrize("cm_mode", [0, 1], ids=["median", "mean"])
+def test_dense_photon_counting_sliced(oracle, cm_mode):
+    """Few row segments and many frames: the frames of a segment are split into slices that run on different warps
+    and accumulate into their own images (merged by pdp_dense_merge_kernel); ragged last slice (301 frames)."""
+    cfg, n = small(0, panels=2, rows=12, cols=128, seg_cols=64, occupancy=0.02), 301
+    raw, ped, gain = make(cfg, n)
+    ctx = binding.Context(panels=cfg.panels, rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, max_frames_per_batch=n,
+                          pedestal=ped.cpu(), gain=gain.cpu(), seed_adu=cfg.seed_adu, cm_adu=cfg.cm_adu,
+                          photon_adu=cfg.photon_adu, cm_mode=cm_mode)
+    img = torch.zeros(cfg.npix, dtype=torch.int32, device=DEV)
+    tot = torch.zeros(n, dtype=torch.int32, device=DEV)
+    ctx.process_dense(raw, img, tot)
+    assert ctx.last_launch_count == 3                                     # counting, slice merge, per-frame totals
+    ctx.process_dense(raw, img, None)                                     # += : twice the image
+    torch.cuda.synchronize()
+    ctx.close()
+    o_img, o_tot, frag = oracle.dense(raw.cpu().numpy(), ped.cpu().numpy(), gain.cpu().numpy(), panels=cfg.panels,
+                                      rows=cfg.rows, cols=cfg.cols, seg_cols=cfg.seg_cols, cm_adu=cfg.cm_adu,
+                                      photon_adu=cfg.photon_adu, cm_mode=cm_mode, zero_below_adu=float("-inf"),
+                                      want_fragile=True)
+    g_img = img.cpu().numpy().astype(np.int64)
+    assert np.all(g_img % 2 == 0)
+    diff = g_img // 2 != o_img.astype(np.int64)
+    fragile_px = frag.any(axis=0)
+    print(cm_mode, "photons", int(o_img.sum()), "pixels differing", int(diff.sum()), "fragile pixels", int(fragile_px.sum()))
+    assert o_img.sum() > 5 * n
+    assert not (diff & ~fragile_px).any()
+    clean = ~frag.reshape(n, -1).any(axis=1)
+    assert np.array_equal(tot.cpu().numpy().astype(np.int64)[clean], o_tot.astype(np.int64)[clean])
+
+
 STAGE_SETS = {
     "row_col_mean": [(1, 64, 1), (8, 1, 1)],
     "paper_3_stacked_mean": [(1, 128, 1), (8, 1, 1), (40, 128, 1)],          # row, column, panel-wise: PAPER.md:L117
