@@ -113,6 +113,36 @@ __device__ __forceinline__ float u16hi_to_f(uint32_t w) {   // I2F.U16 Rd, Rs.H1
 // is exact in float32 whenever |raw - pedestal| < 2^24 ulp(pedestal) (every pixel without signal), so the value carries
 // the rounding of 1/gain and of one product: relative error <= 2^-23, the bound the candidate margin is derived from.
 __device__ __forceinline__ float calib(float raw_f, float ped, float rg) { return __fmul_rn(__fsub_rn(raw_f, ped), rg); }
+// Two pixels per instruction (FADD2 / FMUL2 on register pairs): the same IEEE roundings as the scalar forms, half the
+// issue slots.  Used in the median variant's calibration loop only: measured, it gains 6 % there (config 1: 1.93 ->
+// 1.81 ms), loses 2-3 % in the guarded-mean / no-common-mode loops and gains nothing in the selection passes.
+struct F2 {
+  unsigned long long v;
+};
+__device__ __forceinline__ F2 f2_pack(float lo, float hi) {
+  F2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(F2 a, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
+__device__ __forceinline__ F2 f2_add(F2 a, F2 b) {
+  F2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+  return r;
+}
+__device__ __forceinline__ F2 f2_sub(F2 a, F2 b) {
+  F2 r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+  return r;
+}
+__device__ __forceinline__ F2 f2_mul(F2 a, F2 b) {
+  F2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+  return r;
+}
+__device__ __forceinline__ void calib2(uint32_t w, float p0, float p1, float g0, float g1, float &a0, float &a1) {
+  f2_unpack(f2_mul(f2_sub(f2_pack(u16lo_to_f(w), u16hi_to_f(w)), f2_pack(p0, p1)), f2_pack(g0, g1)), a0, a1);
+}
 __device__ __forceinline__ float magic_lo(uint32_t w) {   // 2^23 + low 16 bits, as a float (one PRMT)
   return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));
 }
@@ -1002,7 +1032,7 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
           if constexpr (MODE == 0) {
             // ================= exact median common mode (north_star (a)) =================
             float b[N];
-            float sb0 = 0.f, sb1 = 0.f;
+            F2 sb01 = f2_pack(0.f, 0.f);
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
               uint32_t w[V / 2];
@@ -1015,19 +1045,20 @@ __global__ void __launch_bounds__(kChainMaxThreads, 1) pdp_chain_kernel(const CP
 #pragma unroll
                 for (int e = 0; e < CS; e += 2) {
                   const uint32_t ww = w[(h * CS + e) / 2];
-                  const float a0 = calib(u16lo_to_f(ww), mk[e], rr[e]);
-                  const float a1 = calib(u16hi_to_f(ww), mk[e + 1], rr[e + 1]);
+                  float a0, a1;
+                  calib2(ww, mk[e], mk[e + 1], rr[e], rr[e + 1], a0, a1);
                   const int j = v * V + h * CS + e;
                   b[j] = fabsf(a0) < T_cm ? a0 : BIG;          // pixels WITHOUT signal keep their value
                   b[j + 1] = fabsf(a1) < T_cm ? a1 : BIG;
-                  sb0 += b[j];
-                  sb1 += b[j + 1];
+                  sb01 = f2_add(sb01, f2_pack(b[j], b[j + 1]));
                   amax[j / U] = max3(amax[j / U], a0, a1);
                 }
               }
             }
             // sum of the masked values and their count from ONE accumulation: sum(b) = s + n_out * BIG with
             // |s| < BIG/2 (BIG >= 4*N*T_cm); decoded per lane, then reduced over the group
+            float sb0, sb1;
+            f2_unpack(sb01, sb0, sb1);
             const float sb = sb0 + sb1;
             const float n_out_l = rintf(sb * (1.f / BIG));
             const float s_l = fmaf(-n_out_l, BIG, sb);
