@@ -389,6 +389,12 @@ def time_next_rows(binding, dev):
     res["stacked_3_mean_stages"] = {"ms": ms, "frames": m, "frames_per_s": m / ms * 1e3, "launches": ctx.last_launch_count,
                                     "alg_gbs": m * cfg.npix * bpp / ms / 1e6, "frac_of_measured": m * cfg.npix * bpp / ms / 1e6 / peak,
                                     "bytes": "%d B per pixel and frame (raw, working image written once, read+written per stage, read by the finder)" % bpp}
+    ctx.set_cm_stages([(1, cfg.seg_cols, 0), (cfg.rows, 1, 0)])      # exact medians on row segments, then on columns
+    ms = _timed(lambda: ctx.process(raw[:m], out2, n_frames=m))
+    bpp = 2 + 4 + 2 * 8 + 4
+    res["stacked_2_median_stages"] = {"ms": ms, "frames": m, "frames_per_s": m / ms * 1e3, "launches": ctx.last_launch_count,
+                                      "alg_gbs": m * cfg.npix * bpp / ms / 1e6, "frac_of_measured": m * cfg.npix * bpp / ms / 1e6 / peak,
+                                      "bytes": "%d B per pixel and frame" % bpp}
     ctx.close()
     return res
 

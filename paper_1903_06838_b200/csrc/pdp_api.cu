@@ -749,7 +749,15 @@ int enqueue_staged(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, cons
       const long long items = (long long)m * k.P * sd.ngr * sd.ngc;
       // guarded-mean stages whose rows can be read with 128-bit loads take the coalesced kernels (pdp_staged.cuh)
       const bool vec4 = sd.mode == PDP_CM_MEAN_GUARDED && k.W % 4 == 0 && npix % 4 == 0;
-      if (vec4 && sd.gw % 4 == 0 && sd.gw >= 8 && (long long)sd.gh * sd.gw <= 2048) {   // a warp per group
+      const long long gpx = (long long)sd.gh * sd.gw;
+      if (sd.mode == PDP_CM_MEDIAN && gpx <= 1024) {   // a warp per group, the values in registers
+        const long long ctas = (items + pdp::kStThreads / 32 - 1) / (pdp::kStThreads / 32);
+        const int grid_s = (int)std::min<long long>(ctas, (long long)c->num_sms * 8);
+        if (gpx <= 256) pdp::pdp_st_median_small_kernel<8><<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+        else if (gpx <= 512) pdp::pdp_st_median_small_kernel<16><<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+        else if (gpx <= 768) pdp::pdp_st_median_small_kernel<24><<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+        else pdp::pdp_st_median_small_kernel<32><<<grid_s, pdp::kStThreads, 0, st>>>(k, s);
+      } else if (vec4 && sd.gw % 4 == 0 && sd.gw >= 8 && (long long)sd.gh * sd.gw <= 2048) {   // a warp per group
         const long long ctas = (items + pdp::kStThreads / 32 - 1) / (pdp::kStThreads / 32);
         pdp::pdp_st_mean_small_kernel<<<(int)std::min<long long>(ctas, (long long)c->num_sms * 8), pdp::kStThreads, 0, st>>>(k, s);
       } else if (vec4 && sd.gw % 4 == 0 && sd.gw >= 8) {

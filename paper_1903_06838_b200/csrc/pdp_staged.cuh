@@ -249,6 +249,54 @@ __global__ void __launch_bounds__(kStThreads) pdp_st_mean_small_kernel(const StP
   }
 }
 
+// Median stages on groups of at most 32 * N pixels (row segments, columns, small blocks): one WARP per (frame, group),
+// the group's values in registers (element i of the group in lane i % 32), the exact median by the hot path's
+// register-resident selection (group_median, pdp_chain.cuh): the same value as the generic kernel's bisection — the
+// middle element, or the fp32 mean of the two middle ones — at a fraction of its passes.
+template <int N>
+__global__ void __launch_bounds__(kStThreads) pdp_st_median_small_kernel(const StParams k, int s) {
+  const StageDesc &st = k.st[s];
+  const int groups_per_frame = k.P * st.ngr * st.ngc;
+  const int G = st.gh * st.gw;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  float big = 1024.f;
+  while (big < 4.f * (float)N * k.T_cm + 1.f) big *= 2.f;   // masked-out values: above every pivot, exact in the sum decode
+  float apr = 0.375f * k.T_cm / (float)G;
+  const long long items = (long long)k.n_frames * groups_per_frame;
+  for (long long item = (long long)blockIdx.x * nw + warp; item < items; item += (long long)gridDim.x * nw) {
+    const int f = (int)(item / groups_per_frame), gidx = (int)(item - (long long)f * groups_per_frame);
+    const int p = gidx / (st.ngr * st.ngc), rem = gidx - p * (st.ngr * st.ngc);
+    const int br = rem / st.ngc, bc = rem - br * st.ngc;
+    float *base = k.v + (size_t)f * k.npix + ((size_t)p * k.H + (size_t)br * st.gh) * k.W + (size_t)bc * st.gw;
+    float x[N], b[N];
+    float sum = 0.f;
+    int cnt = 0;
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      const int i = lane + 32 * j;
+      const bool in = i < G;
+      x[j] = in ? base[(size_t)(i / st.gw) * k.W + (i % st.gw)] : 0.f;
+      const bool m = in && fabsf(x[j]) < k.T_cm;
+      b[j] = m ? x[j] : big;
+      sum += m ? x[j] : 0.f;
+      cnt += m ? 1 : 0;
+    }
+    const int n = __reduce_add_sync(FULL, cnt);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(FULL, sum, o);
+    const bool need = n > 0 && n >= st.min_count;
+    float c = group_median<N, 32>(b, n, sum * rcp_approx(fmaxf((float)n, 1.f)), k.T_cm, big, need, apr);
+    if (!need) c = 0.f;
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      const int i = lane + 32 * j;
+      if (i < G) base[(size_t)(i / st.gw) * k.W + (i % st.gw)] = x[j] - c;   // "subtracted from the input signal": ALL pixels
+    }
+    if (lane == 0) st.est[(size_t)f * groups_per_frame + gidx] = c;
+    __syncwarp();
+  }
+}
+
 // Narrow groups (group_cols 1, 2 or 4: column-wise common mode): one CTA per (frame, panel, group row, chunk of 128
 // columns); a lane owns 4 adjacent columns for all rows of the group, the 8 warps share the rows; the per-column sums
 // of the warps are added in a fixed order, then the columns of a group.

@@ -621,6 +621,7 @@ STAGE_SETS = {
     "panel_median": [(40, 128, 0)],
     "col_median_then_none": [(10, 1, 0), (1, 128, 2)],
     "narrow_mean_groups": [(2, 2, 1), (8, 4, 1), (40, 1, 1)],
+    "median_groups_in_registers": [(4, 128, 0), (20, 32, 0), (8, 128, 0)],   # 512, 640, 1024 pixels: 16, 24, 32 per lane
 }
 
 
