@@ -61,8 +61,8 @@ def kernel_source_hash() -> str:
 
 
 def recorded_traffic(cfg_id: int, cm_mode: str, n_frames: int, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch from the committed ncu capture
-    (profiles/ncu_traffic.json), or None when no capture of THIS source exists."""
+    """The committed ncu capture of this launch (profiles/ncu_traffic.json: dram__bytes_read.sum + dram__bytes_write.sum,
+    executed warp instructions per pixel-lane, issue-slot utilisation), or None when no capture of THIS source exists."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
             table = json.load(f)["captures"]
@@ -72,7 +72,7 @@ def recorded_traffic(cfg_id: int, cm_mode: str, n_frames: int, kernel: str):
     for e in table:
         if (e.get("config") == cfg_id and e.get("cm_mode") == cm_mode and e.get("n_frames") == n_frames
                 and e.get("kernel") == kernel and e.get("source_sha16") == src):
-            return e.get("dram_bytes")
+            return e
     return None
 
 
@@ -259,7 +259,8 @@ def time_config(binding, cfg, cm_name, dev, rank, steps, warmup, rotate=1, min_w
     t_end.record(stream)
     torch.cuda.synchronize()
     total_ms = max_over_ranks(t_begin.elapsed_time(t_end), dist, dev)
-    k_ms = statistics.mean(a.elapsed_time(b) for a, b in ev)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    k_ms = statistics.mean(step_ms)
     assert int(out.status.item()) == 0, "hit overflow during the bench"
     hits = float((out.hit_count.to(torch.int64) & 0xFFFFFFFF).to(torch.float64).mean().item())
     peak, peak_src = measured_peak()
@@ -268,6 +269,7 @@ def time_config(binding, cfg, cm_name, dev, rank, steps, warmup, rotate=1, min_w
            "mpixel_per_s": n * steps * cfg.npix / (total_ms * 1e-3) / 1e6,
            "raw_gbs": n * cfg.npix * 2 / (k_ms * 1e-3) / 1e9, "alg_gbs": alg / (k_ms * 1e-3) / 1e9,
            "frac_of_measured": alg / (k_ms * 1e-3) / 1e9 / peak, "frac_of_8000": alg / (k_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+           "step_ms_median": statistics.median(step_ms), "step_ms_best": min(step_ms),
            "hits_per_frame": hits, "hit_capacity": cap, "kernel": ctx.last_kernel_name,
            "launches_per_step": launches / steps, "generation_s": gen_s, "warmup_steps_run": n_warm,
            "l2": ("rotated over %d distinct copies (%.0f MB) so that a pass is not L2 resident" % (rotate, rotate * n * cfg.npix * 2 / 1e6))
@@ -457,11 +459,18 @@ def main():
         except Exception as exc:
             e2e = {"value": None, "unit": UNIT, "error": str(exc)[:200]}
 
-    traffic = recorded_traffic(cfg.cfg_id, args.cm_mode, n, res["kernel"])
+    cap_rec = recorded_traffic(cfg.cfg_id, args.cm_mode, n, res["kernel"])
+    traffic = cap_rec.get("dram_bytes") if cap_rec else None
     roofline = {"bound": "hbm", "achieved": res["alg_gbs"], "peak": keep["peak"], "unit": "GB/s",
                 "frac": res["frac_of_measured"], "traffic": traffic,
                 "traffic_source": "profiles/ncu_traffic.json (ncu --set full capture of this source)" if traffic else
                                   "no ncu capture of the current kernel source",
+                # which limit saturated.  From the same capture: warp instructions per 32 pixels (the
+                # budget at 100 % of the measured HBM rate is ~11.4) and how busy the issue slots were.
+                "inst_per_pixel_lane": cap_rec.get("inst_per_pixel_lane") if cap_rec else None,
+                "issue_slots_busy_pct": cap_rec.get("issue_slots_busy_pct") if cap_rec else None,
+                "saturated": ("instruction issue (see issue_slots_busy_pct), not DRAM" if cap_rec and
+                              cap_rec.get("issue_slots_busy_pct", 0) > 60 else None),
                 "peak_source": keep["peak_src"], "kernel": res["kernel"], "kernel_ms": res["kernel_ms"],
                 "algorithmic_bytes_per_launch": keep["alg_bytes"], "raw_gbs": res["raw_gbs"],
                 "frac_of_nominal_8TBs": res["frac_of_8000"], "source_sha16": kernel_source_hash()}
@@ -471,6 +480,7 @@ def main():
             "warmup": max(3, args.warmup), "ms_per_step": keep["total_ms"] / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 dense pass, f64 on seed candidates",
             "data": "synthetic", "mpixel_per_s": fps * cfg.npix / 1e6,
+            "step_ms_median": res["step_ms_median"], "step_ms_best": res["step_ms_best"],
             "config": {"workload": workload_name(cfg), "cm_mode": args.cm_mode, "hit_capacity": keep["cap"],
                        "hits_per_frame": res["hits_per_frame"], "l2": res["l2"],
                        "sharding": "each rank processes its own full set of frames; no collective on the data path",
