@@ -803,7 +803,9 @@ int enqueue(pdp_ctx *c, const uint16_t *raw, int n, cudaStream_t st, const pdp_o
     }
     if (!c->cplan[which].ok) which = 0;
     const bool can = c->cplan[which].ok;
-    const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 2 * n >= c->num_sms));
+    // measured crossover (configs 0, 1, 4): the frame-owner kernel wins from about 24 frames on (6 n >= SMs); below
+    // that a frame's bands have to be spread over several CTAs, which only the look-back kernel does
+    const bool use_chain = can && (c->kernel_override == 2 || (c->kernel_override == 0 && 6 * n >= c->num_sms));
     if (c->kernel_override == 2 && !can)
       return fail(c, PDP_E_GEOMETRY, "pdp_debug_set(kernel=2): the throughput kernel does not support this geometry");
     if (use_chain) return enqueue_chain(c, c->cplan[which], raw, n, st, o, keep_cm);
