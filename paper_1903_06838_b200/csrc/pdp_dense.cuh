@@ -12,6 +12,11 @@
 
 namespace pdp {
 
+template <bool B>
+struct BoolTag {
+  static constexpr bool value = B;
+};
+
 constexpr int kDenseThreads = 512;
 constexpr int kDenseRing = 4;     // frames in flight per warp
 
@@ -127,30 +132,44 @@ __global__ void __launch_bounds__(kDenseThreads, 1) pdp_dense_kernel(const DPara
         const float tsum = group_sum<32>(s0);
         c = __fdiv_rn(tsum, fmaxf(n, k.sqrtS));
       }
-      // divide by the single-photon gain and round to the nearest integer
+      // divide by the single-photon gain and round to the nearest integer.  rint() by the magic number
+      // 1.5 * 2^23 (round-half-even for |x| < 2^22; the integer is read from the sum's mantissa: no F2I / FRND, both
+      // quarter-rate); a quotient within 2e-3 of a rounding boundary, or a value within 1e-2 ADU of the zeroing
+      // threshold, is decided in double, in the oracle's order.
       int fsum = 0;
+      constexpr float kMagic = 12582912.f;
+      auto count_pixels = [&](auto zb_tag) {
+        constexpr bool kZero = decltype(zb_tag)::value;
 #pragma unroll
-      for (int j = 0; j < N; ++j) {
-        const float v2 = a[j] - c;
-        const float ratio = v2 * k.inv_Eph;
-        float r = rintf(ratio);
-        // close to a rounding boundary or to the zeroing threshold: decide in double, in the oracle's order
-        if (fabsf(ratio - floorf(ratio) - 0.5f) < 2e-3f || fabsf(v2 - k.zero_below) < 1e-2f) {
-          const size_t gi = off + j;
-          if (lane * N + j < k.S) {
-            const double x = ((double)__ldg(k.raw + (size_t)f * npix + gi) - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - (double)c;
-            double q = x * k.dinv_E_ph;                    // a double division is a ~130-450 cycle sequence: see photon_count()
-            if (fabs(q - floor(q) - 0.5) < 1e-9) q = exact_ratio(x, k.dE_ph);
-            const double rr = rint(q);
-            r = x < k.dzero_below ? 0.f : (float)rr;
+        for (int j = 0; j < N; ++j) {
+          const float v2 = a[j] - c;
+          const float ratio = fmaxf(v2 * k.inv_Eph, -0.25f);   // every quotient below -0.25 counts 0 photons (and padding is -3e38)
+          const float y = ratio + kMagic;
+          const float r = y - kMagic;
+          int n_px = __float_as_int(y) - __float_as_int(kMagic);
+          bool near = fabsf(ratio - r) > 0.498f || !(ratio < 2097152.f);   // (the magic number holds below 2^22)
+          if constexpr (kZero) near = near || fabsf(v2 - k.zero_below) < 1e-2f;
+          if (near) {
+            const size_t gi = off + j;
+            if (lane * N + j < k.S) {
+              const double x = ((double)__ldg(k.raw + (size_t)f * npix + gi) - (double)__ldg(k.ped + gi)) * __ldg(k.rg64 + gi) - (double)c;
+              double q = x * k.dinv_E_ph;                    // a double division is a ~130-450 cycle sequence: see photon_count()
+              if (fabs(q - floor(q) - 0.5) < 1e-9) q = exact_ratio(x, k.dE_ph);
+              const double rr = rint(q);
+              n_px = x < k.dzero_below ? 0 : (rr > 0.0 ? (rr > 2147483647.0 ? 2147483647 : (int)rr) : 0);
+            } else {
+              n_px = 0;   // padding beyond the segment
+            }
+          } else if constexpr (kZero) {
+            if (v2 < k.zero_below) n_px = 0;
           }
-        } else if (v2 < k.zero_below) {
-          r = 0.f;
+          n_px = max(n_px, 0);
+          acc[j] += (uint32_t)n_px;
+          fsum += n_px;
         }
-        const int n_px = r > 0.f ? (int)r : 0;
-        acc[j] += (uint32_t)n_px;
-        fsum += n_px;
-      }
+      };
+      if (k.zero_below > -3.0e38f) count_pixels(BoolTag<true>{});
+      else count_pixels(BoolTag<false>{});
       if (k.partial_totals) {
         const int ft = __reduce_add_sync(FULL, fsum);
         if (lane == 0 && ft) atomicAdd(&tot[f], (uint32_t)ft);   // shared memory
